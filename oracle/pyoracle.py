@@ -73,7 +73,16 @@ def graph_get(L, idx):
 
 
 def all_graphs(L):
-    return [graph_get(L, i) for i in range(graph_count(L))]
+    n = graph_count(L)
+    arr = (OracleGraph * n)()
+    if lib().oracle_graph_list(L, arr) != n:
+        raise RuntimeError("oracle_graph_list")
+    out = []
+    for i in range(n):
+        g = OracleGraph()
+        C.memmove(C.byref(g), C.byref(arr[i]), C.sizeof(OracleGraph))
+        out.append(g)
+    return out
 
 
 def graph_class(g):

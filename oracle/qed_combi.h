@@ -74,13 +74,14 @@ static int graph_init(Graph *g, int L, int e, const int *ca, const int *cb) {
 }
 
 /* ---- canonical enumeration: ascending e, then lexicographic sorted chord list ---- */
-typedef struct { int L, e, count, want_idx, found; int target_a[MAXL], target_b[MAXL], target_e, match_idx; int out_a[MAXL], out_b[MAXL], out_e; } EnumCtx;
+typedef struct { int *list_e, *list_a, *list_b; int L, e, count, want_idx, found; int target_a[MAXL], target_b[MAXL], target_e, match_idx; int out_a[MAXL], out_b[MAXL], out_e; } EnumCtx;
 
 static void enum_rec(EnumCtx *c, int *used, int k, int *a, int *b) {
   int L = c->L, npos = 2 * L + 1;
   if (k == L) {
     Graph g;
     if (graph_init(&g, L, c->e, a, b) != 0) return;
+    if (c->list_e) { c->list_e[c->count] = c->e; memcpy(c->list_a + c->count * MAXL, a, sizeof(int) * L); memcpy(c->list_b + c->count * MAXL, b, sizeof(int) * L); }
     if (c->want_idx == c->count) { c->found = 1; c->out_e = c->e; memcpy(c->out_a, a, sizeof(int) * L); memcpy(c->out_b, b, sizeof(int) * L); }
     if (c->target_e == c->e && memcmp(c->target_a, a, sizeof(int) * L) == 0 && memcmp(c->target_b, b, sizeof(int) * L) == 0) c->match_idx = c->count;
     c->count++;

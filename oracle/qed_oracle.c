@@ -106,6 +106,17 @@ int oracle_graph_get(int L, int idx, oracle_graph *out) {
   for (int i = 0; i < L; i++) { out->chord_a[i] = g.a[i]; out->chord_b[i] = g.b[i]; }
   return 0;
 }
+/* all valid graphs of order L in canonical order; out must hold oracle_graph_count(L) entries */
+int oracle_graph_list(int L, oracle_graph *out) {
+  if (L < 1 || L > MAXL) return -1;
+  int n = graph_count(L);
+  int *le = (int *)malloc(sizeof(int) * n), *la = (int *)malloc(sizeof(int) * n * MAXL), *lb = (int *)malloc(sizeof(int) * n * MAXL);
+  EnumCtx c; memset(&c, 0, sizeof c); c.want_idx = -1; c.target_e = -1; c.list_e = le; c.list_a = la; c.list_b = lb;
+  enum_run(&c, L);
+  for (int i = 0; i < n; i++) { memset(&out[i], 0, sizeof out[i]); out[i].loops = L; out[i].ext_pos = le[i]; for (int k = 0; k < L; k++) { out[i].chord_a[k] = la[i * MAXL + k]; out[i].chord_b[k] = lb[i * MAXL + k]; } }
+  free(le); free(la); free(lb);
+  return n;
+}
 static int to_graph(const oracle_graph *og, Graph *g) {
   int a[MAXL], b[MAXL];
   if (og->loops < 1 || og->loops > MAXL) return -1;

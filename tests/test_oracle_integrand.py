@@ -1,0 +1,211 @@
+"""Pins of the oracle's integrand (forest-like formula, operators, parametric form). Not GPU.
+
+What fixes the numbers: PAPER.md:46 (A1^(2)=1/2), BASELINE.json north_star (2-loop sum without
+lepton loops = -0.344166), closed forms of the 1-loop pieces, identities of the operators.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from conftest import read_golden
+
+PAPER = {r[0]: float(r[1]) for r in read_golden("paper_values.txt")}
+
+
+def _gamma(po, mu):
+    ri = np.zeros(32)
+    po.lib().oracle_dense_gamma(mu, po._p(ri, __import__("ctypes").c_double))
+    return (ri[0::2] + 1j * ri[1::2]).reshape(4, 4)
+
+
+def _functionals(po, X, Y=None):
+    import ctypes as C
+    Xri = np.zeros(128)
+    Xri[0::2], Xri[1::2] = X.real.ravel(), X.imag.ravel()
+    Yp = None
+    if Y is not None:
+        Yri = np.zeros(512)
+        Yri[0::2], Yri[1::2] = Y.real.ravel(), Y.imag.ravel()
+        Yp = po._p(Yri, C.c_double)
+    out = np.zeros(6)
+    po.lib().oracle_functionals(po._p(Xri, C.c_double), Yp, po._p(out, C.c_double))
+    return out[0] + 1j * out[1], out[2] + 1j * out[3], out[4] + 1j * out[5]   # L, U_V, A
+
+
+def test_dirac_algebra(po):
+    g = [_gamma(po, mu) for mu in range(4)]
+    eta = np.diag([1.0, -1, -1, -1])
+    for mu in range(4):
+        for nu in range(4):
+            assert np.allclose(g[mu] @ g[nu] + g[nu] @ g[mu], 2 * eta[mu, nu] * np.eye(4))
+    # gamma^mu gamma^a gamma_mu = -2 gamma^a ; gamma^mu gamma^a gamma^b gamma_mu = 4 g^{ab}
+    for a in range(4):
+        assert np.allclose(sum(eta[m, m] * g[m] @ g[a] @ g[m] for m in range(4)), -2 * g[a])
+        for b in range(4):
+            assert np.allclose(sum(eta[m, m] * g[m] @ g[a] @ g[b] @ g[m] for m in range(4)), 4 * eta[a, b] * np.eye(4))
+
+
+def test_operator_identities(po):
+    """DESIGN.md O4 / P12: on Gamma^mu = a g^mu + b p^mu + c pslash p^mu + d [pslash, g^mu] (p=(1,0,0,0)):
+    U -> a, L -> a+b+c; A vanishes on g^mu, gives 1 on i sigma^{mu nu} q_nu/2m and -1 on p^mu/m"""
+    g = [_gamma(po, mu) for mu in range(4)]
+    p = np.array([1.0, 0, 0, 0])
+    ps = g[0]
+    I4 = np.eye(4)
+    Xg = np.array(g)
+    Xp = np.array([p[mu] * I4 for mu in range(4)])
+    Xpp = np.array([p[mu] * ps for mu in range(4)])
+    Xd = np.array([ps @ g[mu] - g[mu] @ ps for mu in range(4)])
+    for X, (wl, wu) in ((Xg, (1, 1)), (Xp, (1, 0)), (Xpp, (1, 0)), (Xd, (0, 0))):
+        l, u, _ = _functionals(po, X)
+        assert abs(l - wl) < 1e-14 and abs(u - wu) < 1e-14
+    assert abs(_functionals(po, Xg)[2]) < 1e-14
+    assert abs(_functionals(po, Xp)[2] - (-1.0)) < 1e-14          # p^mu = m g^mu - i sigma q/2 between spinors
+    # Gamma^mu = i sigma^{mu nu} q_nu / 2 : X = 0, Y^{mu nu} = i sigma^{mu nu}/2 = -(1/4)[g^mu, g^nu]
+    eta = np.diag([1.0, -1, -1, -1])
+    Y = np.zeros((4, 4, 4, 4), complex)
+    for mu in range(4):
+        for nu in range(4):
+            Y[mu, nu] = -0.25 * (g[mu] @ g[nu] - g[nu] @ g[mu])
+    assert abs(_functionals(po, np.zeros((4, 4, 4), complex), Y)[2] - 1.0) < 1e-14
+
+
+def test_one_loop_pointwise_closed_form(po):
+    """configs[0]: f = z_gamma/(z_e1+z_e2) on the simplex"""
+    d = po.Diagram(po.OracleGraph.make(1, 1, [(0, 2)]))
+    z = np.random.default_rng(0).dirichlet([1, 1, 1], 2000)
+    r = d.eval_z(z, wide=True)
+    want = z[:, 2] / (z[:, 0] + z[:, 1])
+    assert np.allclose(r["f64"], want, rtol=1e-13) and np.allclose(r["fwide"], want, rtol=1e-15)
+
+
+def test_one_loop_quadrature_and_mc(po):
+    d = po.Diagram(po.OracleGraph.make(1, 1, [(0, 2)]))
+    # brute-force midpoint quadrature of int dz_e1 dz_gamma f on the triangle (P5)
+    n = 400
+    h = 1.0 / n
+    pts, wts = [], []
+    for i in range(n):
+        for j in range(n - i):
+            a, b = (i + 1 / 3) * h, (j + 1 / 3) * h
+            pts.append((a, 1 - a - b, b)); wts.append(h * h / 2)
+            if j < n - i - 1:
+                a, b = (i + 2 / 3) * h, (j + 2 / 3) * h
+                pts.append((a, 1 - a - b, b)); wts.append(h * h / 2)
+    val = float(np.dot(d.eval_z(np.array(pts))["f64"], wts))
+    assert abs(val - PAPER["A1_2"]) < 2e-3
+    s1, s2, _ = d.integrate(0, 400000, 1, 0)
+    m, e = po.estimate(s1, s2, 400000)
+    assert abs(m - PAPER["A1_2"]) < 4 * e and e < 2e-3
+
+
+def test_one_loop_self_energy_piece_closed_form(po):
+    """O5 worked piece: gamma^a (A pslash + m) gamma_a = 4m - 2 A pslash  =>  a = -1, b = A/2,
+    A = z_g/(z_e+z_g), U = z_e+z_g, V = z_e^2/(z_e+z_g)"""
+    d = po.Diagram(po.OracleGraph.make(2, 1, [(0, 4), (2, 3)]))
+    child = [k for k, (sub, op, ch) in enumerate(d.nodes()) if sub == 0][0]
+    z = np.random.default_rng(3).dirichlet([1] * 6)
+    v, U, V = d.node_value(child, z)
+    ze, zg = z[2], z[5]
+    assert abs(v[0, 0] + 1.0) < 1e-14 and abs(v[1, 0] - 0.5 * zg / (ze + zg)) < 1e-14
+    assert np.all(v[:, 1:] == 0)
+    assert abs(U - (ze + zg)) < 1e-15 and abs(V - ze * ze / (ze + zg)) < 1e-15
+
+
+def test_two_loop_sum(po):
+    """north_star pin: sum over the 6 two-loop graphs = -0.344166 (here 4e5 points per graph; the
+    high-statistics run is stored in tests/golden/oracle_two_loop_mc.txt)"""
+    n = 400000
+    tot, var = 0.0, 0.0
+    vals = {}
+    for g in po.all_graphs(2):
+        d = po.Diagram(g)
+        s1, s2, _ = d.integrate(0, n, 2, 0)
+        m, e = po.estimate(s1, s2, n)
+        vals[g.key()] = (m, e)
+        tot += m; var += e * e
+    assert abs(tot - PAPER["A1_4_no_lepton_loops"]) < 4 * math.sqrt(var)
+    assert math.sqrt(var) < 0.01
+    # mirror pairs agree (P7, statistically)
+    for g in po.all_graphs(2):
+        a, b = vals[g.key()], vals[po.graph_mirror(g).key()]
+        assert abs(a[0] - b[0]) < 4.5 * math.hypot(a[1], b[1])
+
+
+def test_two_loop_golden_high_statistics():
+    """the stored high-statistics oracle run (written by tests/golden/make_oracle_golden.py, oracle only)"""
+    rows = read_golden("oracle_two_loop_mc.txt")
+    tot = sum(float(r[-2]) for r in rows)
+    err = math.sqrt(sum(float(r[-1]) ** 2 for r in rows))
+    assert err < 1.5e-3
+    assert abs(tot - PAPER["A1_4_no_lepton_loops"]) < 3.5 * err
+
+
+def _line_perm_for_mirror(L):
+    # electron line t -> 2L-1-t ; photons: chords sorted by a get re-sorted in the mirror graph
+    return L
+
+
+@pytest.mark.parametrize("L,idxs", [(2, range(6)), (3, [0, 7, 13, 22, 31, 49])])
+def test_mirror_identity_pointwise(po, L, idxs):
+    """P7: f_G(z) = f_mirror(G)(pi z) with pi the induced line permutation"""
+    rng = np.random.default_rng(5)
+    for i in idxs:
+        g = po.graph_get(L, i)
+        m = po.graph_mirror(g)
+        d, dm = po.Diagram(g), po.Diagram(m)
+        z = rng.dirichlet([1.0] * (3 * L), 40)
+        zm = np.zeros_like(z)
+        for t in range(2 * L):
+            zm[:, 2 * L - 1 - t] = z[:, t]
+        mch = m.chords()
+        for k, (a, b) in enumerate(g.chords()):
+            zm[:, 2 * L + mch.index((2 * L - b, 2 * L - a))] = z[:, 2 * L + k]
+        f, fm = d.eval_z(z, wide=True)["fwide"], dm.eval_z(zm, wide=True)["fwide"]
+        assert np.allclose(f, fm, rtol=1e-11, atol=1e-13)
+
+
+@pytest.mark.parametrize("L,idx", [(2, 1), (2, 3), (2, 0), (3, 0), (3, 7), (3, 8), (3, 9), (3, 18), (3, 29), (3, 38)])
+def test_subtractions_cancel_pointwise(po, L, idx):
+    """P10 / PAPER.md:11: scaling all lines of a divergent subgraph by rho, f*rho^|s| must vanish with rho
+    although individual terms of the forest formula do not"""
+    g = po.graph_get(L, idx)
+    d = po.Diagram(g)
+    subs = d.subgraphs()
+    assert subs
+    z0 = np.random.default_rng(idx).dirichlet([1.0] * d.M)
+    chords = g.chords()
+    for (lo, hi, ty) in subs:
+        lines = list(range(lo, hi)) + [2 * L + k for k, (a, b) in enumerate(chords) if lo <= a and b <= hi]
+        vals, tmax = [], []
+        for rho in (1e-2, 1e-3, 1e-4):
+            z = z0.copy(); z[lines] *= rho; z /= z.sum()
+            r = d.eval_z(z, wide=True, want_terms=True)
+            vals.append(abs(r["fwide"][0]) * rho ** len(lines))
+            tmax.append(np.max(np.abs(r["terms"][0])) * rho ** len(lines))
+        assert vals[1] < 0.5 * vals[0] + 1e-300 and vals[2] < 0.5 * vals[1] + 1e-300, (subs, (lo, hi), vals)
+        assert tmax[2] > 0.05 * tmax[0]                 # a single term alone does not fall off
+
+
+def test_top_grade_vanishes_under_A_and_LmU(po):
+    """O4: the grade c = L_H part of a piece without insertions is ~ gamma^mu and is killed by A and (L-U):
+    pruning it (prune=1) must not change f"""
+    for (L, i) in ((2, 3), (2, 2), (3, 12), (3, 40)):
+        g = po.graph_get(L, i)
+        z = np.random.default_rng(i).dirichlet([1.0] * (3 * L), 20)
+        a = po.Diagram(g, prune=1).eval_z(z)["f64"]
+        b = po.Diagram(g, prune=0).eval_z(z)["f64"]
+        assert np.allclose(a, b, rtol=1e-13, atol=1e-15)
+
+
+def test_estimate_independent_of_deg(po):
+    """P11: any positive Deg table gives an unbiased estimate"""
+    g = po.OracleGraph.make(2, 2, [(0, 4), (1, 3)])
+    res = []
+    for fl, cap in ((0.5, 1e30), (0.75, 1.0), (0.3, 2.0)):
+        d = po.Diagram(g, deg_floor=fl, deg_cap=cap)
+        s1, s2, _ = d.integrate(0, 300000, 7, 0)
+        res.append(po.estimate(s1, s2, 300000))
+    for (m1, e1) in res[1:]:
+        assert abs(m1 - res[0][0]) < 4.5 * math.hypot(e1, res[0][1])
