@@ -1,0 +1,136 @@
+/* include/mcqed.h — C ABI of libmcqed.so: the data-parallel Monte Carlo hot path of
+ * S. Volkov, "Numerical calculation of 5-loop QED contributions to the electron anomalous magnetic
+ * moment" (arXiv:1905.08007; PAPER.md), hand-written CUDA for sm_100a.
+ *
+ * The path (PAPER.md:9-13 items (i)-(iii)): for one Feynman graph without lepton loops
+ * and per sample point
+ *   a1-a3  draw z on the simplex from the graph's own Hepp-sector density, Eq.(1),
+ *          with a Philox4x32-10 counter stream;
+ *   a4     build the loop matrix of every piece of every forest term and derive U, B_ij/U, the
+ *          scalar currents and V in binary64;
+ *   a5-a6  evaluate the Feynman-parametric integrand together with every subtraction term of the
+ *          forest-like formula so that IR and UV divergences cancel point by point;
+ *   a7     weight by f/p and accumulate sum and sum of squares;
+ *   a8     re-evaluate points flagged for round-off in double-double.
+ * Every step runs in CUDA kernels of this library; there is no CPU fallback: every entry point
+ * that touches the device returns MC_ECUDA when no CUDA device / driver is usable.
+ *
+ * Conventions. All functions return 0 (MC_OK) or a negative error code; nothing throws across the
+ * boundary; no global state; handles are thread-safe for concurrent reads. "HOST" / "DEVICE" says
+ * where a pointer must live. Line index convention (R1): electron line t (joining path
+ * positions t,t+1) has index t, photon i (chords sorted by their first end) has index 2L+i; M=3L.
+ */
+#ifndef MCQED_H
+#define MCQED_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MC_OK 0
+#define MC_EINVAL (-1)  /* not a valid graph (no perfect matching, chord on the external vertex, a line not
+                           covered => not 1PI), bad argument, user forests disagree with the enumeration */
+#define MC_ENOMEM (-2)
+#define MC_ECUDA (-3)   /* CUDA runtime error or no device */
+#define MC_ELIMIT (-4)  /* graph exceeds a compiled-in limit */
+
+typedef struct mc_diagram mc_diagram; /* opaque; owns its host and device tables */
+
+/* A vertex graph without lepton loops: an open electron path with positions
+ * 0..2*loops; position ext_pos carries the external photon; the other positions are joined in
+ * pairs by `loops` photon chords. HOST, caller-owned, read during the call only. */
+typedef struct {
+  int32_t loops;                  /* L, 1..5 */
+  int32_t ext_pos;                /* e, 1..2L-1 */
+  int32_t chord_a[5], chord_b[5]; /* chord ends, any order; must form a perfect matching of the positions != e */
+} mc_graph;
+
+/* Optional cross-check of the UV-divergent subgraphs and forests. NULL => the
+ * library enumerates them itself. If given, they must equal the library's own enumeration
+ * (subgraphs ascending (lo,hi); forests = ascending bitmasks over the subgraphs, the empty forest
+ * included), else MC_EINVAL. HOST. */
+typedef struct {
+  int32_t n_sub; const int32_t *seg_lo, *seg_hi;
+  int32_t n_forest; const uint32_t *forest_mask;
+} mc_forests;
+
+/* NULL => defaults {0.5, 1e30, 4096.0, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5);
+ * cond_max: a point is flagged for double-double re-evaluation when
+ * sum_terms sum_grades |contribution| > cond_max * |f| or anything is non-finite (O8);
+ * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0). */
+typedef struct { double deg_floor, deg_cap, cond_max; uint32_t flags; } mc_options;
+
+/* Host-side preparation of one diagram (not on the timed path): validates the graph, enumerates
+ * subgraphs/forests/terms (forest-like formula, O1), builds Deg and the sector-sum table
+ * (Eq.(1)), the numerator tables of every piece, and uploads them to the current CUDA device.
+ * *out is owned by the caller and released with mc_free_diagram. */
+int mc_prepare_diagram(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out);
+
+/* Same as mc_prepare_diagram but builds host tables only (no CUDA call): for introspection and CPU
+ * tests of the host logic. Such a handle is rejected (MC_EINVAL) by mc_integrate / mc_eval_points. */
+int mc_prepare_diagram_host(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out);
+
+void mc_free_diagram(mc_diagram *);
+
+/* Class (k,m,n) of PAPER.md:104; number of formula terms; algorithmic flop per sample point
+ * (2 per stored numerator monomial + the a1-a4,a6 estimate of DESIGN.md §5); device table bytes.
+ * Any output pointer may be NULL. HOST. */
+int mc_diagram_info(const mc_diagram *, int32_t *k, int32_t *m, int32_t *n, int32_t *n_terms,
+                    int64_t *flop_per_sample, int64_t *table_bytes);
+
+/* Canonical index of the graph among the valid graphs of its loop order (ascending e, then
+ * lexicographic sorted chord list; A19) — it is the 4th Philox counter word. */
+int mc_diagram_id(const mc_diagram *, int32_t *id);
+
+/* Introspection (HOST outputs, caller-allocated, any may be NULL; returns the count):
+ * subgraphs (lo,hi,type 0=S/1=V), forests (bitmasks), terms (forest, gprime index or -1, sign). */
+int mc_diagram_subgraphs(const mc_diagram *, int32_t *lo, int32_t *hi, int32_t *type, int32_t cap);
+int mc_diagram_forests(const mc_diagram *, uint32_t *mask, int32_t cap);
+int mc_diagram_terms(const mc_diagram *, uint32_t *forest, int32_t *gprime, int32_t *sign, int32_t cap);
+/* Sampler tables of Eq.(1): deg and Z have 2^M entries, C is the normalisation. HOST outputs. */
+int mc_diagram_sampler_tables(const mc_diagram *, double *deg, double *Z, double *C);
+
+/* Host copy of the device table blob (layout: csrc/device_layout.h), for format tests. Returns the
+ * number of 8-byte words; copies min(words, cap) words into out (may be NULL). HOST. */
+int64_t mc_diagram_blob(const mc_diagram *, uint64_t *out, int64_t cap);
+
+/* The hot path. Processes sample indices first_sample .. first_sample+n_samples-1 of this diagram
+ * (the Philox counter is the sample index, so calls with disjoint ranges are independent and
+ * additive: that is also the checkpoint/resume story). Asynchronous on `cuda_stream`
+ * (a cudaStream_t; NULL = legacy default stream). out_* are DEVICE pointers, one element each,
+ * accumulated into (+=): sum of w=f/p, sum of w^2, number of points re-evaluated in double-double,
+ * number of points dropped because even the double-double value was non-finite (their w is 0). */
+int mc_integrate(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                 double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped);
+
+/* Same computation with HOST outputs: allocates nothing persistent, copies the four results back
+ * and synchronises the stream. For end-to-end use without touching device memory. */
+int mc_integrate_host(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                      double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
+
+/* Parity hook: per-point values for comparison with the oracle. DEVICE outputs, any may be NULL:
+ * z_out n*M (row = point, column = line index), order_out n*M (the Hepp sector j_1..j_M),
+ * p_out n (density), f_out n (value used by mc_integrate: binary64, or double-double rounded to
+ * binary64 if flagged), f64_out n (plain binary64 value), cond_out n (sum|contrib|/|f|), flag_out n. */
+int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
+                   double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out,
+                   double *cond_out, uint8_t *flag_out);
+
+/* Integrand at caller-supplied points (DEVICE z_in n*M): f64_out, fdd_out (double-double evaluation
+ * rounded to binary64), cond_out; any output may be NULL. */
+int mc_eval_z(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream,
+              double *f64_out, double *fdd_out, double *cond_out);
+
+/* Number of kernels this library has launched in the calling process (for gpu_launches in bench.py). */
+unsigned long long mc_kernel_launch_count(void);
+
+/* FP64 FMA throughput micro-benchmark: runs `iters` dependent-chain rounds of 8
+ * independent DFMA chains per thread on all SMs and returns achieved FLOP/s in *flops (HOST). */
+int mc_fp64_peak(int iters, void *cuda_stream, double *flops, double *ms);
+
+const char *mc_strerror(int code);
+const char *mc_version(void);
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -27,9 +27,9 @@ static void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
-/* uniform in (0,1), exact in binary64: ((x>>5)*2^26 + (y>>6) + 0.5) * 2^-53 */
+/* uniform in (0,1), exact in binary64 (52 random bits): ((x>>6)*2^26 + (y>>6) + 0.5) * 2^-52 */
 static double u01_from_words(uint32_t x, uint32_t y) {
-  return ((double)(x >> 5) * 67108864.0 + (double)(y >> 6) + 0.5) * (1.0 / 9007199254740992.0);
+  return ((double)(x >> 6) * 67108864.0 + (double)(y >> 6) + 0.5) * (1.0 / 4503599627370496.0);
 }
 /* uniform number r of sample idx of diagram diag_id: Philox block r/2, words (0,1) or (2,3) */
 static double sample_uniform(uint64_t idx, uint32_t diag_id, uint64_t seed, int r) {

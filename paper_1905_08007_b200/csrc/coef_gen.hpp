@@ -1,0 +1,244 @@
+// coef_gen.hpp — numerator tables of one piece under one operator (host, prepare time).
+// Product code (libmcqed.so); shares nothing with oracle/.
+//
+// DESIGN.md O3-O5. In the rest frame p=(m,0,0,0), m=1, Dirac representation, every factor of the
+// gamma string of a piece is a generalised permutation matrix (one non-zero entry i^k per column)
+// or a block projector:
+//     line t, unpaired :  (A_t pslash + m) = g_t (P+ + r_t P-),   g_t = 2-x_t, r_t = x_t/g_t, x_t = 1-A_t
+//     kappaslash, vertices, free vertex, q-slot : gamma^rho
+// So for fixed Lorentz indices a basis spinor follows ONE path through the string, picking up a
+// phase, and the block (upper/lower) it is in at an unpaired line decides P+ or P-. The coefficient
+// of a monomial is the signed count of such paths: exact integer arithmetic, no matrix products.
+//
+// Output format ("families"): for a fixed role of every slot
+// {binary line, insertion a-part, insertion b*p-part, Wick-paired, q-slot} and a fixed P+/P- choice
+// of the outer binary lines, ALL pairings of the paired slots times ALL 2^kd choices of the inner
+// binary lines, as one dense coefficient block the kernel evaluates with static register indexing.
+#pragma once
+#include <atomic>
+#include <complex>
+#include <thread>
+
+#include "host_model.hpp"
+
+namespace mq {
+
+struct Family {
+  int c = 0, kd = 0, pattern = 0, out = 0;
+  std::vector<uint8_t> paired, inner;
+  std::vector<uint8_t> scal;       // kind<<4 | slot
+  std::vector<double> coef;        // stream order (see device_layout.h)
+  int64_t nonzero = 0;
+};
+struct TableBuild { int nout = 1; std::vector<Family> fams; int64_t n_stored = 0, n_nonzero = 0; };
+
+namespace detail {
+// column action of gamma^rho on basis spinor s: gamma^rho e_s = i^PH e_DST   (Dirac representation)
+static const int8_t G_DST[4][4] = {{0, 1, 2, 3}, {3, 2, 1, 0}, {3, 2, 1, 0}, {2, 3, 0, 1}};
+static const int8_t G_PH[4][4] = {{0, 0, 2, 2}, {2, 2, 0, 0}, {3, 1, 1, 3}, {2, 0, 0, 2}};
+
+enum { W_FIX, W_OPEN, W_CLOSE, W_BIN, W_G0 };
+struct WElem { uint8_t type, arg; };
+
+struct Variant {               // one trace of the operator functional
+  int freeIdx, qIdx, prepend, append;     // Lorentz index of the free vertex / q-slot; extra gamma applied first / last (-1 none)
+  std::complex<double> w[4];              // weight per start spinor (0 = not used)
+  int out;
+};
+
+struct Walker {
+  const WElem *el; int n; int start;
+  int8_t rho[16];
+  std::complex<double> weight;
+  std::complex<double> *acc;   // [2^k]
+  void go(int pos, int s, int ph, uint32_t sig) {
+    for (; pos < n; pos++) {
+      const WElem e = el[pos];
+      switch (e.type) {
+        case W_FIX: ph += G_PH[e.arg][s]; s = G_DST[e.arg][s]; break;
+        case W_G0: ph += (s >= 2) ? 2 : 0; break;
+        case W_BIN: sig |= (uint32_t)(s >= 2) << e.arg; break;
+        case W_CLOSE: { int r = rho[e.arg]; ph += G_PH[r][s] + (r ? 2 : 0); s = G_DST[r][s]; break; }
+        case W_OPEN:
+          for (int r = 0; r < 4; r++) { rho[e.arg] = (int8_t)r; go(pos + 1, G_DST[r][s], ph + G_PH[r][s], sig); }
+          return;
+      }
+    }
+    if (s != start) return;
+    static const std::complex<double> I4[4] = {{1, 0}, {0, 1}, {-1, 0}, {0, -1}};
+    acc[sig] += weight * I4[ph & 3];
+  }
+};
+
+inline std::vector<Variant> variantsFor(int op, bool sType, bool hasQ) {
+  using cd = std::complex<double>;
+  std::vector<Variant> v;
+  const cd i(0, 1);
+  auto L = [&](double sc) { v.push_back({0, -1, -1, -1, {cd(0.5 * sc), cd(0.5 * sc), 0, 0}, 0}); };
+  auto U = [&](double sc) { for (int j = 1; j <= 3; j++) v.push_back({j, -1, -1, j, {cd(-sc / 12), cd(-sc / 12), cd(-sc / 12), cd(-sc / 12)}, 0}); };
+  if (sType) {            // U on an electron self-energy: a = Tr S/4, b = Tr[gamma^0 S]/4
+    v.push_back({-1, -1, -1, -1, {0.25, 0.25, 0.25, 0.25}, 0});
+    v.push_back({-1, -1, -1, 0, {0.25, 0.25, 0.25, 0.25}, 1});
+    return v;
+  }
+  switch (op) {
+    case MQ_OP_L: L(1); break;
+    case MQ_OP_U: U(1); break;
+    case MQ_OP_LMU: L(1); U(-1); break;
+    case MQ_OP_A:
+      if (!hasQ) {        // [ (g2 X1 - X1 g2)_00 - (..)_11 ]/(4i) - (X0_00 + X0_11)/2      (O4)
+        v.push_back({1, -1, -1, 2, {-0.25 * i, 0.25 * i, 0, 0}, 0});
+        v.push_back({1, -1, 2, -1, {0.25 * i, -0.25 * i, 0, 0}, 0});
+        v.push_back({0, -1, -1, -1, {-0.5, -0.5, 0, 0}, 0});
+      } else {            // -i [ Y12_00 - Y12_11 ]
+        v.push_back({1, 2, -1, -1, {-i, i, 0, 0}, 0});
+      }
+      break;
+  }
+  return v;
+}
+
+// all perfect matchings of {0..2c-1} in canonical order: the first free element pairs with every later one
+inline void allPairings(int n2, std::vector<std::vector<std::pair<int, int>>> &out) {
+  std::vector<std::pair<int, int>> cur;
+  std::vector<int> used(n2, 0);
+  std::function<void()> rec = [&]() {
+    int f = 0; while (f < n2 && used[f]) f++;
+    if (f == n2) { out.push_back(cur); return; }
+    used[f] = 1;
+    for (int s = f + 1; s < n2; s++) if (!used[s]) { used[s] = 1; cur.emplace_back(f, s); rec(); cur.pop_back(); used[s] = 0; }
+    used[f] = 0;
+  };
+  rec();
+}
+}  // namespace detail
+
+enum Role : uint8_t { R_BIN, R_INS_A, R_INS_BP, R_PAIRED, R_Q };
+
+struct RoleJob { std::vector<uint8_t> role; int c; bool hasQ; };
+
+inline TableBuild buildTable(const Piece &p, int op, int nthreads) {
+  using namespace detail;
+  TableBuild tb;
+  const bool sType = !p.seg.vertexLike;
+  tb.nout = sType ? 2 : 1;
+  const int nslot = (int)p.slots.size(), nch = (int)p.ownChord.size();
+  int maxc = nslot / 2;
+  if ((op == MQ_OP_A || op == MQ_OP_LMU) && p.nS == 0) maxc = std::min(maxc, nch - 1);  // top grade ~ gamma^mu: killed (O4)
+  // ---- enumerate slot roles ----
+  std::vector<RoleJob> jobs;
+  {
+    std::vector<uint8_t> role(nslot);
+    std::function<void(int, int, bool)> rec = [&](int s, int npaired, bool usedQ) {
+      if (s == nslot) { if (npaired % 2 == 0 && npaired / 2 <= maxc) jobs.push_back({role, npaired / 2, usedQ}); return; }
+      if (!p.slots[s].insertion) { role[s] = R_BIN; rec(s + 1, npaired, usedQ); }
+      else { role[s] = R_INS_A; rec(s + 1, npaired, usedQ); role[s] = R_INS_BP; rec(s + 1, npaired, usedQ); }
+      if (npaired + 1 <= 2 * maxc) { role[s] = R_PAIRED; rec(s + 1, npaired + 1, usedQ); }
+      if (op == MQ_OP_A && !usedQ) { role[s] = R_Q; rec(s + 1, npaired, true); }
+    };
+    rec(0, 0, false);
+  }
+  std::vector<std::vector<std::vector<std::pair<int, int>>>> pairingsOf(maxc + 1);
+  for (int c = 0; c <= maxc; c++) allPairings(2 * c, pairingsOf[c]);
+
+  std::vector<std::vector<Family>> famsOf(jobs.size());
+  std::atomic<size_t> next{0};
+  auto worker = [&]() {
+    std::vector<std::complex<double>> acc;
+    for (;;) {
+      size_t j = next.fetch_add(1);
+      if (j >= jobs.size()) break;
+      const RoleJob &job = jobs[j];
+      std::vector<int> binSlots, pairedSlots, atSlots; int qSlot = -1, pattern = 0;
+      for (int s = 0; s < nslot; s++) {
+        Role r = (Role)job.role[s];
+        if (r == R_BIN) binSlots.push_back(s);
+        if (r == R_PAIRED) pairedSlots.push_back(s);
+        if (r == R_INS_BP) atSlots.push_back(s);
+        if (r == R_Q) qSlot = s;
+        if (p.slots[s].insertion && r != R_INS_A) pattern |= 1 << p.patbit[p.slots[s].child];
+      }
+      const int k = (int)binSlots.size(), c = job.c;
+      const auto &pairings = pairingsOf[c];
+      const size_t nsig = (size_t)1 << k;
+      auto variants = variantsFor(op, sType, job.hasQ);
+      // coefficient matrix [out][pairing][sigma]
+      std::vector<double> cm((size_t)tb.nout * pairings.size() * nsig, 0.0);
+      double pref = 1.0;
+      for (int i = 0; i < nch; i++) pref *= -0.25;
+      for (int i = 0; i < c; i++) pref *= -0.5;
+      std::vector<int> pairIdOfSlot(nslot, -1), binIdx(nslot, -1);
+      for (int b = 0; b < k; b++) binIdx[binSlots[b]] = b;
+      for (size_t pi = 0; pi < pairings.size(); pi++) {
+        std::vector<int> firstOfPair(nslot, 0);
+        for (int q = 0; q < c; q++) {
+          pairIdOfSlot[pairedSlots[pairings[pi][q].first]] = nch + q; firstOfPair[pairedSlots[pairings[pi][q].first]] = 1;
+          pairIdOfSlot[pairedSlots[pairings[pi][q].second]] = nch + q;
+        }
+        for (const Variant &var : variants) {
+          std::vector<WElem> el;
+          if (var.prepend >= 0) el.push_back({W_FIX, (uint8_t)var.prepend});
+          std::vector<int> chordSeen(nch, 0);
+          for (const auto &e : p.elems) {
+            if (e.kind == Piece::VERT_FREE) el.push_back({W_FIX, (uint8_t)var.freeIdx});
+            else if (e.kind == Piece::VERT_CHORD) { el.push_back({(uint8_t)(chordSeen[e.chord] ? W_CLOSE : W_OPEN), (uint8_t)e.chord}); chordSeen[e.chord] = 1; }
+            else {
+              int s = e.slot;
+              switch ((Role)job.role[s]) {
+                case R_BIN: el.push_back({W_BIN, (uint8_t)binIdx[s]}); break;
+                case R_INS_A: break;
+                case R_INS_BP: el.push_back({W_G0, 0}); break;
+                case R_PAIRED: el.push_back({(uint8_t)(firstOfPair[s] ? W_OPEN : W_CLOSE), (uint8_t)pairIdOfSlot[s]}); break;
+                case R_Q: el.push_back({W_FIX, (uint8_t)var.qIdx}); break;
+              }
+            }
+          }
+          if (var.append >= 0) el.push_back({W_FIX, (uint8_t)var.append});
+          for (int a = 0; a < 4; a++) {
+            if (var.w[a] == std::complex<double>(0, 0)) continue;
+            acc.assign(nsig, 0.0);
+            Walker w; w.el = el.data(); w.n = (int)el.size(); w.start = a; w.weight = var.w[a]; w.acc = acc.data();
+            w.go(0, a, 0, 0u);
+            double *dst = &cm[((size_t)var.out * pairings.size() + pi) * nsig];
+            for (size_t sg = 0; sg < nsig; sg++) {
+              // imaginary parts cancel between start spinors / variants; they are dropped after the sum below
+              dst[sg] += pref * acc[sg].real();
+              if (std::abs(acc[sg].imag()) > 0) dst[sg] += 0.0;  // (kept real; imaginary parts checked in tests via parity)
+            }
+          }
+        }
+      }
+      // ---- split into families: inner = last kd binary slots, outer P+/P- fixed ----
+      const int kd = std::min(k, MQ_KD_MAX), ko = k - kd;
+      const size_t ninner = (size_t)1 << kd, half = ninner >> 1;
+      for (int out = 0; out < tb.nout; out++)
+        for (size_t so = 0; so < ((size_t)1 << ko); so++) {
+          Family f; f.c = c; f.kd = kd; f.pattern = pattern; f.out = out;
+          bool any = false;
+          for (size_t pi = 0; pi < pairings.size(); pi++) {
+            const double *src = &cm[((size_t)out * pairings.size() + pi) * nsig];
+            auto at = [&](size_t si) { return src[so | (si << ko)]; };   // outer bits low, inner bits high
+            if (kd == 0) f.coef.push_back(at(0));
+            else for (size_t jj = 0; jj < half; jj++) { f.coef.push_back(at(jj)); f.coef.push_back(at(jj + half)); }
+          }
+          for (double v : f.coef) if (v != 0.0) { any = true; f.nonzero++; }
+          if (!any) continue;
+          for (int s : pairedSlots) f.paired.push_back((uint8_t)s);
+          for (int b = 0; b < kd; b++) f.inner.push_back((uint8_t)binSlots[ko + b]);
+          for (int b = 0; b < ko; b++) if (so >> b & 1) f.scal.push_back((uint8_t)(MQ_SC_R << 4 | binSlots[b]));
+          for (int s : atSlots) f.scal.push_back((uint8_t)(MQ_SC_AT << 4 | s));
+          if (qSlot >= 0) f.scal.push_back((uint8_t)(MQ_SC_AQ << 4 | qSlot));
+          famsOf[j].push_back(std::move(f));
+        }
+    }
+  };
+  int nt = std::max(1, std::min<int>(nthreads, (int)jobs.size()));
+  std::vector<std::thread> pool;
+  for (int t = 1; t < nt; t++) pool.emplace_back(worker);
+  worker();
+  for (auto &t : pool) t.join();
+  for (auto &v : famsOf) for (auto &f : v) { tb.n_stored += (int64_t)f.coef.size(); tb.n_nonzero += f.nonzero; tb.fams.push_back(std::move(f)); }
+  return tb;
+}
+
+}  // namespace mq

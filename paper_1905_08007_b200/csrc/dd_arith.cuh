@@ -1,0 +1,69 @@
+// dd_arith.cuh — double-double arithmetic for the precision-fallback kernel (O8, step a8;
+// PAPER.md:91 "arithmetic with different precisions"). Error-free transformations with FMA
+// (two_sum / two_prod); ~106-bit significand. Device only.
+#pragma once
+#include <cuda_runtime.h>
+
+struct dd {
+  double hi, lo;
+  __device__ __forceinline__ dd() {}
+  __device__ __forceinline__ dd(double h) : hi(h), lo(0.0) {}
+  __device__ __forceinline__ dd(double h, double l) : hi(h), lo(l) {}
+};
+
+__device__ __forceinline__ dd dd_two_sum(double a, double b) {
+  double s = __dadd_rn(a, b), bb = __dadd_rn(s, -a);
+  double e = __dadd_rn(__dadd_rn(a, -__dadd_rn(s, -bb)), __dadd_rn(b, -bb));
+  return dd(s, e);
+}
+__device__ __forceinline__ dd dd_quick_two_sum(double a, double b) {  // |a| >= |b|
+  double s = __dadd_rn(a, b);
+  return dd(s, __dadd_rn(b, -__dadd_rn(s, -a)));
+}
+__device__ __forceinline__ dd dd_two_prod(double a, double b) {
+  double p = __dmul_rn(a, b);
+  return dd(p, __fma_rn(a, b, -p));
+}
+__device__ __forceinline__ dd operator+(dd a, dd b) {   // accurate (IEEE-style) addition
+  dd s = dd_two_sum(a.hi, b.hi), t = dd_two_sum(a.lo, b.lo);
+  s.lo = __dadd_rn(s.lo, t.hi);
+  s = dd_quick_two_sum(s.hi, s.lo);
+  s.lo = __dadd_rn(s.lo, t.lo);
+  return dd_quick_two_sum(s.hi, s.lo);
+}
+__device__ __forceinline__ dd operator-(dd a) { return dd(-a.hi, -a.lo); }
+__device__ __forceinline__ dd operator-(dd a, dd b) { return a + (-b); }
+__device__ __forceinline__ dd operator*(dd a, dd b) {
+  dd p = dd_two_prod(a.hi, b.hi);
+  p.lo = __dadd_rn(p.lo, __fma_rn(a.hi, b.lo, __dmul_rn(a.lo, b.hi)));
+  return dd_quick_two_sum(p.hi, p.lo);
+}
+__device__ __forceinline__ dd operator*(dd a, double b) {
+  dd p = dd_two_prod(a.hi, b);
+  p.lo = __fma_rn(a.lo, b, p.lo);
+  return dd_quick_two_sum(p.hi, p.lo);
+}
+__device__ __forceinline__ dd operator/(dd a, dd b) {
+  double q1 = __ddiv_rn(a.hi, b.hi);
+  dd r = a - b * q1;
+  double q2 = __ddiv_rn(r.hi, b.hi);
+  r = r - b * q2;
+  double q3 = __ddiv_rn(r.hi, b.hi);
+  dd q = dd_quick_two_sum(q1, q2);
+  return q + dd(q3);
+}
+__device__ __forceinline__ dd &operator+=(dd &a, dd b) { a = a + b; return a; }
+__device__ __forceinline__ dd &operator-=(dd &a, dd b) { a = a - b; return a; }
+__device__ __forceinline__ dd &operator*=(dd &a, dd b) { a = a * b; return a; }
+
+// generic helpers so that one templated evaluator serves binary64 and double-double
+__device__ __forceinline__ double mq_fma(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ dd mq_fma(dd a, dd b, dd c) { return a * b + c; }
+__device__ __forceinline__ double mq_fma_c(double coef, double x, double c0, double) { return fma(coef, x, c0); }   // coef*x + c0
+__device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) { return x * coef + dd(c0); }
+__device__ __forceinline__ double mq_to_double(double a) { return a; }
+__device__ __forceinline__ double mq_to_double(dd a) { return a.hi + a.lo; }
+__device__ __forceinline__ double mq_abs(double a) { return fabs(a); }
+__device__ __forceinline__ dd mq_abs(dd a) { return a.hi < 0 ? -a : a; }
+__device__ __forceinline__ bool mq_lt0(double a) { return a < 0; }
+__device__ __forceinline__ bool mq_lt0(dd a) { return a.hi < 0; }

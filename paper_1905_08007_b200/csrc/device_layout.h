@@ -1,0 +1,79 @@
+// device_layout.h — plain-old-data layout of one prepared diagram as the kernels read it.
+// Product code (libmcqed.so). Shares nothing with oracle/.
+//
+// One diagram = one contiguous blob of 8-byte words in HBM:
+//   DevHeader | Z[2^M] | invDeg[2^M] | DevGeom[ngeom] | DevTable[ntable] | DevNode[nnode] | DevTerm[nterm] | streams
+// A "stream" is the numerator table of one (piece, operator): a sequence of families.
+#pragma once
+#include <cstdint>
+
+#define MQ_MAXL 5
+#define MQ_MAXM 15
+#define MQ_MAXSLOT 14
+#define MQ_MAXCHILD 5
+#define MQ_NGRADE 6
+#define MQ_MAXGEOM 96
+#define MQ_MAXNODE 256
+#define MQ_MAXPAT 16      // 2^(max #S-children of a piece)
+#define MQ_KD_MAX 4       // inner dense binary dimensions of a family
+#define MQ_MAXSCAL 12
+
+enum { MQ_OP_A = 0, MQ_OP_U = 1, MQ_OP_L = 2, MQ_OP_LMU = 3 };
+enum { MQ_SLOT_LINE = 0, MQ_SLOT_INS = 1 };
+// scalar-factor kinds in a family header (index into the per-point scalar arrays of the piece)
+enum { MQ_SC_R = 0, MQ_SC_AT = 1, MQ_SC_AQ = 2 };
+
+struct DevSlot {
+  int8_t kind;    // MQ_SLOT_LINE / MQ_SLOT_INS
+  int8_t zline;   // line index of z for a line slot; for an insertion the line before it (routing only)
+  int8_t sgn;     // -1 before the external vertex, +1 after (A' only)
+  int8_t child;   // child index for an insertion, else -1
+  uint32_t eps;   // bit i: own chord i spans this slot
+};
+
+struct DevGeom {
+  int32_t nch, nslot, nchild, nS;         // own chords, momentum slots, children, S-type children
+  int32_t chord_zline[MQ_MAXL];           // photon line index of own chord i
+  DevSlot slot[MQ_MAXSLOT];
+  int8_t child_type[MQ_MAXCHILD];         // 0 = S, 1 = V
+  int8_t child_patbit[MQ_MAXCHILD];       // bit position of an S-child in the compressed pattern, -1 for V
+  int16_t pad;
+  int32_t first_table, ntable;            // tables of this geom are consecutive
+};
+
+struct DevTable {
+  int32_t geom, op, nout, nfam;
+  int32_t first_node, nnode;              // nodes using this table are consecutive
+  int64_t stream_off, stream_words;       // in 8-byte words from the blob start
+  int64_t n_monomials;                    // stored (dense) numerator coefficients
+};
+
+struct DevNode {
+  int32_t table, geom, nchild, nout;
+  int32_t child[MQ_MAXCHILD];
+  int32_t val_off;                        // offset (doubles) of this node's graded value(s) in the per-point array
+  int32_t ngr;                            // grades stored per output
+};
+
+struct DevTerm { int32_t root, sign; };
+
+struct DevHeader {
+  int32_t L, M, diag_id, ngeom, ntable, nnode, nterm, nodeval_len;
+  int32_t max_scal_len, pad0;
+  double C, cond_max;
+  int64_t off_Z, off_invdeg, off_geom, off_table, off_node, off_term, total_words;
+};
+
+// Family header word (uint64), then index bytes, padded to 8 bytes, then the dense coefficients:
+//   bits  0..2  c   (#Wick pairs)              bits  3..5  kd (#inner binary slots)
+//   bits  6..9  pattern (compressed)           bits 10..13 nscal (#extra scalar factors)
+//   bits 14     out (0/1: which output of an S-type piece)
+//   bits 16..31 number of 8-byte words of index bytes that follow
+//   bits 32..63 number of coefficient doubles that follow the index bytes
+// index bytes: 2c paired slot ids | kd inner binary slot ids | nscal x (kind<<4 | slot)
+// coefficients: for every pairing (canonical order) 2^kd values, stored as (lo,hi) pairs for the
+// first Horner level: c[j], c[j+2^(kd-1)], j < 2^(kd-1)   (kd = 0: one value per pairing).
+static inline uint64_t mq_pack_family(int c, int kd, int pattern, int nscal, int out, int idx_words, uint32_t ncoef) {
+  return (uint64_t)c | (uint64_t)kd << 3 | (uint64_t)pattern << 6 | (uint64_t)nscal << 10 | (uint64_t)out << 14 |
+         (uint64_t)idx_words << 16 | (uint64_t)ncoef << 32;
+}

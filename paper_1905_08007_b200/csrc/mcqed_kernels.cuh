@@ -1,0 +1,363 @@
+// mcqed_kernels.cuh — device code of the hot path (steps a1-a8 of DESIGN.md §2), sm_100a.
+// Product code (libmcqed.so); shares nothing with oracle/.
+//
+// Mapping: one thread = one sample point (lanes = points). All threads of a launch work on the same
+// diagram, so every table read (family headers, coefficients, Z/invDeg rows) is warp-uniform and
+// control flow never diverges inside the integrand. Per-point operands that the tables address by
+// index (r_t, A_t, A'_t/g_t, beta_tu/(g_t g_u)) live in shared memory laid out [index][thread]
+// (conflict-free); everything with static indexing lives in registers. FP64 FMA pipe is the roofline.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dd_arith.cuh"
+#include "device_layout.h"
+
+namespace mqk {
+
+struct DiagView {
+  const uint64_t *blob; const DevHeader *h; const double *Z, *invdeg;
+  const DevGeom *geom; const DevTable *tab; const DevNode *node; const DevTerm *term;
+};
+__device__ __forceinline__ DiagView make_view(const uint64_t *blob) {
+  DiagView v; v.blob = blob; v.h = reinterpret_cast<const DevHeader *>(blob);
+  v.Z = reinterpret_cast<const double *>(blob + v.h->off_Z);
+  v.invdeg = reinterpret_cast<const double *>(blob + v.h->off_invdeg);
+  v.geom = reinterpret_cast<const DevGeom *>(blob + v.h->off_geom);
+  v.tab = reinterpret_cast<const DevTable *>(blob + v.h->off_table);
+  v.node = reinterpret_cast<const DevNode *>(blob + v.h->off_node);
+  v.term = reinterpret_cast<const DevTerm *>(blob + v.h->off_term);
+  return v;
+}
+
+// ------------------------------------------------------------------ a1: Philox4x32-10
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; r++) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+__device__ __forceinline__ double u01(uint32_t x, uint32_t y) {   // 52 random bits, strictly inside (0,1), exact
+  return __dmul_rn(__dadd_rn(__dadd_rn(__dmul_rn((double)(x >> 6), 67108864.0), (double)(y >> 6)), 0.5), 1.0 / 4503599627370496.0);
+}
+
+// ------------------------------------------------------------------ a3: deterministic pow (S4)
+// explicit round-to-nearest mul/add only (never contracted) so that the bits equal the oracle's
+__device__ __forceinline__ double det_log2(double u) {
+  uint64_t bits = (uint64_t)__double_as_longlong(u);
+  int ex = (int)((bits >> 52) & 0x7FF) - 1023;
+  double m = __longlong_as_double((long long)((bits & 0x000FFFFFFFFFFFFFull) | 0x3FF0000000000000ull));
+  if (m > 1.4142135623730951) { m = __dmul_rn(m, 0.5); ex += 1; }
+  double s = __ddiv_rn(__dadd_rn(m, -1.0), __dadd_rn(m, 1.0)), s2 = __dmul_rn(s, s);
+  double P = 1.0 / 23.0;
+#define MQ_H(c) P = __dadd_rn(__dmul_rn(P, s2), (c))
+  MQ_H(1.0 / 21.0); MQ_H(1.0 / 19.0); MQ_H(1.0 / 17.0); MQ_H(1.0 / 15.0); MQ_H(1.0 / 13.0); MQ_H(1.0 / 11.0);
+  MQ_H(1.0 / 9.0); MQ_H(1.0 / 7.0); MQ_H(1.0 / 5.0); MQ_H(1.0 / 3.0); MQ_H(1.0);
+#undef MQ_H
+  double lnm = __dmul_rn(__dmul_rn(2.0, s), P);
+  return __dadd_rn((double)ex, __dmul_rn(lnm, 1.4426950408889634));
+}
+__device__ __forceinline__ double det_exp2(double y) {
+  if (y < -1020.0) return 0.0;
+  double n = floor(__dadd_rn(y, 0.5)), r = __dadd_rn(y, -n), w = __dmul_rn(r, 0.6931471805599453);
+  double P = 1.0 / 87178291200.0;
+#define MQ_H(c) P = __dadd_rn(__dmul_rn(P, w), (c))
+  MQ_H(1.0 / 6227020800.0); MQ_H(1.0 / 479001600.0); MQ_H(1.0 / 39916800.0); MQ_H(1.0 / 3628800.0); MQ_H(1.0 / 362880.0);
+  MQ_H(1.0 / 40320.0); MQ_H(1.0 / 5040.0); MQ_H(1.0 / 720.0); MQ_H(1.0 / 120.0); MQ_H(1.0 / 24.0); MQ_H(1.0 / 6.0);
+  MQ_H(0.5); MQ_H(1.0); MQ_H(1.0);
+#undef MQ_H
+  double sc = __longlong_as_double((long long)((uint64_t)((long long)n + 1023) << 52));
+  return __dmul_rn(P, sc);
+}
+
+// ------------------------------------------------------------------ a2+a3: sector walk, coordinates, density (Eq.(1))
+// z[] is written by line index; order[] (optional) gets the sector j_1..j_M; returns p(z)
+template <bool WANT_ORDER>
+__device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, uint64_t seed, double *z, int32_t *order_out) {
+  const int M = v.h->M;
+  const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), i0 = (uint32_t)idx, i1 = (uint32_t)(idx >> 32), dg = (uint32_t)v.h->diag_id;
+  uint32_t mask = (1u << M) - 1;
+  double r[MQ_MAXM]; int8_t ord[MQ_MAXM];
+  double rl = 1.0, pu = 1.0;
+  uint32_t ws[4], wr[4];
+  for (int l = 0; l < M; l++) {
+    int x;
+    if (l == M - 1) x = __ffs(mask) - 1;
+    else {
+      if ((l & 1) == 0) philox4x32_10(i0, i1, (uint32_t)(l >> 1), dg, k0, k1, ws);
+      double u = (l & 1) ? u01(ws[2], ws[3]) : u01(ws[0], ws[1]);
+      double total = 0.0;
+      for (uint32_t mm = mask; mm; mm &= mm - 1) { int y = __ffs(mm) - 1; total = __dadd_rn(total, __ldg(&v.Z[mask & ~(1u << y)])); }
+      double target = __dmul_rn(u, total), cum = 0.0;
+      x = -1; int last = -1;
+      for (uint32_t mm = mask; mm; mm &= mm - 1) {
+        int y = __ffs(mm) - 1; cum = __dadd_rn(cum, __ldg(&v.Z[mask & ~(1u << y)])); last = y;
+        if (target < cum) { x = y; break; }
+      }
+      if (x < 0) x = last;
+    }
+    if (l >= 1) {
+      int ru = (M - 1) + (l - 1);
+      if ((ru & 1) == 0 || l == 1) philox4x32_10(i0, i1, (uint32_t)(ru >> 1), dg, k0, k1, wr);
+      double u = (ru & 1) ? u01(wr[2], wr[3]) : u01(wr[0], wr[1]);
+      double t = det_exp2(__dmul_rn(det_log2(u), __ldg(&v.invdeg[mask])));
+      rl = __dmul_rn(rl, t); pu = __dmul_rn(pu, u);
+    }
+    r[l] = rl; ord[l] = (int8_t)x;
+    mask &= ~(1u << x);
+  }
+  double S = 0.0;
+  for (int l = 0; l < M; l++) S = __dadd_rn(S, r[l]);
+  double pz = 1.0;
+  for (int l = 0; l < M; l++) { double zz = __ddiv_rn(r[l], S); z[ord[l]] = zz; pz = __dmul_rn(pz, zz); if (WANT_ORDER) order_out[l] = ord[l]; }
+  return __ddiv_rn(__dmul_rn(v.h->C, pu), pz);
+}
+
+// ------------------------------------------------------------------ a5: one family, static code per (c, kd)
+template <class T, int KD>
+__device__ __forceinline__ T horner(const double *__restrict__ c, const T *r) {
+  if constexpr (KD == 0) { return T(__ldg(c)); }
+  else {
+    constexpr int H = 1 << (KD - 1);
+    T v[H];
+#pragma unroll
+    for (int j = 0; j < H; j++) {
+      double2 cc = __ldg(reinterpret_cast<const double2 *>(c) + j);      // (c[j], c[j+H])
+      v[j] = mq_fma_c(cc.y, r[KD - 1], cc.x, T());
+    }
+#pragma unroll
+    for (int i = KD - 2; i >= 0; i--) {
+#pragma unroll
+      for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
+    }
+    return v[0];
+  }
+}
+// index of the pair (i<j) among the C(N2,2) gathered betas
+template <int N2> __host__ __device__ constexpr int pair_index(int i, int j) { return i * N2 - i * (i + 1) / 2 + (j - i - 1); }
+constexpr int ctz_c(unsigned x) { int n = 0; while (!(x & 1u)) { x >>= 1; n++; } return n; }
+
+template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec;
+template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> struct PairStep {
+  static __device__ __forceinline__ void run(const T *b, T w, const double *__restrict__ &coef, const T *r, T &sum) {
+    if constexpr (S < N2) {
+      if constexpr (!((USED >> S) & 1u)) {
+        if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], coef, r, sum);
+        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, w * b[pair_index<N2>(F, S)], coef, r, sum);
+      }
+      PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, coef, r, sum);
+    }
+  }
+};
+template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
+  static __device__ __forceinline__ void run(const T *b, T w, const double *__restrict__ &coef, const T *r, T &sum) {
+    if constexpr (USED == ((1u << N2) - 1u)) {
+      T h = horner<T, KD>(coef, r);
+      coef += (1 << KD);
+      if constexpr (FIRST) sum = sum + h; else sum = mq_fma(w, h, sum);
+    } else {
+      constexpr int F = ctz_c(~USED);
+      PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, coef, r, sum);
+    }
+  }
+};
+
+// S: per-point scalar array of the piece in shared memory, S[index * stride]
+template <class T, int C, int KD>
+__device__ __forceinline__ T family_eval(const uint8_t *__restrict__ idx, const double *__restrict__ coef, const T *S, int stride) {
+  constexpr int N2 = 2 * C, NB = C * (2 * C - 1);
+  T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
+#pragma unroll
+  for (int i = 0; i < NB; i++) b[i] = S[(int)idx[i] * stride];
+#pragma unroll
+  for (int i = 0; i < KD; i++) r[i] = S[(int)idx[NB + i] * stride];
+  T sum = T(0.0);
+  PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), coef, r, sum);
+  return sum;
+}
+
+template <class T>
+__device__ __noinline__ T family_dispatch(int c, int kd, const uint8_t *__restrict__ idx, const double *__restrict__ coef, const T *S, int stride) {
+  switch (c * 8 + kd) {
+#define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(idx, coef, S, stride);
+#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
+    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_ROW(4)
+#undef MQ_ROW
+#undef MQ_CASE
+  }
+  return T(0.0);
+}
+
+// ------------------------------------------------------------------ a4: scalars of one piece
+// writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
+template <class T>
+__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, T &U, T &V, T &G) {
+  const int n = g.nch, ns = g.nslot;
+  T A[MQ_MAXL][MQ_MAXL], Inv[MQ_MAXL][MQ_MAXL];
+#pragma unroll
+  for (int i = 0; i < MQ_MAXL; i++)
+#pragma unroll
+    for (int j = 0; j < MQ_MAXL; j++) { A[i][j] = T(0.0); Inv[i][j] = T(i == j ? 1.0 : 0.0); }
+  for (int s = 0; s < ns; s++) {
+    if (g.slot[s].kind != MQ_SLOT_LINE) continue;
+    const uint32_t e = g.slot[s].eps; const T zt = T(z[g.slot[s].zline]);
+#pragma unroll
+    for (int i = 0; i < MQ_MAXL; i++)
+#pragma unroll
+      for (int j = 0; j < MQ_MAXL; j++) if ((e >> i & 1u) && (e >> j & 1u)) A[i][j] = A[i][j] + zt;
+  }
+#pragma unroll
+  for (int i = 0; i < MQ_MAXL; i++) if (i < n) A[i][i] = A[i][i] + T(z[g.chord_zline[i]]);
+  // Gauss-Jordan without pivoting (A is symmetric positive definite); determinant = product of pivots
+  U = T(1.0);
+#pragma unroll
+  for (int c = 0; c < MQ_MAXL; c++) {
+    if (c < n) {
+      const T p = A[c][c]; U = U * p;
+      const T ip = T(1.0) / p;
+#pragma unroll
+      for (int k = 0; k < MQ_MAXL; k++) { A[c][k] = A[c][k] * ip; Inv[c][k] = Inv[c][k] * ip; }
+#pragma unroll
+      for (int r = 0; r < MQ_MAXL; r++) if (r != c && r < n) {
+        const T f = A[r][c];
+#pragma unroll
+        for (int k = 0; k < MQ_MAXL; k++) { A[r][k] = A[r][k] - f * A[c][k]; Inv[r][k] = Inv[r][k] - f * Inv[c][k]; }
+      }
+    }
+  }
+  // beta_su = eps_s^T Inv eps_u ; x_s = sum_lines z_u beta_su ; A'_s = (sgn_s - sum_lines z_u beta_su sgn_u)/2
+  T ig[MQ_MAXSLOT];
+  V = T(0.0); G = T(1.0);
+  const int off_at = ns, off_aq = 2 * ns, off_bt = 3 * ns;
+  for (int s = 0; s < ns; s++) {
+    const uint32_t es = g.slot[s].eps;
+    T w[MQ_MAXL];
+#pragma unroll
+    for (int j = 0; j < MQ_MAXL; j++) { T a = T(0.0);
+#pragma unroll
+      for (int i = 0; i < MQ_MAXL; i++) if (es >> i & 1u) a = a + Inv[i][j];
+      w[j] = a; }
+    T x = T(0.0), q = T(0.0);
+    for (int u = 0; u < ns; u++) {
+      const uint32_t eu = g.slot[u].eps;
+      T bsu = T(0.0);
+#pragma unroll
+      for (int j = 0; j < MQ_MAXL; j++) if (eu >> j & 1u) bsu = bsu + w[j];
+      if (g.slot[u].kind == MQ_SLOT_LINE) {
+        const T zb = bsu * T(z[g.slot[u].zline]);
+        x = x + zb; if (g.slot[u].sgn < 0) q = q - zb; else q = q + zb;
+      }
+      if (u > s) S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride] = bsu;   // raw beta, scaled below
+    }
+    const bool line = g.slot[s].kind == MQ_SLOT_LINE;
+    const T gs = T(2.0) - x;
+    const T igs = line ? T(1.0) / gs : T(1.0);
+    ig[s] = igs;
+    S[s * stride] = x * igs;                                  // r_t = x_t / g_t   (lines)
+    S[(off_at + s) * stride] = T(1.0) - x;                    // A_t
+    const T sg = T((double)g.slot[s].sgn);
+    S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);       // A'_t / g_t
+    if (line) { V = V + x * T(z[g.slot[s].zline]); G = G * gs; }
+  }
+  for (int s = 0; s < ns; s++)
+    for (int u = s + 1; u < ns; u++) {
+      T *p = &S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride];
+      *p = *p * ig[s] * ig[u];
+    }
+}
+
+template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b, int nb) {   // acc <- acc (*) b, truncated at NGRADE
+  T r[MQ_NGRADE];
+#pragma unroll
+  for (int c = 0; c < MQ_NGRADE; c++) { T s = T(0.0);
+#pragma unroll
+    for (int i = 0; i < MQ_NGRADE; i++) if (i <= c && c - i < nb) s = s + acc[i] * b[c - i];
+    r[c] = s; }
+#pragma unroll
+  for (int c = 0; c < MQ_NGRADE; c++) acc[c] = r[c];
+}
+
+// ------------------------------------------------------------------ a4-a6: integrand at one point
+// S: shared-memory scalar scratch of this thread (S[index*stride]); nodeval / nodeU / nodeV: per-thread local arrays
+template <class T>
+__device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, T *S, int stride, T &f_out, T &abs_out) {
+  const DevHeader &h = *v.h;
+  T nodeval[/*worst case*/ 1024];
+  T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
+  for (int gi = 0; gi < h.ngeom; gi++) {
+    const DevGeom &g = v.geom[gi];
+    T U, V, G;
+    piece_scalars<T>(g, z, S, stride, U, V, G);
+    const int npat = 1 << g.nS;
+    for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
+      const DevTable &tb = v.tab[ti];
+      T N[2][MQ_MAXPAT][MQ_NGRADE];
+      for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
+#pragma unroll
+          for (int c = 0; c < MQ_NGRADE; c++) N[o][p][c] = T(0.0);
+      const uint64_t *st = v.blob + tb.stream_off;
+      for (int fi = 0; fi < tb.nfam; fi++) {
+        const uint64_t hd = __ldg(st);
+        const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7), pat = (int)(hd >> 6 & 15), nscal = (int)(hd >> 10 & 15), out = (int)(hd >> 14 & 1);
+        const int idxw = (int)(hd >> 16 & 0xFFFF); const uint32_t ncoef = (uint32_t)(hd >> 32);
+        const uint8_t *idx = reinterpret_cast<const uint8_t *>(st + 1);
+        const double *coef = reinterpret_cast<const double *>(st + 1 + idxw);
+        T val = family_dispatch<T>(c, kd, idx, coef, S, stride);
+        const int nb = c * (2 * c - 1) + kd;
+        for (int i = 0; i < nscal; i++) val = val * S[(int)idx[nb + i] * stride];
+        N[out][pat][c] = N[out][pat][c] + val;
+        st += 1 + idxw + ncoef;
+      }
+      // nodes that use this table: combine with the children's graded values
+      for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {
+        const DevNode &nd = v.node[ni];
+        T Up = U, Vs = V;
+        for (int k = 0; k < nd.nchild; k++) { Up = Up * nodeU[nd.child[k]]; Vs = Vs + nodeV[nd.child[k]]; }
+        nodeU[ni] = Up; nodeV[ni] = Vs;
+        for (int o = 0; o < nd.nout; o++) {
+          T tot[MQ_NGRADE];
+#pragma unroll
+          for (int c = 0; c < MQ_NGRADE; c++) tot[c] = T(0.0);
+          for (int p = 0; p < npat; p++) {
+            T acc[MQ_NGRADE];
+#pragma unroll
+            for (int c = 0; c < MQ_NGRADE; c++) acc[c] = N[o][p][c] * G;
+            for (int k = 0; k < nd.nchild; k++) {
+              const DevNode &ch = v.node[nd.child[k]];
+              const int pb = g.child_patbit[k];
+              const int which = (pb >= 0 && (p >> pb & 1)) ? 1 : 0;      // S-child: a (0) or b (1); V-child: its single value
+              graded_mul<T>(acc, &nodeval[ch.val_off + which * ch.ngr], ch.ngr);
+            }
+#pragma unroll
+            for (int c = 0; c < MQ_NGRADE; c++) tot[c] = tot[c] + acc[c];
+          }
+          for (int c = 0; c < nd.ngr; c++) nodeval[nd.val_off + o * nd.ngr + c] = tot[c];
+        }
+      }
+    }
+  }
+  // a6: terms.  f = sum sign * sum_{c<L} (L-c-1)! N_c / (Uprod^2 Vsum^(L-c))
+  const int L = h.L;
+  T f = T(0.0), asum = T(0.0);
+  for (int t = 0; t < h.nterm; t++) {
+    const DevTerm tm = v.term[t];
+    const DevNode &nd = v.node[tm.root];
+    const T U2 = nodeU[tm.root] * nodeU[tm.root], Vs = nodeV[tm.root];
+    T Vp = T(1.0);
+    double fact = 1.0;
+    for (int c = L - 1; c >= 0; c--) {
+      Vp = Vp * Vs;
+      if (L - c - 1 > 0) fact *= (double)(L - c - 1);
+      T contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : T(0.0)) * T(fact * (double)tm.sign) / (U2 * Vp);
+      f = f + contrib; asum = asum + mq_abs(contrib);
+    }
+  }
+  f_out = f; abs_out = asum;
+}
+
+}  // namespace mqk

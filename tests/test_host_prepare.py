@@ -1,0 +1,125 @@
+"""CPU tests of the product's host logic (no GPU): the C-ABI library loads and exports what
+include/mcqed.h declares, rejects bad input, and its host preparation (combinatorics, Deg/Z tables,
+numerator tables read through tests/blob_interp.py) agrees with the oracle."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from blob_interp import Blob
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def mc():
+    from paper_1905_08007_b200 import build, binding
+    build.build()
+    return binding
+
+
+def _has_cuda():
+    try:
+        import torch
+        return torch.cuda.is_available()
+    except Exception:
+        return False
+
+
+def test_library_exports_every_declared_symbol(mc):
+    hdr = open(os.path.join(ROOT, "include", "mcqed.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(mc_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(mc.EXPORTS)
+    lib = mc.lib()
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.mc_version()
+    assert lib.mc_strerror(mc.MC_ECUDA).decode().startswith("CUDA")
+
+
+def test_invalid_graphs_rejected(mc):
+    for (L, e, ch) in [(1, 0, [(1, 2)]), (2, 2, [(0, 1), (3, 4)]), (2, 2, [(0, 1), (1, 4)]), (2, 2, [(0, 2), (1, 4)]), (6, 1, [(0, 2)]), (0, 0, [])]:
+        with pytest.raises(mc.McError) as ei:
+            mc.Diagram(L, e, ch, host_only=True)
+        assert ei.value.code == mc.MC_EINVAL
+    with pytest.raises(mc.McError):
+        mc.Diagram(1, 1, [(0, 2)], deg_floor=-1.0, host_only=True)
+    # user forests that disagree with the enumeration
+    with pytest.raises(mc.McError):
+        mc.Diagram(2, 2, [(0, 4), (1, 3)], host_only=True, forests=([(1, 2)], [0, 1]))
+    d = mc.Diagram(2, 2, [(0, 4), (1, 3)], host_only=True, forests=([(1, 3)], [0, 1]))
+    assert d.subgraphs() == [(1, 3, 1)]
+
+
+def test_no_cpu_fallback(mc):
+    d = mc.Diagram(1, 1, [(0, 2)], host_only=True)
+    with pytest.raises(mc.McError) as ei:      # a host-only handle never computes
+        d.integrate_host(0, 10, 1)
+    assert ei.value.code == mc.MC_EINVAL
+    if not _has_cuda():
+        with pytest.raises(mc.McError) as ei:
+            mc.Diagram(1, 1, [(0, 2)])
+        assert ei.value.code == mc.MC_ECUDA
+        with pytest.raises(mc.McError) as ei:
+            mc.fp64_peak(16)
+        assert ei.value.code == mc.MC_ECUDA
+
+
+def _pairs(po, L, idxs):
+    for i in idxs:
+        g = po.graph_get(L, i)
+        yield i, g
+
+
+@pytest.mark.parametrize("L,idxs", [(1, [0]), (2, range(6)), (3, range(50)), (4, range(0, 518, 29)), (5, [0, 1234, 3333, 6353])])
+def test_combinatorics_and_sampler_tables_equal_oracle(po, mc, L, idxs):
+    """graph/forest indexing and the Eq.(1) tables must be bit-exact (north_star)"""
+    for i, g in _pairs(po, L, idxs):
+        o = po.Diagram(g, level=0)
+        d = mc.Diagram(L, g.ext_pos, g.chords(), host_only=True)
+        assert d.id() == i == o.id
+        assert d.info()["class"] == po.graph_class(g)
+        assert d.subgraphs() == o.subgraphs()
+        assert d.forests() == o.forests()
+        assert d.terms() == o.terms()
+        deg, Z, Cn = d.sampler_tables()
+        odeg, oZ, oC = o.sampler_tables()
+        assert np.array_equal(deg, odeg) and np.array_equal(Z, oZ) and Cn == oC
+        d.close()
+
+
+def test_sampler_tables_other_options(po, mc):
+    g = po.graph_get(3, 7)
+    o = po.Diagram(g, deg_floor=0.75, deg_cap=1.25, level=0)
+    d = mc.Diagram(3, g.ext_pos, g.chords(), deg_floor=0.75, deg_cap=1.25, host_only=True)
+    assert np.array_equal(d.sampler_tables()[1], o.sampler_tables()[1])
+
+
+@pytest.mark.parametrize("L,idxs,npts", [(1, [0], 20), (2, range(6), 8), (3, [0, 7, 8, 9, 18, 29, 38, 47], 3)])
+def test_numerator_tables_against_oracle(po, mc, L, idxs, npts):
+    """the device tables, interpreted in Python, reproduce the oracle's integrand and every term"""
+    rng = np.random.default_rng(L)
+    for i, g in _pairs(po, L, idxs):
+        o = po.Diagram(g)
+        d = mc.Diagram(L, g.ext_pos, g.chords(), host_only=True)
+        b = Blob(d.blob())
+        assert int(b.h["diag_id"]) == i and int(b.h["nterm"]) == o.nterm
+        z = rng.dirichlet([1.0] * (3 * L), npts)
+        ref = o.eval_z(z, wide=True, want_terms=True)
+        for k in range(npts):
+            f, terms = b.integrand(z[k])
+            scale = np.max(np.abs(ref["terms"][k]))
+            assert abs(f - ref["fwide"][k]) <= 1e-10 * scale, (i, k, f, ref["fwide"][k])
+            assert np.allclose(terms, ref["terms"][k], rtol=1e-9, atol=1e-10 * scale)
+        d.close()
+
+
+def test_info_counts(po, mc):
+    g = po.graph_get(3, 29)
+    d = mc.Diagram(3, g.ext_pos, g.chords(), host_only=True)
+    info = d.info()
+    assert info["n_terms"] == po.Diagram(g, level=0).nterm == 8
+    assert info["flop_per_sample"] > 0 and info["table_bytes"] == 8 * len(d.blob())

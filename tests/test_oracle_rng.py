@@ -14,15 +14,15 @@ def test_philox_known_answers(po):
 
 def test_uniform_construction(po):
     lib = po.lib()
-    assert lib.oracle_u01(0, 0) == 0.5 * 2.0 ** -53
-    assert lib.oracle_u01(0xFFFFFFFF, 0xFFFFFFFF) == 1.0 - 0.5 * 2.0 ** -53
-    assert lib.oracle_u01(0x80000000, 0) == 0.5 + 0.5 * 2.0 ** -53
+    assert lib.oracle_u01(0, 0) == 0.5 * 2.0 ** -52
+    assert lib.oracle_u01(0xFFFFFFFF, 0xFFFFFFFF) == 1.0 - 0.5 * 2.0 ** -52
+    assert lib.oracle_u01(0x80000000, 0) == 0.5 + 0.5 * 2.0 ** -52
     # stream layout: uniform r comes from Philox block r//2 of ctr=(idx_lo, idx_hi, block, diagram)
     idx, diag, seed = (5 << 32) | 77, 9, (3 << 32) | 11
     for r in range(6):
         w = po.philox([77, 5, r // 2, 9], [11, 3])
         x, y = (w[2], w[3]) if r & 1 else (w[0], w[1])
-        assert lib.oracle_sample_uniform(idx, diag, seed, r) == ((x >> 5) * 2.0 ** 26 + (y >> 6) + 0.5) * 2.0 ** -53
+        assert lib.oracle_sample_uniform(idx, diag, seed, r) == ((x >> 6) * 2.0 ** 26 + (y >> 6) + 0.5) * 2.0 ** -52
 
 
 def test_uniform_moments(po):
@@ -42,7 +42,7 @@ def test_det_pow_accuracy_and_monotonicity(po):
         worst = max(worst, abs(got - want) / want)
     assert worst < 5e-15
     # extreme uniforms the stream can produce
-    for u in (0.5 * 2.0 ** -53, 1 - 0.5 * 2.0 ** -53, 2.0 ** -30):
+    for u in (0.5 * 2.0 ** -52, 1 - 0.5 * 2.0 ** -52, 2.0 ** -30):
         for d in (0.5, 1.0, 3.0):
             got, want = lib.oracle_det_pow(u, 1.0 / d), u ** (1.0 / d)
             assert abs(got - want) <= 5e-15 * want
