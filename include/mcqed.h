@@ -54,11 +54,14 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {0.5, 1e30, 4096.0, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5);
- * cond_max: a point is flagged for double-double re-evaluation when
- * sum_terms sum_grades |contribution| > cond_max * |f| or anything is non-finite (O8);
- * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0). */
-typedef struct { double deg_floor, deg_cap, cond_max; uint32_t flags; } mc_options;
+/* NULL => defaults {0.5, 1e30, 4096.0, 1e-5, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5).
+ * Precision flag (O8): a point is re-evaluated in double-double when
+ *   sum_terms sum_grades |contribution| > cond_max * |f|,  or  min over electron lines of every piece of
+ *   A_t = 1 - x_t is below amin_min (the scalar currents lose relative accuracy like eps/A_t),  or
+ *   anything is non-finite / some z_l < 2^-600.
+ * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0).
+ * flags bit 1: build no numerator tables (introspection of the combinatorics only; host handles). */
+typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; } mc_options;
 
 /* Host-side preparation of one diagram (not on the timed path): validates the graph, enumerates
  * subgraphs/forests/terms (forest-like formula, O1), builds Deg and the sector-sum table
@@ -117,9 +120,10 @@ int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64
                    double *cond_out, uint8_t *flag_out);
 
 /* Integrand at caller-supplied points (DEVICE z_in n*M): f64_out, fdd_out (double-double evaluation
- * rounded to binary64), cond_out; any output may be NULL. */
+ * rounded to binary64), cond_out (sum|contrib|/|f|), aux_out n*2 (min A_t, min x_t over the electron
+ * lines of all pieces); any output may be NULL. */
 int mc_eval_z(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream,
-              double *f64_out, double *fdd_out, double *cond_out);
+              double *f64_out, double *fdd_out, double *cond_out, double *aux_out);
 
 /* Number of kernels this library has launched in the calling process (for gpu_launches in bench.py). */
 unsigned long long mc_kernel_launch_count(void);

@@ -13,12 +13,19 @@ DEPS = SRC + ["qed_combi.h", "qed_piece.h", "qed_sampler.h", "qed_tables.h", "qe
 
 
 def build(force=False):
-    newest = max(os.path.getmtime(os.path.join(HERE, f)) for f in DEPS)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
-        return LIB
+    import hashlib
+    h = hashlib.sha256()
+    for f in DEPS:
+        with open(os.path.join(HERE, f), "rb") as fh:
+            h.update(fh.read())
+    digest, stamp = h.hexdigest(), LIB + ".stamp"
+    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == digest:
+        return LIB      # content hash, not mtime: snapshots lose mtimes
     cmd = ["gcc", "-O2", "-std=gnu11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
            "-Wall", "-Wno-unused-function", "-o", LIB] + [os.path.join(HERE, f) for f in SRC] + ["-lm"]
     subprocess.check_call(cmd)
+    with open(stamp, "w") as fh:
+        fh.write(digest)
     return LIB
 
 

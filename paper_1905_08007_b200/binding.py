@@ -11,6 +11,7 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ELIMIT = 0, -1, -2, -3, -4
+FLAG_NO_DD, FLAG_NO_TABLES = 1, 2
 
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
@@ -30,7 +31,7 @@ class McForests(C.Structure):
 
 
 class McOptions(C.Structure):
-    _fields_ = [("deg_floor", C.c_double), ("deg_cap", C.c_double), ("cond_max", C.c_double), ("flags", C.c_uint32)]
+    _fields_ = [("deg_floor", C.c_double), ("deg_cap", C.c_double), ("cond_max", C.c_double), ("amin_min", C.c_double), ("flags", C.c_uint32)]
 
 
 class McError(RuntimeError):
@@ -70,7 +71,7 @@ def lib():
         L.mc_integrate.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
-        L.mc_eval_z.argtypes = [vp, u64, vp, vp, vp, vp, vp]
+        L.mc_eval_z.argtypes = [vp, u64, vp, vp, vp, vp, vp, vp]
         L.mc_kernel_launch_count.restype = C.c_ulonglong
         L.mc_fp64_peak.argtypes = [C.c_int, vp, dp, dp]
         L.mc_strerror.restype = C.c_char_p
@@ -107,10 +108,10 @@ def make_graph(loops, ext_pos, chords):
 class Diagram:
     """RAII handle around mc_diagram*"""
 
-    def __init__(self, loops, ext_pos, chords, deg_floor=0.5, deg_cap=1e30, cond_max=4096.0, flags=0, host_only=False, forests=None):
+    def __init__(self, loops, ext_pos, chords, deg_floor=0.5, deg_cap=1e30, cond_max=4096.0, amin_min=1e-5, flags=0, host_only=False, forests=None):
         self.loops, self.M = loops, 3 * loops
         g = make_graph(loops, ext_pos, chords)
-        opt = McOptions(deg_floor, deg_cap, cond_max, flags)
+        opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags)
         self.h = C.c_void_p()
         fo = None
         if forests is not None:
@@ -183,8 +184,8 @@ class Diagram:
         _check(lib().mc_eval_points(self.h, first_sample, n, seed, _ptr(stream), _ptr(z), _ptr(order), _ptr(p), _ptr(f), _ptr(f64),
                                     _ptr(cond), _ptr(flag)), "mc_eval_points")
 
-    def eval_z(self, n, z_in, stream=None, f64=None, fdd=None, cond=None):
-        _check(lib().mc_eval_z(self.h, n, _ptr(z_in), _ptr(stream), _ptr(f64), _ptr(fdd), _ptr(cond)), "mc_eval_z")
+    def eval_z(self, n, z_in, stream=None, f64=None, fdd=None, cond=None, aux=None):
+        _check(lib().mc_eval_z(self.h, n, _ptr(z_in), _ptr(stream), _ptr(f64), _ptr(fdd), _ptr(cond), _ptr(aux)), "mc_eval_z")
 
 
 def kernel_launch_count():

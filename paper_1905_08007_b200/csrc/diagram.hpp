@@ -1,0 +1,58 @@
+// diagram.hpp — the object behind mc_diagram* and the host-callable launchers of the kernels.
+// Product code (libmcqed.so); shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "../../include/mcqed.h"
+#include "host_model.hpp"
+
+namespace mqk {
+constexpr int TPB_F64 = 128, TPB_DD = 64, TPB_EVAL = 64;
+constexpr uint64_t CHUNK = 1ull << 22;     // samples per launch (bounds the flagged-index list)
+constexpr int MAXGRID = 148 * 16;
+}  // namespace mqk
+
+struct McWorkspace {
+  double *partial = nullptr;               // [2][MAXGRID][4] per-block compensated partial sums (f64 pass, dd pass)
+  unsigned long long *flag_list = nullptr; // [CHUNK] sample indices flagged in the current chunk
+  unsigned long long *counters = nullptr;  // [4]: flagged in chunk, dropped, -, -
+};
+
+struct mc_diagram {
+  mq::VertexGraph g;
+  mq::ForestTerms ft;
+  mq::SamplerTables st;
+  mc_options opt{};
+  int id = -1;
+  std::vector<uint64_t> blob;              // host copy of the device blob (device_layout.h)
+  std::vector<DevGeom> geoms; std::vector<DevTable> tables; std::vector<DevNode> nodes; std::vector<DevTerm> terms;
+  int64_t n_stored = 0, n_nonzero = 0;
+  int max_scal_len = 0, nodeval_len = 0;
+  bool have_tables = false;
+  // device side
+  uint64_t *d_blob = nullptr;
+  McWorkspace ws;
+  bool on_device = false;
+  int grid_f64 = 0, grid_dd = 0;
+  size_t smem_f64 = 0, smem_dd = 0, smem_eval = 0;
+};
+
+// host preparation (host_prepare.cpp)
+int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, mc_diagram **out);
+
+// launchers (kern_f64.cu / kern_dd.cu); every one returns a cudaError_t cast to int
+typedef struct CUstream_st *mq_stream;
+int mq_config_f64(mc_diagram *d);
+int mq_config_dd(mc_diagram *d);
+void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st);
+void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st);
+void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);
+void mq_launch_reset(const mc_diagram *d, mq_stream st);
+void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,
+                           double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out,
+                           uint8_t *flag_out, bool list_flagged, mq_stream st);
+void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st);
+void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st);
+void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st);
+int mq_fp64_peak(int iters, mq_stream st, double *flops, double *ms);

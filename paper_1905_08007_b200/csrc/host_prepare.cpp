@@ -1,0 +1,209 @@
+// host_prepare.cpp — host-side preparation of one diagram: term trees, unique pieces and nodes,
+// numerator tables, and the device blob (device_layout.h). Not on the timed path.
+// Product code (libmcqed.so); shares nothing with oracle/.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <functional>
+#include <memory>
+#include <thread>
+
+#include "coef_gen.hpp"
+#include "diagram.hpp"
+
+// =====================================================================================
+//                                   host preparation
+// =====================================================================================
+namespace {
+
+struct NodeKey { int geom, op; std::vector<int> kids; bool operator==(const NodeKey &o) const { return geom == o.geom && op == o.op && kids == o.kids; } };
+
+struct Builder {
+  mc_diagram &d;
+  std::vector<mq::Piece> pieces;                 // one per geom
+  std::vector<std::pair<int, uint32_t>> geomKey; // (sub index or -1, child mask)
+  std::vector<NodeKey> nodeKeys;
+  explicit Builder(mc_diagram &dd_) : d(dd_) {}
+
+  mq::Segment segOf(int sub) const { return sub < 0 ? mq::Segment{0, 2 * d.g.L, true} : d.ft.subs[sub]; }
+
+  int opOf(int H, int gprime) const {
+    if (H == gprime) return MQ_OP_A;
+    const bool inI = H < 0 || (d.ft.subs[H].vertexLike && d.ft.subs[H].has(d.g.e));
+    const bool insideGp = H >= 0 && (gprime < 0 || (d.ft.subs[H].within(d.ft.subs[gprime]) && H != gprime));
+    if (!inI || insideGp) return MQ_OP_U;
+    return H < 0 ? MQ_OP_LMU : MQ_OP_L;
+  }
+  int geomOf(int H, uint32_t F) {
+    auto kids = d.ft.childrenOf(F, segOf(H));
+    uint32_t cm = 0; for (int k : kids) cm |= 1u << k;
+    for (size_t i = 0; i < geomKey.size(); i++) if (geomKey[i].first == H && geomKey[i].second == cm) return (int)i;
+    std::vector<mq::Segment> ks; for (int k : kids) ks.push_back(d.ft.subs[k]);
+    mq::Piece p; p.build(d.g, segOf(H), ks);
+    pieces.push_back(p); geomKey.emplace_back(H, cm);
+    return (int)pieces.size() - 1;
+  }
+  int nodeOf(int H, uint32_t F, int gprime) {
+    NodeKey k; k.geom = geomOf(H, F); k.op = opOf(H, gprime);
+    for (int c : d.ft.childrenOf(F, segOf(H))) k.kids.push_back(nodeOf(c, F, gprime));
+    for (size_t i = 0; i < nodeKeys.size(); i++) if (nodeKeys[i] == k) return (int)i;
+    nodeKeys.push_back(k);
+    return (int)nodeKeys.size() - 1;
+  }
+};
+
+}  // namespace
+
+int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, mc_diagram **out) {
+  if (!graph || !out) return MC_EINVAL;
+  std::unique_ptr<mc_diagram> d(new mc_diagram);
+  d->opt = opts ? *opts : mc_options{0.5, 1e30, 4096.0, 1e-5, 0u};
+  if (!(d->opt.deg_floor > 0) || !(d->opt.deg_cap >= d->opt.deg_floor) || !(d->opt.cond_max > 0)) return MC_EINVAL;
+  if (!d->g.build(graph->loops, graph->ext_pos, graph->chord_a, graph->chord_b)) return MC_EINVAL;
+  d->id = d->g.canonicalId();
+  if (d->id < 0) return MC_EINVAL;
+  d->ft.enumerate(d->g);
+  if (uf) {   // user forests must agree with the enumeration
+    if (uf->n_sub != (int)d->ft.subs.size() || uf->n_forest != (int)d->ft.forests.size()) return MC_EINVAL;
+    for (int i = 0; i < uf->n_sub; i++) if (uf->seg_lo[i] != d->ft.subs[i].lo || uf->seg_hi[i] != d->ft.subs[i].hi) return MC_EINVAL;
+    for (int i = 0; i < uf->n_forest; i++) if (uf->forest_mask[i] != d->ft.forests[i]) return MC_EINVAL;
+  }
+  d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap);
+
+  // ---- term trees -> unique pieces (geoms) and nodes ----
+  Builder B(*d);
+  std::vector<int> roots;
+  for (auto &t : d->ft.terms) roots.push_back(B.nodeOf(-1, t.forest, t.gprime));
+  const int ngeom0 = (int)B.pieces.size(), nnode0 = (int)B.nodeKeys.size();
+  if (ngeom0 > MQ_MAXGEOM || nnode0 > MQ_MAXNODE) return MC_ELIMIT;
+  // geoms sorted by segment length (children first), then lo, then child mask
+  std::vector<int> gorder(ngeom0);
+  for (int i = 0; i < ngeom0; i++) gorder[i] = i;
+  std::sort(gorder.begin(), gorder.end(), [&](int a, int b) {
+    const auto &pa = B.pieces[a].seg, &pb = B.pieces[b].seg;
+    if (pa.hi - pa.lo != pb.hi - pb.lo) return pa.hi - pa.lo < pb.hi - pb.lo;
+    if (pa.lo != pb.lo) return pa.lo < pb.lo;
+    return B.geomKey[a].second < B.geomKey[b].second;
+  });
+  std::vector<int> gnew(ngeom0);
+  for (int i = 0; i < ngeom0; i++) gnew[gorder[i]] = i;
+  // tables: (geom, op) pairs in geom order; nodes sorted by (geom, op)
+  std::vector<int> norder(nnode0);
+  for (int i = 0; i < nnode0; i++) norder[i] = i;
+  std::stable_sort(norder.begin(), norder.end(), [&](int a, int b) {
+    int ga = gnew[B.nodeKeys[a].geom], gb = gnew[B.nodeKeys[b].geom];
+    if (ga != gb) return ga < gb;
+    return B.nodeKeys[a].op < B.nodeKeys[b].op;
+  });
+  std::vector<int> nnew(nnode0);
+  for (int i = 0; i < nnode0; i++) nnew[norder[i]] = i;
+
+  d->geoms.resize(ngeom0);
+  for (int gi = 0; gi < ngeom0; gi++) {
+    const mq::Piece &p = B.pieces[gorder[gi]];
+    DevGeom G; std::memset(&G, 0, sizeof G);
+    G.nch = (int)p.ownChord.size(); G.nslot = (int)p.slots.size(); G.nchild = (int)p.kids.size(); G.nS = p.nS;
+    if (G.nslot > MQ_MAXSLOT || G.nchild > MQ_MAXCHILD || (1 << G.nS) > MQ_MAXPAT) return MC_ELIMIT;
+    for (int i = 0; i < G.nch; i++) G.chord_zline[i] = 2 * d->g.L + p.ownChord[i];
+    for (int s = 0; s < G.nslot; s++) {
+      G.slot[s].kind = p.slots[s].insertion ? MQ_SLOT_INS : MQ_SLOT_LINE;
+      G.slot[s].zline = (int8_t)p.slots[s].line; G.slot[s].sgn = (int8_t)p.slots[s].sgn;
+      G.slot[s].child = (int8_t)p.slots[s].child; G.slot[s].eps = p.slots[s].eps;
+    }
+    for (int c = 0; c < G.nchild; c++) { G.child_type[c] = p.kids[c].vertexLike ? 1 : 0; G.child_patbit[c] = (int8_t)p.patbit[c]; }
+    d->geoms[gi] = G;
+    d->max_scal_len = std::max(d->max_scal_len, 3 * G.nslot + G.nslot * (G.nslot - 1) / 2);
+  }
+  // nodes + tables
+  const bool no_tables = d->opt.flags & 2u;
+  d->nodes.resize(nnode0);
+  std::vector<mq::TableBuild> builds;
+  unsigned hw = std::thread::hardware_concurrency();
+  int nthreads = hw ? (int)hw : 4;
+  if (const char *env = std::getenv("MCQED_PREPARE_THREADS")) nthreads = std::max(1, atoi(env));
+  for (int ni = 0; ni < nnode0; ni++) {
+    const NodeKey &k = B.nodeKeys[norder[ni]];
+    const int gi = gnew[k.geom];
+    const mq::Piece &p = B.pieces[k.geom];
+    if (d->tables.empty() || d->tables.back().geom != gi || d->tables.back().op != k.op) {
+      DevTable T; std::memset(&T, 0, sizeof T);
+      T.geom = gi; T.op = k.op; T.nout = p.seg.vertexLike ? 1 : 2; T.first_node = ni; T.nnode = 0;
+      d->tables.push_back(T);
+      builds.push_back(no_tables ? mq::TableBuild{} : mq::buildTable(p, k.op, nthreads));
+    }
+    d->tables.back().nnode++;
+    DevNode N; std::memset(&N, 0, sizeof N);
+    N.table = (int)d->tables.size() - 1; N.geom = gi; N.nchild = (int)k.kids.size(); N.nout = p.seg.vertexLike ? 1 : 2;
+    for (int c = 0; c < N.nchild; c++) N.child[c] = nnew[k.kids[c]];
+    int loops_inside = 0;
+    for (int i = 0; i < d->g.L; i++) if (p.seg.has(d->g.ca[i]) && p.seg.has(d->g.cb[i])) loops_inside++;
+    N.ngr = std::min(MQ_NGRADE, loops_inside + 1);
+    N.val_off = d->nodeval_len; d->nodeval_len += N.nout * N.ngr;
+    d->nodes[ni] = N;
+  }
+  if (d->nodeval_len > 1024) return MC_ELIMIT;
+  for (size_t ti = 0; ti < d->tables.size(); ti++) {
+    DevGeom &G = d->geoms[d->tables[ti].geom];
+    if (G.ntable == 0) G.first_table = (int)ti;
+    G.ntable++;
+  }
+  for (size_t t = 0; t < d->ft.terms.size(); t++) d->terms.push_back({nnew[roots[t]], d->ft.terms[t].sign});
+
+  // ---- blob ----
+  auto words = [](size_t bytes) { return (int64_t)((bytes + 7) / 8); };
+  DevHeader H; std::memset(&H, 0, sizeof H);
+  H.L = d->g.L; H.M = d->g.M; H.diag_id = d->id; H.ngeom = ngeom0; H.ntable = (int)d->tables.size(); H.nnode = nnode0; H.nterm = (int)d->terms.size();
+  H.nodeval_len = d->nodeval_len; H.max_scal_len = d->max_scal_len; H.C = d->st.C; H.cond_max = d->opt.cond_max;
+  int64_t off = words(sizeof(DevHeader));
+  const int64_t nZ = (int64_t)1 << d->g.M;
+  H.off_Z = off; off += nZ; H.off_invdeg = off; off += nZ;
+  H.off_geom = off; off += words(sizeof(DevGeom) * d->geoms.size());
+  H.off_table = off; off += words(sizeof(DevTable) * d->tables.size());
+  H.off_node = off; off += words(sizeof(DevNode) * d->nodes.size());
+  H.off_term = off; off += words(sizeof(DevTerm) * d->terms.size());
+  // streams: every family = header word | index bytes (padded) | coefficients; the coefficients start on a
+  // 16-byte boundary (the kernel reads them as double2), so the index words are padded to make pos+1+idxw even
+  std::vector<uint64_t> streams;
+  const int64_t stream_base = off;
+  for (size_t ti = 0; ti < d->tables.size(); ti++) {
+    DevTable &T = d->tables[ti]; const mq::TableBuild &tb = builds[ti];
+    T.stream_off = stream_base + (int64_t)streams.size(); T.nfam = (int)tb.fams.size(); T.n_monomials = tb.n_stored;
+    const int ns = d->geoms[T.geom].nslot;
+    auto tri = [&](int a, int b) { if (a > b) std::swap(a, b); return 3 * ns + a * ns - a * (a + 1) / 2 + (b - a - 1); };
+    for (auto &f : tb.fams) {
+      std::vector<uint8_t> idx;
+      const int n2 = 2 * f.c;
+      for (int i = 0; i < n2; i++) for (int j = i + 1; j < n2; j++) idx.push_back((uint8_t)tri(f.paired[i], f.paired[j]));
+      for (uint8_t sl : f.inner) idx.push_back(sl);                            // r_t lives at S[t]
+      for (uint8_t sc : f.scal) {
+        const int kind = sc >> 4, slot = sc & 15;
+        idx.push_back((uint8_t)(kind == MQ_SC_R ? slot : kind == MQ_SC_AT ? ns + slot : 2 * ns + slot));
+      }
+      int idxw = (int)words(idx.size());
+      const int64_t pos = stream_base + (int64_t)streams.size();
+      if ((pos + 1 + idxw) & 1) idxw++;
+      streams.push_back(mq_pack_family(f.c, f.kd, f.pattern, (int)f.scal.size(), f.out, idxw, (uint32_t)f.coef.size()));
+      const size_t at = streams.size();
+      streams.resize(at + idxw + f.coef.size(), 0ull);
+      std::memcpy(streams.data() + at, idx.data(), idx.size());
+      std::memcpy(streams.data() + at + idxw, f.coef.data(), sizeof(double) * f.coef.size());
+    }
+    T.stream_words = stream_base + (int64_t)streams.size() - T.stream_off;
+    d->n_stored += tb.n_stored; d->n_nonzero += tb.n_nonzero;
+  }
+  off += (int64_t)streams.size();
+  H.total_words = off;
+  d->blob.assign((size_t)off, 0ull);
+  std::memcpy(d->blob.data(), &H, sizeof H);
+  std::memcpy(d->blob.data() + H.off_Z, d->st.Z.data(), sizeof(double) * nZ);
+  std::memcpy(d->blob.data() + H.off_invdeg, d->st.invdeg.data(), sizeof(double) * nZ);
+  std::memcpy(d->blob.data() + H.off_geom, d->geoms.data(), sizeof(DevGeom) * d->geoms.size());
+  std::memcpy(d->blob.data() + H.off_table, d->tables.data(), sizeof(DevTable) * d->tables.size());
+  std::memcpy(d->blob.data() + H.off_node, d->nodes.data(), sizeof(DevNode) * d->nodes.size());
+  std::memcpy(d->blob.data() + H.off_term, d->terms.data(), sizeof(DevTerm) * d->terms.size());
+  if (!streams.empty()) std::memcpy(d->blob.data() + stream_base, streams.data(), sizeof(uint64_t) * streams.size());
+  d->have_tables = !no_tables;
+  *out = d.release();
+  return MC_OK;
+}
+

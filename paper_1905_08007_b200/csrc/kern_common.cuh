@@ -1,0 +1,41 @@
+// kern_common.cuh — pieces shared by the two kernel translation units (binary64 and double-double).
+// Product code (libmcqed.so).
+#pragma once
+#include "diagram.hpp"
+#include "mcqed_kernels.cuh"
+
+namespace mqk {
+
+struct KahanPair {   // compensated running sum (hi, lo)
+  double hi, lo;
+  __device__ __forceinline__ void add(double x) { dd s = dd_two_sum(hi, x); hi = s.hi; lo = __dadd_rn(lo, s.lo); }
+  __device__ __forceinline__ void merge(double ohi, double olo) { dd s = dd_two_sum(hi, ohi); hi = s.hi; lo = __dadd_rn(lo, __dadd_rn(s.lo, olo)); }
+};
+
+// a7: block reduction of two compensated sums (warp shuffles, then shared memory); thread 0 writes partial[block][0..3]
+__device__ __forceinline__ void block_reduce_store(KahanPair a, KahanPair b, double *partial) {
+  __shared__ double red[32][4];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    double ah = __shfl_down_sync(0xffffffffu, a.hi, off), al = __shfl_down_sync(0xffffffffu, a.lo, off);
+    double bh = __shfl_down_sync(0xffffffffu, b.hi, off), bl = __shfl_down_sync(0xffffffffu, b.lo, off);
+    a.merge(ah, al); b.merge(bh, bl);
+  }
+  if (lane == 0) { red[warp][0] = a.hi; red[warp][1] = a.lo; red[warp][2] = b.hi; red[warp][3] = b.lo; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    KahanPair sa{0.0, 0.0}, sb{0.0, 0.0};
+    for (int w = 0; w < nw; w++) { sa.merge(red[w][0], red[w][1]); sb.merge(red[w][2], red[w][3]); }
+    partial[blockIdx.x * 4 + 0] = sa.hi; partial[blockIdx.x * 4 + 1] = sa.lo;
+    partial[blockIdx.x * 4 + 2] = sb.hi; partial[blockIdx.x * 4 + 3] = sb.lo;
+  }
+}
+
+__device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   // DESIGN.md A15
+  bool bad = !(p > 0.0) || !isfinite(p);
+  for (int i = 0; i < M; i++) bad |= !(z[i] >= 0x1p-600);
+  return bad;
+}
+
+}  // namespace mqk

@@ -1,0 +1,87 @@
+// kern_dd.cu — double-double kernels: the precision fallback (a8) and their launchers. sm_100a.
+// Product code (libmcqed.so); shares nothing with oracle/.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+
+#include "kern_common.cuh"
+
+namespace mqk {
+
+// a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
+__global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
+                                                         const unsigned long long *flag_list, unsigned long long *counters) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  dd *S = reinterpret_cast<dd *>(smem) + threadIdx.x;
+  const int stride = blockDim.x;
+  const unsigned long long cnt = counters[0];
+  KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (unsigned long long)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM];
+    const double p = draw_point<false>(v, flag_list[i], seed, z, nullptr);
+    dd f, a; double amin, xmin;
+    eval_integrand<dd>(v, z, S, stride, f, a, amin, xmin);
+    const double fd = mq_to_double(f);
+    if (bad_point(z, v.h->M, p) || !isfinite(fd)) atomicAdd(&counters[1], 1ull);
+    else { const double w = fd / p; s1.add(w); s2.add(w * w); }
+  }
+  block_reduce_store(s1, s2, partial);
+}
+
+__global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
+                                                           const unsigned long long *flag_list, const unsigned long long *counters) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  dd *S = reinterpret_cast<dd *>(smem) + threadIdx.x;
+  const unsigned long long cnt = counters[0];
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (unsigned long long)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM];
+    const unsigned long long rel = flag_list[i];
+    draw_point<false>(v, first + rel, seed, z, nullptr);
+    dd f, a; double amin, xmin;
+    eval_integrand<dd>(v, z, S, blockDim.x, f, a, amin, xmin);
+    f_out[rel] = mq_to_double(f);
+  }
+}
+
+__global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in, double *fdd_out) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  const int M = v.h->M;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM];
+    for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
+    dd f, a; double amin, xmin;
+    eval_integrand<dd>(v, z, reinterpret_cast<dd *>(smem) + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    fdd_out[i] = mq_to_double(f);
+  }
+}
+
+}  // namespace mqk
+
+using namespace mqk;
+
+int mq_config_dd(mc_diagram *d) {
+  d->smem_dd = (size_t)d->max_scal_len * 2 * sizeof(double) * TPB_DD;
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_integrate_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_points_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_z_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
+  int nsm = 0, occ = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_integrate_dd, TPB_DD, d->smem_dd)) != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  d->grid_dd = std::min(MAXGRID, nsm * occ);
+  return 0;
+}
+void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st) {
+  k_integrate_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, seed, d->ws.partial + (size_t)MAXGRID * 4, d->ws.flag_list, d->ws.counters);
+}
+void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st) {
+  k_eval_points_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, first, seed, f_out, d->ws.flag_list, d->ws.counters);
+}
+void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st) {
+  k_eval_z_dd<<<grid, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, n, z_in, fdd_out);
+}

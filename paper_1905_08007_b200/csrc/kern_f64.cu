@@ -1,0 +1,157 @@
+// kern_f64.cu — binary64 kernels of the hot path (a1-a7) and their launchers. sm_100a.
+// Product code (libmcqed.so); shares nothing with oracle/.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+
+#include "kern_common.cuh"
+
+namespace mqk {
+
+// a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
+__global__ void __launch_bounds__(TPB_F64) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
+                                                           double cond_max, double amin_min, double *partial,
+                                                           unsigned long long *flag_list, unsigned long long *counters) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  double *S = smem + threadIdx.x;
+  const int stride = blockDim.x;
+  KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM];
+    const double p = draw_point<false>(v, first + i, seed, z, nullptr);
+    double f, a, amin, xmin;
+    eval_integrand<double>(v, z, S, stride, f, a, amin, xmin);
+    const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || amin < amin_min;
+    if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
+    else { const double w = f / p; s1.add(w); s2.add(w * w); }
+  }
+  block_reduce_store(s1, s2, partial);
+}
+
+// deterministic final reduction of the per-block partials of both passes; out += result
+__global__ void k_finish(const double *partial, int nb1, int nb2, unsigned long long *counters,
+                         double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  KahanPair a{0.0, 0.0}, b{0.0, 0.0};
+  for (int i = 0; i < nb1; i++) { a.merge(partial[i * 4], partial[i * 4 + 1]); b.merge(partial[i * 4 + 2], partial[i * 4 + 3]); }
+  const double *p2 = partial + (size_t)MAXGRID * 4;
+  for (int i = 0; i < nb2; i++) { a.merge(p2[i * 4], p2[i * 4 + 1]); b.merge(p2[i * 4 + 2], p2[i * 4 + 3]); }
+  if (out_sum) *out_sum += a.hi + a.lo;
+  if (out_sumsq) *out_sumsq += b.hi + b.lo;
+  if (out_nflag) *out_nflag += counters[0];
+  if (out_ndrop) *out_ndrop += counters[1];
+  counters[0] = 0; counters[1] = 0;
+}
+__global__ void k_reset_counters(unsigned long long *counters) { counters[0] = 0; counters[1] = 0; }
+
+// parity hook: per-point outputs (binary64 pass); flagged points are listed for the dd pass
+__global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
+                                                          double cond_max, double amin_min,
+                                                          double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out,
+                                                          double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  double *S = smem + threadIdx.x;
+  const int M = v.h->M;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM]; int32_t ord[MQ_MAXM];
+    const double p = draw_point<true>(v, first + i, seed, z, ord);
+    double f, a, amin, xmin;
+    eval_integrand<double>(v, z, S, blockDim.x, f, a, amin, xmin);
+    const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || amin < amin_min;
+    if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
+    if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
+    if (p_out) p_out[i] = p;
+    if (f_out) f_out[i] = f;
+    if (f64_out) f64_out[i] = f;
+    if (cond_out) cond_out[i] = a / fabs(f);
+    if (flag_out) flag_out[i] = flag ? 1 : 0;
+    if (flag && flag_list) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = i; }
+  }
+}
+
+__global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in,
+                                                         double *f64_out, double *cond_out, double *aux_out) {
+  extern __shared__ double smem[];
+  const DiagView v = make_view(blob);
+  const int M = v.h->M;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    double z[MQ_MAXM];
+    for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
+    double f, a, amin, xmin;
+    eval_integrand<double>(v, z, smem + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    if (f64_out) f64_out[i] = f;
+    if (cond_out) cond_out[i] = a / fabs(f);
+    if (aux_out) { aux_out[2 * i] = amin; aux_out[2 * i + 1] = xmin; }
+  }
+}
+
+// FP64 FMA peak: 8 independent chains per thread
+__global__ void k_fp64_peak(int iters, double *sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3, a4 = a0 + 4e-3, a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.999999999, c = 1e-9;
+  for (int i = 0; i < iters; i++) {
+#pragma unroll
+    for (int k = 0; k < 16; k++) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+  }
+  if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == 12345.678) sink[0] = a0;
+}
+
+}  // namespace mqk
+
+using namespace mqk;
+
+int mq_config_f64(mc_diagram *d) {
+  d->smem_f64 = (size_t)d->max_scal_len * sizeof(double) * TPB_F64;
+  d->smem_eval = (size_t)d->max_scal_len * sizeof(double) * TPB_EVAL;
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_integrate_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_f64)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_points, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_z_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;
+  int nsm = 0, occ = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_integrate_f64, TPB_F64, d->smem_f64)) != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  d->grid_f64 = std::min(MAXGRID, nsm * occ);
+  return 0;
+}
+void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st) {
+  k_integrate_f64<<<grid, TPB_F64, d->smem_f64, (cudaStream_t)st>>>(d->d_blob, first, n, seed, cond_max, amin_min, d->ws.partial, d->ws.flag_list, d->ws.counters);
+}
+void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
+  k_finish<<<1, 32, 0, (cudaStream_t)st>>>(d->ws.partial, nb1, nb2, d->ws.counters, out_sum, out_sumsq, out_nflag, out_ndrop);
+}
+void mq_launch_reset(const mc_diagram *d, mq_stream st) { k_reset_counters<<<1, 1, 0, (cudaStream_t)st>>>(d->ws.counters); }
+void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,
+                           double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out,
+                           uint8_t *flag_out, bool list_flagged, mq_stream st) {
+  k_eval_points<<<grid, TPB_EVAL, d->smem_eval, (cudaStream_t)st>>>(d->d_blob, first, n, seed, cond_max, amin_min, z_out, order_out, p_out, f_out, f64_out,
+                                                                  cond_out, flag_out, list_flagged ? d->ws.flag_list : nullptr, d->ws.counters);
+}
+void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st) {
+  k_eval_z_f64<<<grid, TPB_EVAL, d->smem_eval, (cudaStream_t)st>>>(d->d_blob, n, z_in, f64_out, cond_out, aux_out);
+}
+int mq_fp64_peak(int iters, mq_stream stream, double *flops, double *ms) {
+  cudaStream_t st = (cudaStream_t)stream;
+  int nsm = 0, dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  double *sink = nullptr;
+  cudaError_t e;
+  if ((e = cudaMalloc(&sink, 8)) != cudaSuccess) return (int)e;
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = nsm * 2, tpb = 1024;
+  k_fp64_peak<<<blocks, tpb, 0, st>>>(iters / 8 + 1, sink);   // warm-up
+  cudaEventRecord(e0, st);
+  k_fp64_peak<<<blocks, tpb, 0, st>>>(iters, sink);
+  cudaEventRecord(e1, st);
+  e = cudaEventSynchronize(e1);
+  float t = 0; cudaEventElapsedTime(&t, e0, e1);
+  if (ms) *ms = t;
+  if (flops) *flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)blocks * tpb / (t * 1e-3);
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  return (int)e;
+}

@@ -1,0 +1,200 @@
+// mcqed_api.cpp — the C ABI of include/mcqed.h: argument checks, device upload, launch sequencing.
+// Product code (libmcqed.so); shares nothing with oracle/. No CPU fallback: every device entry
+// point fails with MC_ECUDA if CUDA is unusable.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "diagram.hpp"
+
+namespace {
+std::atomic<unsigned long long> g_launches{0};
+
+int to_device(mc_diagram *d) {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MC_ECUDA;
+  if (!d->have_tables) return MC_EINVAL;
+  const size_t bytes = d->blob.size() * 8;
+  if (cudaMalloc(&d->d_blob, bytes) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMemcpy(d->d_blob, d->blob.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) return MC_ECUDA;
+  if (cudaMalloc(&d->ws.partial, sizeof(double) * 2 * mqk::MAXGRID * 4) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMalloc(&d->ws.flag_list, sizeof(unsigned long long) * mqk::CHUNK) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMalloc(&d->ws.counters, sizeof(unsigned long long) * 4) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMemset(d->ws.counters, 0, sizeof(unsigned long long) * 4) != cudaSuccess) return MC_ECUDA;
+  if (mq_config_f64(d) != 0 || mq_config_dd(d) != 0) return MC_ECUDA;
+  d->on_device = true;
+  return MC_OK;
+}
+}  // namespace
+
+#define MQ_CK(x) do { if ((x) != cudaSuccess) return MC_ECUDA; } while (0)
+
+extern "C" {
+
+int mc_prepare_diagram_host(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out) {
+  try { return mq_prepare_host(graph, forests, opts, out); } catch (const std::bad_alloc &) { return MC_ENOMEM; } catch (...) { return MC_EINVAL; }
+}
+int mc_prepare_diagram(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out) {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MC_ECUDA;   // fail loudly: no CPU fallback
+  mc_diagram *d = nullptr;
+  int rc = mc_prepare_diagram_host(graph, forests, opts, &d);
+  if (rc != MC_OK) return rc;
+  rc = to_device(d);
+  if (rc != MC_OK) { mc_free_diagram(d); return rc; }
+  *out = d;
+  return MC_OK;
+}
+void mc_free_diagram(mc_diagram *d) {
+  if (!d) return;
+  if (d->d_blob) cudaFree(d->d_blob);
+  if (d->ws.partial) cudaFree(d->ws.partial);
+  if (d->ws.flag_list) cudaFree(d->ws.flag_list);
+  if (d->ws.counters) cudaFree(d->ws.counters);
+  delete d;
+}
+int mc_diagram_info(const mc_diagram *d, int32_t *k, int32_t *m, int32_t *n, int32_t *n_terms, int64_t *flop_per_sample, int64_t *table_bytes) {
+  if (!d) return MC_EINVAL;
+  int kk, mm, nn; d->g.classKMN(kk, mm, nn);
+  if (k) *k = kk;
+  if (m) *m = mm;
+  if (n) *n = nn;
+  if (n_terms) *n_terms = (int32_t)d->terms.size();
+  // 2 flop per non-zero numerator monomial (one FMA in the nested evaluation) + ~600 flop per piece (a4) + ~3000 (a1-a3) + 12 per term grade (a6)
+  if (flop_per_sample) *flop_per_sample = 2 * d->n_nonzero + 600 * (int64_t)d->geoms.size() + 3000 + 12 * (int64_t)d->terms.size() * d->g.L;
+  if (table_bytes) *table_bytes = (int64_t)d->blob.size() * 8;
+  return MC_OK;
+}
+int mc_diagram_id(const mc_diagram *d, int32_t *id) { if (!d || !id) return MC_EINVAL; *id = d->id; return MC_OK; }
+int mc_diagram_subgraphs(const mc_diagram *d, int32_t *lo, int32_t *hi, int32_t *type, int32_t cap) {
+  if (!d) return MC_EINVAL;
+  int n = (int)d->ft.subs.size();
+  for (int i = 0; i < n && i < cap; i++) { if (lo) lo[i] = d->ft.subs[i].lo; if (hi) hi[i] = d->ft.subs[i].hi; if (type) type[i] = d->ft.subs[i].vertexLike ? 1 : 0; }
+  return n;
+}
+int mc_diagram_forests(const mc_diagram *d, uint32_t *mask, int32_t cap) {
+  if (!d) return MC_EINVAL;
+  int n = (int)d->ft.forests.size();
+  for (int i = 0; i < n && i < cap; i++) if (mask) mask[i] = d->ft.forests[i];
+  return n;
+}
+int mc_diagram_terms(const mc_diagram *d, uint32_t *forest, int32_t *gprime, int32_t *sign, int32_t cap) {
+  if (!d) return MC_EINVAL;
+  int n = (int)d->ft.terms.size();
+  for (int i = 0; i < n && i < cap; i++) { if (forest) forest[i] = d->ft.terms[i].forest; if (gprime) gprime[i] = d->ft.terms[i].gprime; if (sign) sign[i] = d->ft.terms[i].sign; }
+  return n;
+}
+int mc_diagram_sampler_tables(const mc_diagram *d, double *deg, double *Z, double *C) {
+  if (!d) return MC_EINVAL;
+  size_t n = (size_t)1 << d->g.M;
+  if (deg) std::memcpy(deg, d->st.deg.data(), n * sizeof(double));
+  if (Z) std::memcpy(Z, d->st.Z.data(), n * sizeof(double));
+  if (C) *C = d->st.C;
+  return MC_OK;
+}
+int64_t mc_diagram_blob(const mc_diagram *d, uint64_t *out, int64_t cap) {
+  if (!d) return MC_EINVAL;
+  int64_t n = (int64_t)d->blob.size();
+  if (out) std::memcpy(out, d->blob.data(), sizeof(uint64_t) * (size_t)std::min(n, cap));
+  return n;
+}
+
+int mc_integrate(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                 double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
+  if (!d || !d->on_device) return MC_EINVAL;
+  mq_stream st = (mq_stream)cuda_stream;
+  const bool no_dd = d->opt.flags & 1u;
+  for (uint64_t done = 0; done < n_samples; done += mqk::CHUNK) {
+    const uint64_t n = std::min<uint64_t>(mqk::CHUNK, n_samples - done);
+    const int g1 = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + mqk::TPB_F64 - 1) / mqk::TPB_F64);
+    mq_launch_integrate_f64(d, g1, first_sample + done, n, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min, st);
+    int g2 = 0;
+    if (!no_dd) { g2 = d->grid_dd; mq_launch_integrate_dd(d, seed, st); g_launches++; }
+    mq_launch_finish(d, g1, g2, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
+    g_launches += 2;
+  }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+
+int mc_integrate_host(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                      double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped) {
+  if (!d || !d->on_device) return MC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  struct Out { double s, s2; unsigned long long nf, nd; } *dev = nullptr, host{0, 0, 0, 0};
+  MQ_CK(cudaMallocAsync((void **)&dev, sizeof(Out), st));
+  MQ_CK(cudaMemsetAsync(dev, 0, sizeof(Out), st));
+  int rc = mc_integrate(d, first_sample, n_samples, seed, cuda_stream, &dev->s, &dev->s2, &dev->nf, &dev->nd);
+  if (rc != MC_OK) { cudaFreeAsync(dev, st); return rc; }
+  MQ_CK(cudaMemcpyAsync(&host, dev, sizeof(Out), cudaMemcpyDeviceToHost, st));
+  MQ_CK(cudaFreeAsync(dev, st));
+  MQ_CK(cudaStreamSynchronize(st));
+  if (sum) *sum = host.s;
+  if (sumsq) *sumsq = host.s2;
+  if (n_flagged) *n_flagged = host.nf;
+  if (n_dropped) *n_dropped = host.nd;
+  return MC_OK;
+}
+
+int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
+                   double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out, uint8_t *flag_out) {
+  if (!d || !d->on_device) return MC_EINVAL;
+  mq_stream st = (mq_stream)cuda_stream;
+  const bool no_dd = d->opt.flags & 1u;
+  const int M = d->g.M;
+  for (uint64_t done = 0; done < n; done += mqk::CHUNK) {
+    const uint64_t m = std::min<uint64_t>(mqk::CHUNK, n - done);
+    const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (m + mqk::TPB_EVAL - 1) / mqk::TPB_EVAL);
+    const bool list = f_out && !no_dd;
+    mq_launch_reset(d, st);
+    mq_launch_eval_points(d, g1, first_sample + done, m, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min,
+                          z_out ? z_out + done * M : nullptr, order_out ? order_out + done * M : nullptr, p_out ? p_out + done : nullptr,
+                          f_out ? f_out + done : nullptr, f64_out ? f64_out + done : nullptr, cond_out ? cond_out + done : nullptr,
+                          flag_out ? flag_out + done : nullptr, list, st);
+    g_launches += 2;
+    if (list) { mq_launch_eval_points_dd(d, first_sample + done, seed, f_out + done, st); g_launches++; }
+    mq_launch_reset(d, st);
+    g_launches++;
+  }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+
+int mc_eval_z(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda_stream, double *f64_out, double *fdd_out, double *cond_out, double *aux_out) {
+  if (!d || !d->on_device || !z_in) return MC_EINVAL;
+  if (n == 0) return MC_OK;
+  mq_stream st = (mq_stream)cuda_stream;
+  const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (n + mqk::TPB_EVAL - 1) / mqk::TPB_EVAL);
+  if (f64_out || cond_out || aux_out) { mq_launch_eval_z_f64(d, g1, n, z_in, f64_out, cond_out, aux_out, st); g_launches++; }
+  if (fdd_out) { mq_launch_eval_z_dd(d, g1, n, z_in, fdd_out, st); g_launches++; }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+
+unsigned long long mc_kernel_launch_count(void) { return g_launches.load(); }
+
+int mc_fp64_peak(int iters, void *cuda_stream, double *flops, double *ms) {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MC_ECUDA;
+  if (mq_fp64_peak(iters, (mq_stream)cuda_stream, flops, ms) != 0) return MC_ECUDA;
+  g_launches += 2;
+  return MC_OK;
+}
+
+const char *mc_strerror(int code) {
+  switch (code) {
+    case MC_OK: return "ok";
+    case MC_EINVAL: return "invalid argument or not a valid 1PI vertex graph";
+    case MC_ENOMEM: return "out of memory";
+    case MC_ECUDA: return "CUDA error or no CUDA device (this library has no CPU fallback)";
+    case MC_ELIMIT: return "graph exceeds a compiled-in limit";
+  }
+  return "unknown error";
+}
+const char *mc_version(void) { return "mcqed-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -196,7 +196,7 @@ __device__ __noinline__ T family_dispatch(int c, int kd, const uint8_t *__restri
 // ------------------------------------------------------------------ a4: scalars of one piece
 // writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
 template <class T>
-__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, T &U, T &V, T &G) {
+__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, T &U, T &V, T &G, double &amin, double &xmin) {
   const int n = g.nch, ns = g.nslot;
   T A[MQ_MAXL][MQ_MAXL], Inv[MQ_MAXL][MQ_MAXL];
 #pragma unroll
@@ -262,7 +262,11 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
     S[(off_at + s) * stride] = T(1.0) - x;                    // A_t
     const T sg = T((double)g.slot[s].sgn);
     S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);       // A'_t / g_t
-    if (line) { V = V + x * T(z[g.slot[s].zline]); G = G * gs; }
+    if (line) {
+      V = V + x * T(z[g.slot[s].zline]); G = G * gs;
+      const double xd = mq_to_double(x);
+      amin = fmin(amin, 1.0 - xd); xmin = fmin(xmin, xd);
+    }
   }
   for (int s = 0; s < ns; s++)
     for (int u = s + 1; u < ns; u++) {
@@ -283,23 +287,30 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 }
 
 // ------------------------------------------------------------------ a4-a6: integrand at one point
-// S: shared-memory scalar scratch of this thread (S[index*stride]); nodeval / nodeU / nodeV: per-thread local arrays
+// S: shared-memory scalar scratch of this thread (S[index*stride]); nodeval / nodeU / nodeV: per-thread local arrays.
+// For T = double a second, sign-free copy of the whole computation is carried along at family granularity
+// (|family value| summed, |child value| multiplied): abs_out = sum over terms and grades of that bound. It measures
+// every cancellation between families, pieces and terms (O8) at the cost of one add per family.
 template <class T>
-__device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, T *S, int stride, T &f_out, T &abs_out) {
+__device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, T *S, int stride, T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
+  constexpr bool TRACK = sizeof(T) == sizeof(double);
   const DevHeader &h = *v.h;
   T nodeval[/*worst case*/ 1024];
+  double nodeabs[TRACK ? 1024 : 1];
   T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
+  double amin = 1.0, xmin = 1.0;
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
     T U, V, G;
-    piece_scalars<T>(g, z, S, stride, U, V, G);
+    piece_scalars<T>(g, z, S, stride, U, V, G, amin, xmin);
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
       const DevTable &tb = v.tab[ti];
       T N[2][MQ_MAXPAT][MQ_NGRADE];
+      double Na[TRACK ? 2 : 1][TRACK ? MQ_MAXPAT : 1][MQ_NGRADE];
       for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) N[o][p][c] = T(0.0);
+          for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = 0.0; }
       const uint64_t *st = v.blob + tb.stream_off;
       for (int fi = 0; fi < tb.nfam; fi++) {
         const uint64_t hd = __ldg(st);
@@ -311,6 +322,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, 
         const int nb = c * (2 * c - 1) + kd;
         for (int i = 0; i < nscal; i++) val = val * S[(int)idx[nb + i] * stride];
         N[out][pat][c] = N[out][pat][c] + val;
+        if constexpr (TRACK) Na[out][pat][c] += fabs(mq_to_double(val));
         st += 1 + idxw + ncoef;
       }
       // nodes that use this table: combine with the children's graded values
@@ -320,23 +332,24 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, 
         for (int k = 0; k < nd.nchild; k++) { Up = Up * nodeU[nd.child[k]]; Vs = Vs + nodeV[nd.child[k]]; }
         nodeU[ni] = Up; nodeV[ni] = Vs;
         for (int o = 0; o < nd.nout; o++) {
-          T tot[MQ_NGRADE];
+          T tot[MQ_NGRADE]; double tota[MQ_NGRADE];
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) tot[c] = T(0.0);
+          for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = T(0.0); tota[c] = 0.0; }
           for (int p = 0; p < npat; p++) {
-            T acc[MQ_NGRADE];
+            T acc[MQ_NGRADE]; double acca[MQ_NGRADE];
 #pragma unroll
-            for (int c = 0; c < MQ_NGRADE; c++) acc[c] = N[o][p][c] * G;
+            for (int c = 0; c < MQ_NGRADE; c++) { acc[c] = N[o][p][c] * G; if constexpr (TRACK) acca[c] = Na[o][p][c] * mq_to_double(G); }
             for (int k = 0; k < nd.nchild; k++) {
               const DevNode &ch = v.node[nd.child[k]];
               const int pb = g.child_patbit[k];
               const int which = (pb >= 0 && (p >> pb & 1)) ? 1 : 0;      // S-child: a (0) or b (1); V-child: its single value
               graded_mul<T>(acc, &nodeval[ch.val_off + which * ch.ngr], ch.ngr);
+              if constexpr (TRACK) graded_mul<double>(acca, &nodeabs[ch.val_off + which * ch.ngr], ch.ngr);
             }
 #pragma unroll
-            for (int c = 0; c < MQ_NGRADE; c++) tot[c] = tot[c] + acc[c];
+            for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = tot[c] + acc[c]; if constexpr (TRACK) tota[c] += acca[c]; }
           }
-          for (int c = 0; c < nd.ngr; c++) nodeval[nd.val_off + o * nd.ngr + c] = tot[c];
+          for (int c = 0; c < nd.ngr; c++) { nodeval[nd.val_off + o * nd.ngr + c] = tot[c]; if constexpr (TRACK) nodeabs[nd.val_off + o * nd.ngr + c] = tota[c]; }
         }
       }
     }
@@ -353,11 +366,14 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, 
     for (int c = L - 1; c >= 0; c--) {
       Vp = Vp * Vs;
       if (L - c - 1 > 0) fact *= (double)(L - c - 1);
-      T contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : T(0.0)) * T(fact * (double)tm.sign) / (U2 * Vp);
-      f = f + contrib; asum = asum + mq_abs(contrib);
+      const T scale = T(fact * (double)tm.sign) / (U2 * Vp);
+      const T contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : T(0.0)) * scale;
+      f = f + contrib;
+      if constexpr (TRACK) asum = asum + T(c < nd.ngr ? nodeabs[nd.val_off + c] * fabs(mq_to_double(scale)) : 0.0);
+      else asum = asum + mq_abs(contrib);
     }
   }
-  f_out = f; abs_out = asum;
+  f_out = f; abs_out = asum; amin_out = amin; xmin_out = xmin;
 }
 
 }  // namespace mqk

@@ -1,0 +1,145 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C ABI against the CPU oracle, element by element
+on the same seeded points (north_star tolerances):
+  * sample coordinates, sector and density: bit-exact;
+  * per-point integrand: relative 1e-10 against the oracle's wide value for unflagged points; flagged
+    points are compared separately (their double-double value against the wide value);
+  * fixed-point-set sums: relative 1e-9; final estimates: within the combined 1-sigma error.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def mc():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1905_08007_b200 import binding, build
+    build.build()
+    return binding
+
+
+def _gpu_points(mc, d, first, n, seed):
+    dev = "cuda"
+    z = torch.zeros(n, d.M, dtype=torch.float64, device=dev)
+    order = torch.zeros(n, d.M, dtype=torch.int32, device=dev)
+    p, f, f64, cond = (torch.zeros(n, dtype=torch.float64, device=dev) for _ in range(4))
+    flag = torch.zeros(n, dtype=torch.uint8, device=dev)
+    d.eval_points(first, n, seed, torch.cuda.current_stream().cuda_stream, z, order, p, f, f64, cond, flag)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in dict(z=z, order=order, p=p, f=f, f64=f64, cond=cond, flag=flag).items()}
+
+
+CASES = [(1, [0], 4099, 1), (2, list(range(6)), 2053, 2), (3, [0, 7, 8, 9, 18, 29, 38, 47], 517, 3), (4, [1, 100, 305], 131, 4)]
+
+
+@pytest.mark.parametrize("L,idxs,n,seed", CASES)
+def test_points_bit_exact_and_integrand_parity(po, mc, L, idxs, n, seed):
+    for i in idxs:
+        g = po.graph_get(L, i)
+        o = po.Diagram(g)
+        d = mc.Diagram(L, g.ext_pos, g.chords())
+        first = 1000003 * i + 17                     # not a multiple of any tile size; ragged n
+        r = _gpu_points(mc, d, first, n, seed)
+        z, p, order = o.sample(first, n, seed)
+        assert np.array_equal(r["z"], z), "sample coordinates must be bit-exact"
+        assert np.array_equal(r["order"], order), "Hepp sector must be identical"
+        assert np.array_equal(r["p"], p), "density must be bit-exact"
+        ref = o.eval_z(z, wide=True)
+        fw = ref["fwide"]
+        unfl = r["flag"] == 0
+        assert unfl.sum() > 0
+        rel = np.abs(r["f"] - fw) / np.abs(fw)
+        assert np.all(rel[unfl] <= 1e-10), (L, i, rel[unfl].max())
+        # flagged points: the double-double value against the oracle's wide value
+        assert np.all(rel[~unfl] <= 1e-10), (L, i, rel[~unfl].max() if (~unfl).any() else 0)
+        # the proxy has no false negatives against the oracle's truth flag (O8)
+        truth = np.abs(ref["f64"] - fw) > 1e-10 * np.abs(fw)
+        assert not np.any(truth & unfl), "a point that loses precision in binary64 was not flagged"
+        # fixed-point-set sums
+        w_gpu, w_ref = r["f"] / r["p"], fw / p
+        assert abs(w_gpu.sum() - w_ref.sum()) <= 1e-9 * np.abs(w_ref).sum()
+        d.close()
+
+
+@pytest.mark.parametrize("L,idx,n,seed", [(1, 0, 1 << 20, 1), (2, 3, 300007, 2), (2, 1, 300007, 2), (3, 8, 65537, 3)])
+def test_integrate_sums_match_eval_points_and_oracle(po, mc, L, idx, n, seed):
+    g = po.graph_get(L, idx)
+    d = mc.Diagram(L, g.ext_pos, g.chords())
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    # two calls with disjoint ranges accumulate (+=): ragged split
+    n1 = n // 3 + 1
+    d.integrate(5, n1, seed, st, out[0:1], out[1:2], cnt[0:1], cnt[1:2])
+    d.integrate(5 + n1, n - n1, seed, st, out[0:1], out[1:2], cnt[0:1], cnt[1:2])
+    torch.cuda.synchronize()
+    s1, s2 = out.cpu().numpy()
+    nflag, ndrop = cnt.cpu().numpy()
+    assert ndrop == 0
+    r = _gpu_points(mc, d, 5, n, seed)
+    w = r["f"] / r["p"]
+    assert int(r["flag"].sum()) == nflag
+    assert abs(s1 - math.fsum(w)) <= 1e-12 * math.fsum(np.abs(w))
+    assert abs(s2 - math.fsum(w * w)) <= 1e-12 * math.fsum(w * w)
+    # host-output variant gives the same numbers
+    h1, h2, hf, hd = d.integrate_host(5, n, seed, st)
+    assert abs(h1 - s1) <= 1e-13 * abs(s1) + 1e-300 and hf == nflag and hd == 0
+    # oracle on a bounded sample of the same points: fixed-set sums within 1e-9, estimate within 1 sigma
+    m = min(n, 20000)
+    o = po.Diagram(g)
+    os1, os2, _ = o.integrate(5, m, seed, 1)
+    gs1 = math.fsum(w[:m])
+    assert abs(gs1 - os1) <= 1e-9 * math.fsum(np.abs(w[:m]))
+    mean, err = po.estimate(s1, s2, n)
+    omean, oerr = po.estimate(os1, os2, m)
+    assert abs(mean - omean) <= math.hypot(err, oerr) * 3.0
+    d.close()
+
+
+def test_one_loop_estimate_is_one_half(mc):
+    d = mc.Diagram(1, 1, [(0, 2)])
+    n = 4_000_000
+    s1, s2, nf, nd = d.integrate_host(0, n, 1)
+    mean = s1 / n
+    err = math.sqrt(max(s2 / n - mean * mean, 0) / n)
+    assert abs(mean - 0.5) < 4 * err and err < 1e-3 and nd == 0
+
+
+def test_edge_cases(mc):
+    d = mc.Diagram(2, 2, [(0, 3), (1, 4)])
+    assert d.integrate_host(0, 0, 1) == (0.0, 0.0, 0, 0)               # empty range
+    a = d.integrate_host(123, 1, 9)                                   # single point
+    b = d.integrate_host(123, 1, 9)
+    assert a == b and a[0] != 0.0
+    big = (1 << 40) + 12345                                           # 64-bit sample indices reach the counter
+    c = d.integrate_host(big, 1000, 9)
+    e = d.integrate_host(big & 0xFFFFFFFF, 1000, 9)
+    assert c[0] != e[0]
+    # additivity over a chunk boundary (CHUNK = 2^22 samples per launch)
+    n = (1 << 22) + 777
+    whole = d.integrate_host(0, n, 4)
+    p1 = d.integrate_host(0, 1 << 22, 4)
+    p2 = d.integrate_host(1 << 22, 777, 4)
+    assert abs(whole[0] - (p1[0] + p2[0])) <= 1e-12 * abs(whole[0])
+    assert whole[2] == p1[2] + p2[2]
+
+
+def test_eval_z_double_double_agrees_with_oracle_wide(po, mc):
+    g = po.graph_get(3, 7)                      # two adjacent self-energy insertions: heavy cancellation
+    o = po.Diagram(g)
+    d = mc.Diagram(3, g.ext_pos, g.chords())
+    z, p, _ = o.sample(0, 400, 5)
+    zt = torch.tensor(z, device="cuda")
+    f64, fdd, cond = (torch.zeros(len(z), dtype=torch.float64, device="cuda") for _ in range(3))
+    d.eval_z(len(z), zt, torch.cuda.current_stream().cuda_stream, f64, fdd, cond)
+    torch.cuda.synchronize()
+    ref = o.eval_z(z, wide=True)
+    rel = np.abs(fdd.cpu().numpy() - ref["fwide"]) / np.abs(ref["fwide"])
+    assert rel.max() <= 1e-10
+    d.close()
