@@ -1,0 +1,244 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Monte Carlo hot path on BASELINE.json configs[4] (5-loop graphs).
+
+Contract (driver): python bench.py --gpus N --steps K --warmup W [--impl reference]; under torchrun for N>1.
+A "step" is one pass of the whole hot path (sampler, scalars, integrand with all subtraction terms, weight,
+reduction, double-double re-evaluation of flagged points) over one batch of --batch sample points for EVERY
+diagram of the workload. The workload is the 256 seeded 5-loop graphs of configs[4] (A12); the
+path shards trivially (independent sample-index ranges), so N GPUs run N replicas on disjoint ranges with no
+data-path collective: scaling is "weak".
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "5-loop integrand samples/s on 1 B200; % of FP64 peak; sigma^2*time"
+UNIT = "samples/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (4 = the metric's workload)")
+    ap.add_argument("--graphs", type=int, default=0, help="use only the first G graphs of the config (0 = all; for debugging)")
+    ap.add_argument("--batch", type=int, default=1 << 13, help="sample points per diagram per step")
+    ap.add_argument("--ref-points", type=int, default=768, help="oracle sample points per step (reference arm / cpu_baseline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler(threading.Thread):
+    """samples nvidia-smi clocks and throttle reasons during the timed region"""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        mx = max((int(r[1]) for r in self.rows if r[1].isdigit()), default=0)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else 0, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_run(args, graphs, seed, steps, warmup):
+    """times the CPU oracle as it stands on a bounded sample of the workload: the first graph(s) of the set"""
+    from oracle import pyoracle as po
+    idx, g = graphs[0]
+    og = po.OracleGraph.make(g[0], g[1], g[2])
+    t0 = time.perf_counter()
+    d = po.Diagram(og)
+    prep = time.perf_counter() - t0
+    n = args.ref_points
+    for w in range(warmup):
+        d.integrate(w * n, n, seed, 2)
+    t0 = time.perf_counter()
+    s1 = s2 = 0.0
+    for k in range(steps):
+        a, b, _ = d.integrate((warmup + k) * n, n, seed, 2)
+        s1 += a
+        s2 += b
+    dt = time.perf_counter() - t0
+    tot = n * steps
+    mean, err = po.estimate(s1, s2, tot)
+    return {"value": tot / dt, "seconds": dt, "cores": po.num_threads(), "prepare_s": prep, "points": tot,
+            "sample": "graph #%d of the workload (canonical index %d), %d points per step, binary64 + __float128 re-evaluation" % (0, idx, n),
+            "mean": mean, "err": err, "sigma2_time": err * err * dt}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1905_08007_b200 import workloads
+    graphs = workloads.config_graphs(args.config)
+    seed = workloads.CONFIG_SEED[args.config]
+    r = oracle_run(args, graphs, seed, max(1, args.steps), args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * r["seconds"] / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": "configs[%d] (bounded sample)" % args.config, "sample": r["sample"]},
+            "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1905_08007_b200 import binding as mc
+    from paper_1905_08007_b200 import build, workloads
+    build.build()
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    graphs = workloads.config_graphs(args.config)
+    if args.graphs:
+        graphs = graphs[:args.graphs]
+    seed = workloads.CONFIG_SEED[args.config]
+    G, B = len(graphs), args.batch
+    # ---- prepare (not timed as throughput; reported) ----
+    t0 = time.perf_counter()
+    diagrams = [mc.Diagram(g[0], g[1], g[2]) for _, g in graphs]
+    prepare_s = time.perf_counter() - t0
+    infos = [d.info() for d in diagrams]
+    flop = [i["flop_per_sample"] for i in infos]
+    stream = torch.cuda.current_stream().cuda_stream
+    sums = torch.zeros(G, 2, dtype=torch.float64, device="cuda")
+    cnts = torch.zeros(G, 2, dtype=torch.int64, device="cuda")
+    state = {"first": rank * (1 << 44)}        # disjoint sample-index ranges per rank (weak scaling, no collective)
+
+    def step():
+        f = state["first"]
+        for i, d in enumerate(diagrams):
+            d.integrate(f, B, seed, stream, sums[i, 0:1], sums[i, 1:2], cnts[i, 0:1], cnts[i, 1:2])
+        state["first"] = f + B
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    def timed(nsteps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(nsteps):
+            step()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(args.warmup):
+        step()
+    sums.zero_(); cnts.zero_()
+    clocks = ClockSampler(local)
+    clocks.start()
+    l0 = mc.kernel_launch_count()
+    ms = timed(args.steps)
+    launches = mc.kernel_launch_count() - l0
+    clocks.stop_flag = True
+    clocks.join(timeout=2)
+    n_tot = args.steps * B
+    s = sums.cpu().numpy(); c = cnts.cpu().numpy()
+    value = world * G * n_tot / (ms * 1e-3)
+    var_sum = 0.0
+    for i in range(G):
+        mean = s[i, 0] / n_tot
+        var_sum += max(s[i, 1] / n_tot - mean * mean, 0.0) / n_tot
+    flagged_frac = float(c[:, 0].sum()) / (G * n_tot)
+    # ---- per-kernel times: the same steps with the double-double pass switched off time k_integrate_f64 alone ----
+    for d in diagrams:
+        d.set_flags(mc.FLAG_NO_DD)
+    step()
+    ms_f64 = timed(args.steps)
+    for d in diagrams:
+        d.set_flags(0)
+    ms_dd = max(ms - ms_f64, 0.0)
+    peak_flops, _ = mc.fp64_peak(4096)
+    flops_f64 = sum(flop) * n_tot                                    # every point goes through the binary64 kernel
+    flops_dd = float(sum(fl * cc for fl, cc in zip(flop, c[:, 0])))  # flagged points are re-evaluated (same algorithmic flop)
+    ach_f64 = flops_f64 / (ms_f64 * 1e-3) if ms_f64 > 0 else 0.0
+    ach_dd = flops_dd / (ms_dd * 1e-3) if ms_dd > 0 else 0.0
+    dom = "k_integrate_dd" if ms_dd > ms_f64 else "k_integrate_f64"
+    ach = ach_dd if dom == "k_integrate_dd" else ach_f64
+    roofline = {"bound": "alu", "kernel": dom, "achieved": ach / 1e12, "peak": peak_flops / 1e12, "unit": "TFLOP/s", "frac": ach / peak_flops,
+                "traffic": None, "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
+                "kernels": {"k_integrate_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
+                            "k_integrate_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
+                                               "points_per_step": float(c[:, 0].sum()) / args.steps,
+                                               "note": "double-double: ~20 binary64 flop per algorithmic flop, so frac is bounded by ~0.05"}}}
+    # ---- end to end through the public host-pointer API (mc_integrate_host: results copied back every call) ----
+    barrier()
+    t0 = time.perf_counter()
+    f = state["first"]
+    for _ in range(args.steps):
+        for d in diagrams:
+            d.integrate_host(f, B, seed, stream)
+        f += B
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": world * G * n_tot / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 32 * G,
+           "note": "inputs are (first_sample, n, seed) scalars: no host->device tensor; 4 results (32 B) per diagram come back per step"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[%d]: %d seeded 5-loop graphs without lepton loops, %d points per graph per step" % (args.config, G, B) if args.config == 4
+                       else "configs[%d]: %d graphs, %d points per graph per step" % (args.config, G, B),
+                       "n_graphs": G, "batch": B, "seed": seed, "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
+                       "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "dropped": int(c[:, 1].sum()),
+                       "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[:, 0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
+                       "algorithmic_flop_per_sample_mean": sum(flop) / G},
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = oracle_run(args, graphs, seed, 1, 0)
+        line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+                                "prepare_s": r["prepare_s"], "sigma2_time_s": r["sigma2_time"]}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

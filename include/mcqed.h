@@ -93,6 +93,10 @@ int mc_diagram_terms(const mc_diagram *, uint32_t *forest, int32_t *gprime, int3
 /* Sampler tables of Eq.(1): deg and Z have 2^M entries, C is the normalisation. HOST outputs. */
 int mc_diagram_sampler_tables(const mc_diagram *, double *deg, double *Z, double *C);
 
+/* Changes the run-time flag bits of mc_options.flags on an existing handle (bit 0: skip the double-double
+ * pass). Used by bench.py to time the binary64 kernel alone. HOST. */
+int mc_diagram_set_flags(mc_diagram *, uint32_t flags);
+
 /* Host copy of the device table blob (layout: csrc/device_layout.h), for format tests. Returns the
  * number of 8-byte words; copies min(words, cap) words into out (may be NULL). HOST. */
 int64_t mc_diagram_blob(const mc_diagram *, uint64_t *out, int64_t cap);

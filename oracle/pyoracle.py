@@ -118,7 +118,7 @@ def philox(ctr, key):
 class Diagram:
     """One prepared diagram (combinatorics + sampler tables [+ integrand tables])."""
 
-    def __init__(self, g, deg_floor=0.5, deg_cap=1e30, level=1, prune=1):
+    def __init__(self, g, deg_floor=0.75, deg_cap=1e30, level=1, prune=1):
         self.g = g
         self.h = C.c_void_p()
         rc = lib().oracle_prepare_diagram(C.byref(g), deg_floor, deg_cap, level, prune, C.byref(self.h))

@@ -87,6 +87,8 @@ static void FN(eval_node)(const struct oracle_diagram *d, int ni, const REAL *z,
     }
     for (int o = 0; o < tab->nout; o++) N[o][m->pattern][m->grade] += (REAL)m->coef[o] * prod;
   }
+  if (h->type == 1 && (nd->op == OP_U || nd->op == OP_LMU))     /* these tables hold 12*coefficient (qed_tables.h func_UV12) */
+    for (int pat = 0; pat < npat; pat++) for (int c = 0; c < NGRADE; c++) N[0][pat][c] /= 12;
   for (int o = 0; o < 2; o++) for (int c = 0; c < NGRADE; c++) nv->v[o][c] = 0;
   for (int o = 0; o < tab->nout; o++)
     for (int pat = 0; pat < npat; pat++) {

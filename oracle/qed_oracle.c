@@ -156,8 +156,7 @@ int oracle_prepare_diagram(const oracle_graph *og, double deg_floor, double deg_
     for (int k = 0; k < d->nnode; k++) need[d->nodes[k].geom][d->nodes[k].op] = 1;
     int jobs[MAXGEOM * 4][2], njob = 0;
     for (int k = 0; k < d->ngeom; k++) for (int op = 0; op < 4; op++) if (need[k][op]) { jobs[njob][0] = k; jobs[njob][1] = op; njob++; }
-#pragma omp parallel for schedule(dynamic, 1)
-    for (int j = 0; j < njob; j++) {
+    for (int j = 0; j < njob; j++) {   /* each table build is parallel inside (qed_tables.h) */
       int k = jobs[j][0], op = jobs[j][1];
       PieceTable *t = (PieceTable *)calloc(1, sizeof(PieceTable));
       int mg = -1;

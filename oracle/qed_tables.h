@@ -58,8 +58,18 @@ static cplx trace4(const cplx A[4][4]) { return A[0][0] + A[1][1] + A[2][2] + A[
 enum { AX_CHORD = 0, AX_KAPPA = 1, AX_MU = 2, AX_NU = 3 };
 typedef struct { int nax; int tag[14], id[14]; cplx (*m)[4][4]; } Tens;
 
-static Tens tens_alloc(int nax) { Tens t; t.nax = nax; t.m = (cplx(*)[4][4])malloc(sizeof(cplx) * 16 * ((size_t)1 << (2 * nax))); return t; }
-static void tens_free(Tens *t) { free(t->m); t->m = NULL; }
+/* tensors live on a per-thread LIFO arena (the depth-first walk frees in reverse order of allocation) */
+static __thread char *tens_arena = NULL;
+static __thread size_t tens_top = 0, tens_cap = 0;
+static Tens tens_alloc(int nax) {
+  Tens t; t.nax = nax;
+  size_t bytes = sizeof(cplx) * 16 * ((size_t)1 << (2 * nax));
+  if (!tens_arena) { tens_cap = (size_t)6 << 30; tens_arena = (char *)malloc(tens_cap); /* virtual; touched lazily */ }
+  if (tens_top + bytes > tens_cap) { fprintf(stderr, "oracle: tensor arena exhausted\n"); abort(); }
+  t.m = (cplx(*)[4][4])(tens_arena + tens_top); tens_top += bytes;
+  return t;
+}
+static void tens_free(Tens *t) { tens_top -= sizeof(cplx) * 16 * ((size_t)1 << (2 * t->nax)); t->m = NULL; }
 static Tens tens_open(const Tens *src, int tag, int id) {     /* T'[.., rho] = gamma^rho T[..] */
   Tens t = tens_alloc(src->nax + 1);
   memcpy(t.tag, src->tag, sizeof(int) * src->nax); memcpy(t.id, src->id, sizeof(int) * src->nax);
@@ -102,13 +112,17 @@ static cplx func_L(cplx X[4][4][4]) {
   memcpy(P, G0, sizeof P); for (int i = 0; i < 4; i++) P[i][i] += 1.0;
   matmul(P, X[0], T); return trace4(T) / 4.0;
 }
-/* U_V[X] = ( Tr[gamma_mu X^mu] - Tr[pslash p_mu X^mu]/m^2 ) / 12 */
-static cplx func_UV(cplx X[4][4][4]) {
+/* U_V[X] = ( Tr[gamma_mu X^mu] - Tr[pslash p_mu X^mu]/m^2 ) / 12.  func_UV12 returns 12 U_V[X]: the
+ * traces are integers, so 12 U_V is exactly representable while U_V (a multiple of 1/12) is not; tables
+ * of the operators U and (L-U) on vertex-like pieces therefore store 12*coefficient and the evaluation
+ * divides by 12 once in its working precision (O5, "exact coefficients") */
+static cplx func_UV12(cplx X[4][4][4]) {
   cplx s = 0, G[4][4], T[4][4];
   for (int mu = 0; mu < 4; mu++) { dense_gamma(mu, G); matmul(G, X[mu], T); s += GMET[mu] * trace4(T); }
   dense_gamma(0, G); matmul(G, X[0], T); s -= trace4(T);
-  return s / 12.0;
+  return s;
 }
+static cplx func_UV(cplx X[4][4][4]) { return func_UV12(X) / 12.0; }
 /* R[T] = sum_{jkl} eps_jkl Tr[ Sigma^l P+ T^{jk} ] with
  * T^{jk} = (ps+m) Y^{jk} (ps+m) + 1/2 g^k X^j (ps+m) - 1/2 (ps+m) X^j g^k   (j,k spatial) */
 static void sigma_Pplus(int l, cplx S[4][4]) { /* Sigma^l P+ , Sigma^l = diag(sigma^l, sigma^l) */
@@ -153,7 +167,10 @@ typedef struct {
   int nfac; struct { unsigned char kind, i, j; } fac[MAXFAC];
   int grade, pattern, used_q, max_grade;
   int nopenk;
+  int spawn_at;                 /* element index at which the walk is cut into independent sub-walks (-1: never) */
+  struct Frontier *front;
 } Dfs;
+typedef struct Frontier { int n, cap; struct FrontierItem { Dfs d; Tens T; } *item; } Frontier;
 
 static void table_push(PieceTable *t, const Monomial *m) {
   if (t->n == t->cap) { t->cap = t->cap ? 2 * t->cap : 256; t->mono = (Monomial *)realloc(t->mono, sizeof(Monomial) * t->cap); }
@@ -168,8 +185,8 @@ static void dfs_leaf(Dfs *d, const Tens *T) {
   } else if (!d->used_q) {
     cplx X[4][4][4]; memcpy(X, T->m, sizeof X);   /* single axis MU */
     if (d->op == OP_L) out[0] = func_L(X);
-    else if (d->op == OP_U) out[0] = func_UV(X);
-    else if (d->op == OP_LMU) out[0] = func_L(X) - func_UV(X);
+    else if (d->op == OP_U) out[0] = func_UV12(X);                         /* 12 * coefficient, see func_UV12 */
+    else if (d->op == OP_LMU) out[0] = 12.0 * func_L(X) - func_UV12(X);     /* 12 * coefficient */
     else out[0] = func_R_X(X) / d->Rg - func_L(X);
   } else {
     int amu = tens_find(T, AX_MU, -1), anu = tens_find(T, AX_NU, -1);
@@ -205,6 +222,15 @@ static void dfs_choice_fixed(Dfs *d, int ei, const Tens *T, const double diag[4]
 static void dfs_step(Dfs *d, int ei, const Tens *T) {
   const Geom *h = d->h;
   if (ei == h->nelem) { if (d->nopenk == 0) dfs_leaf(d, T); return; }
+  if (ei == d->spawn_at && d->front) {     /* save the state; the sub-walk is run later, possibly on another thread */
+    Frontier *f = d->front;
+    if (f->n == f->cap) { f->cap = f->cap ? 2 * f->cap : 64; f->item = (struct FrontierItem *)realloc(f->item, sizeof(struct FrontierItem) * f->cap); }
+    struct FrontierItem *it = &f->item[f->n++];
+    it->d = *d; it->d.front = NULL; it->T = *T;
+    size_t bytes = sizeof(cplx) * 16 * ((size_t)1 << (2 * T->nax));
+    it->T.m = (cplx(*)[4][4])malloc(bytes); memcpy(it->T.m, T->m, bytes);
+    return;
+  }
   /* not enough slots left to close the open kappas? */
   int slots_left = 0;
   for (int k = ei; k < h->nelem; k++) if (h->elem[k].kind == EL_SLOT) slots_left++;
@@ -268,9 +294,24 @@ static void build_piece_table(const Geom *h, int op, int max_grade, PieceTable *
   Dfs d; memset(&d, 0, sizeof d);
   d.h = h; d.op = op; d.tab = tab; d.Rg = R_gamma();
   d.max_grade = max_grade < 0 ? 99 : max_grade;
+  Frontier fr; memset(&fr, 0, sizeof fr);
+  d.spawn_at = h->nelem > 8 ? 6 : -1; d.front = d.spawn_at >= 0 ? &fr : NULL;
   Tens T = tens_alloc(0);
   memset(T.m[0], 0, sizeof(cplx) * 16); for (int i = 0; i < 4; i++) T.m[0][i][i] = 1.0;
   dfs_step(&d, 0, &T);
   tens_free(&T);
+  if (fr.n) {   /* run the sub-walks in parallel, then concatenate their monomials in walk order */
+    PieceTable *part = (PieceTable *)calloc(fr.n, sizeof(PieceTable));
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < fr.n; k++) {
+      Dfs sub = fr.item[k].d; sub.tab = &part[k]; sub.front = NULL;
+      dfs_step(&sub, sub.spawn_at, &fr.item[k].T);
+    }
+    for (int k = 0; k < fr.n; k++) {
+      for (int i = 0; i < part[k].n; i++) table_push(tab, &part[k].mono[i]);
+      free(part[k].mono); free(fr.item[k].T.m);
+    }
+    free(part); free(fr.item);
+  }
 }
 #endif

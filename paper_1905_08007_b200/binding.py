@@ -15,7 +15,7 @@ FLAG_NO_DD, FLAG_NO_TABLES = 1, 2
 
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
-    "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob",
+    "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags",
     "mc_integrate", "mc_integrate_host", "mc_eval_points", "mc_eval_z", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
@@ -68,6 +68,7 @@ def lib():
         L.mc_diagram_sampler_tables.argtypes = [vp, dp, dp, dp]
         L.mc_diagram_blob.argtypes = [vp, C.POINTER(C.c_uint64), C.c_int64]
         L.mc_diagram_blob.restype = C.c_int64
+        L.mc_diagram_set_flags.argtypes = [vp, C.c_uint32]
         L.mc_integrate.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -108,7 +109,7 @@ def make_graph(loops, ext_pos, chords):
 class Diagram:
     """RAII handle around mc_diagram*"""
 
-    def __init__(self, loops, ext_pos, chords, deg_floor=0.5, deg_cap=1e30, cond_max=4096.0, amin_min=1e-5, flags=0, host_only=False, forests=None):
+    def __init__(self, loops, ext_pos, chords, deg_floor=0.75, deg_cap=1e30, cond_max=1e4, amin_min=1e-2, flags=0, host_only=False, forests=None):
         self.loops, self.M = loops, 3 * loops
         g = make_graph(loops, ext_pos, chords)
         opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags)
@@ -162,6 +163,9 @@ class Diagram:
         dp = C.POINTER(C.c_double)
         _check(lib().mc_diagram_sampler_tables(self.h, deg.ctypes.data_as(dp), Z.ctypes.data_as(dp), C.byref(Cn)), "mc_diagram_sampler_tables")
         return deg, Z, Cn.value
+
+    def set_flags(self, flags):
+        _check(lib().mc_diagram_set_flags(self.h, flags), "mc_diagram_set_flags")
 
     def blob(self):
         n = lib().mc_diagram_blob(self.h, None, 0)

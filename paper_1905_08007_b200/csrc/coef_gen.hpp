@@ -17,6 +17,8 @@
 #pragma once
 #include <atomic>
 #include <complex>
+#include <cstring>
+#include <functional>
 #include <thread>
 
 #include "host_model.hpp"
@@ -37,8 +39,9 @@ namespace detail {
 static const int8_t G_DST[4][4] = {{0, 1, 2, 3}, {3, 2, 1, 0}, {3, 2, 1, 0}, {2, 3, 0, 1}};
 static const int8_t G_PH[4][4] = {{0, 0, 2, 2}, {2, 2, 0, 0}, {3, 1, 1, 3}, {2, 0, 0, 2}};
 
-enum { W_FIX, W_OPEN, W_CLOSE, W_BIN, W_G0 };
-struct WElem { uint8_t type, arg; };
+enum { W_FIX = MQ_W_FIX, W_OPEN = MQ_W_OPEN, W_CLOSE = MQ_W_CLOSE, W_BIN = MQ_W_BIN, W_G0 = MQ_W_G0 };
+using WElem = MqWElem;
+using CountUnit = MqCountUnit;
 
 struct Variant {               // one trace of the operator functional
   int freeIdx, qIdx, prepend, append;     // Lorentz index of the free vertex / q-slot; extra gamma applied first / last (-1 none)
@@ -46,11 +49,11 @@ struct Variant {               // one trace of the operator functional
   int out;
 };
 
+// integer path counting on the host (the same walk runs as a CUDA kernel in prep_kernel.cu)
 struct Walker {
   const WElem *el; int n; int start;
   int8_t rho[16];
-  std::complex<double> weight;
-  std::complex<double> *acc;   // [2^k]
+  int32_t *acc;   // [2^k][2]
   void go(int pos, int s, int ph, uint32_t sig) {
     for (; pos < n; pos++) {
       const WElem e = el[pos];
@@ -65,8 +68,7 @@ struct Walker {
       }
     }
     if (s != start) return;
-    static const std::complex<double> I4[4] = {{1, 0}, {0, 1}, {-1, 0}, {0, -1}};
-    acc[sig] += weight * I4[ph & 3];
+    acc[2 * sig + (ph & 1)] += (ph & 2) ? -1 : 1;
   }
 };
 
@@ -75,7 +77,9 @@ inline std::vector<Variant> variantsFor(int op, bool sType, bool hasQ) {
   std::vector<Variant> v;
   const cd i(0, 1);
   auto L = [&](double sc) { v.push_back({0, -1, -1, -1, {cd(0.5 * sc), cd(0.5 * sc), 0, 0}, 0}); };
-  auto U = [&](double sc) { for (int j = 1; j <= 3; j++) v.push_back({j, -1, -1, j, {cd(-sc / 12), cd(-sc / 12), cd(-sc / 12), cd(-sc / 12)}, 0}); };
+  // U_V = -(1/12) sum_j Tr[gamma^j X^j] is a multiple of 1/12: tables of U and (L-U) on vertex-like pieces store
+  // 12*coefficient (exactly representable); the kernel divides by 12 once in its working precision
+  auto U = [&](double sc) { for (int j = 1; j <= 3; j++) v.push_back({j, -1, -1, j, {cd(-sc), cd(-sc), cd(-sc), cd(-sc)}, 0}); };
   if (sType) {            // U on an electron self-energy: a = Tr S/4, b = Tr[gamma^0 S]/4
     v.push_back({-1, -1, -1, -1, {0.25, 0.25, 0.25, 0.25}, 0});
     v.push_back({-1, -1, -1, 0, {0.25, 0.25, 0.25, 0.25}, 1});
@@ -84,7 +88,7 @@ inline std::vector<Variant> variantsFor(int op, bool sType, bool hasQ) {
   switch (op) {
     case MQ_OP_L: L(1); break;
     case MQ_OP_U: U(1); break;
-    case MQ_OP_LMU: L(1); U(-1); break;
+    case MQ_OP_LMU: L(12); U(-1); break;      // 12 (L - U)
     case MQ_OP_A:
       if (!hasQ) {        // [ (g2 X1 - X1 g2)_00 - (..)_11 ]/(4i) - (X0_00 + X0_11)/2      (O4)
         v.push_back({1, -1, -1, 2, {-0.25 * i, 0.25 * i, 0, 0}, 0});
@@ -117,7 +121,10 @@ enum Role : uint8_t { R_BIN, R_INS_A, R_INS_BP, R_PAIRED, R_Q };
 
 struct RoleJob { std::vector<uint8_t> role; int c; bool hasQ; };
 
-inline TableBuild buildTable(const Piece &p, int op, int nthreads) {
+// optional accelerator: counts all units on the GPU (prep_kernel.cu); returns 0 on success
+using GpuCountFn = int (*)(const detail::CountUnit *units, size_t nunits, int32_t *counts, size_t nints);
+
+inline TableBuild buildTable(const Piece &p, int op, int nthreads, GpuCountFn gpuCount = nullptr) {
   using namespace detail;
   TableBuild tb;
   const bool sType = !p.seg.vertexLike;
@@ -141,102 +148,123 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads) {
   std::vector<std::vector<std::vector<std::pair<int, int>>>> pairingsOf(maxc + 1);
   for (int c = 0; c <= maxc; c++) allPairings(2 * c, pairingsOf[c]);
 
-  std::vector<std::vector<Family>> famsOf(jobs.size());
-  std::atomic<size_t> next{0};
-  auto worker = [&]() {
-    std::vector<std::complex<double>> acc;
-    for (;;) {
-      size_t j = next.fetch_add(1);
-      if (j >= jobs.size()) break;
-      const RoleJob &job = jobs[j];
-      std::vector<int> binSlots, pairedSlots, atSlots; int qSlot = -1, pattern = 0;
-      for (int s = 0; s < nslot; s++) {
-        Role r = (Role)job.role[s];
-        if (r == R_BIN) binSlots.push_back(s);
-        if (r == R_PAIRED) pairedSlots.push_back(s);
-        if (r == R_INS_BP) atSlots.push_back(s);
-        if (r == R_Q) qSlot = s;
-        if (p.slots[s].insertion && r != R_INS_A) pattern |= 1 << p.patbit[p.slots[s].child];
-      }
-      const int k = (int)binSlots.size(), c = job.c;
-      const auto &pairings = pairingsOf[c];
-      const size_t nsig = (size_t)1 << k;
-      auto variants = variantsFor(op, sType, job.hasQ);
-      // coefficient matrix [out][pairing][sigma]
-      std::vector<double> cm((size_t)tb.nout * pairings.size() * nsig, 0.0);
-      double pref = 1.0;
-      for (int i = 0; i < nch; i++) pref *= -0.25;
-      for (int i = 0; i < c; i++) pref *= -0.5;
-      std::vector<int> pairIdOfSlot(nslot, -1), binIdx(nslot, -1);
-      for (int b = 0; b < k; b++) binIdx[binSlots[b]] = b;
-      for (size_t pi = 0; pi < pairings.size(); pi++) {
-        std::vector<int> firstOfPair(nslot, 0);
-        for (int q = 0; q < c; q++) {
-          pairIdOfSlot[pairedSlots[pairings[pi][q].first]] = nch + q; firstOfPair[pairedSlots[pairings[pi][q].first]] = 1;
-          pairIdOfSlot[pairedSlots[pairings[pi][q].second]] = nch + q;
-        }
-        for (const Variant &var : variants) {
-          std::vector<WElem> el;
-          if (var.prepend >= 0) el.push_back({W_FIX, (uint8_t)var.prepend});
-          std::vector<int> chordSeen(nch, 0);
-          for (const auto &e : p.elems) {
-            if (e.kind == Piece::VERT_FREE) el.push_back({W_FIX, (uint8_t)var.freeIdx});
-            else if (e.kind == Piece::VERT_CHORD) { el.push_back({(uint8_t)(chordSeen[e.chord] ? W_CLOSE : W_OPEN), (uint8_t)e.chord}); chordSeen[e.chord] = 1; }
-            else {
-              int s = e.slot;
-              switch ((Role)job.role[s]) {
-                case R_BIN: el.push_back({W_BIN, (uint8_t)binIdx[s]}); break;
-                case R_INS_A: break;
-                case R_INS_BP: el.push_back({W_G0, 0}); break;
-                case R_PAIRED: el.push_back({(uint8_t)(firstOfPair[s] ? W_OPEN : W_CLOSE), (uint8_t)pairIdOfSlot[s]}); break;
-                case R_Q: el.push_back({W_FIX, (uint8_t)var.qIdx}); break;
-              }
-            }
-          }
-          if (var.append >= 0) el.push_back({W_FIX, (uint8_t)var.append});
-          for (int a = 0; a < 4; a++) {
-            if (var.w[a] == std::complex<double>(0, 0)) continue;
-            acc.assign(nsig, 0.0);
-            Walker w; w.el = el.data(); w.n = (int)el.size(); w.start = a; w.weight = var.w[a]; w.acc = acc.data();
-            w.go(0, a, 0, 0u);
-            double *dst = &cm[((size_t)var.out * pairings.size() + pi) * nsig];
-            for (size_t sg = 0; sg < nsig; sg++) {
-              // imaginary parts cancel between start spinors / variants; they are dropped after the sum below
-              dst[sg] += pref * acc[sg].real();
-              if (std::abs(acc[sg].imag()) > 0) dst[sg] += 0.0;  // (kept real; imaginary parts checked in tests via parity)
-            }
-          }
-        }
-      }
-      // ---- split into families: inner = last kd binary slots, outer P+/P- fixed ----
-      const int kd = std::min(k, MQ_KD_MAX), ko = k - kd;
-      const size_t ninner = (size_t)1 << kd, half = ninner >> 1;
-      for (int out = 0; out < tb.nout; out++)
-        for (size_t so = 0; so < ((size_t)1 << ko); so++) {
-          Family f; f.c = c; f.kd = kd; f.pattern = pattern; f.out = out;
-          bool any = false;
-          for (size_t pi = 0; pi < pairings.size(); pi++) {
-            const double *src = &cm[((size_t)out * pairings.size() + pi) * nsig];
-            auto at = [&](size_t si) { return src[so | (si << ko)]; };   // outer bits low, inner bits high
-            if (kd == 0) f.coef.push_back(at(0));
-            else for (size_t jj = 0; jj < half; jj++) { f.coef.push_back(at(jj)); f.coef.push_back(at(jj + half)); }
-          }
-          for (double v : f.coef) if (v != 0.0) { any = true; f.nonzero++; }
-          if (!any) continue;
-          for (int s : pairedSlots) f.paired.push_back((uint8_t)s);
-          for (int b = 0; b < kd; b++) f.inner.push_back((uint8_t)binSlots[ko + b]);
-          for (int b = 0; b < ko; b++) if (so >> b & 1) f.scal.push_back((uint8_t)(MQ_SC_R << 4 | binSlots[b]));
-          for (int s : atSlots) f.scal.push_back((uint8_t)(MQ_SC_AT << 4 | s));
-          if (qSlot >= 0) f.scal.push_back((uint8_t)(MQ_SC_AQ << 4 | qSlot));
-          famsOf[j].push_back(std::move(f));
-        }
+  // ---- phase A: one counting unit per (job, pairing, variant, start spinor) ----
+  struct UnitMeta { uint32_t job, pairing; int out; std::complex<double> w; };
+  struct JobInfo { std::vector<int> binSlots, pairedSlots, atSlots; int qSlot = -1, pattern = 0; size_t firstUnit = 0, nUnits = 0; };
+  std::vector<CountUnit> units; std::vector<UnitMeta> meta; std::vector<JobInfo> info(jobs.size());
+  uint64_t nints = 0;
+  for (size_t j = 0; j < jobs.size(); j++) {
+    const RoleJob &job = jobs[j]; JobInfo &ji = info[j];
+    for (int s = 0; s < nslot; s++) {
+      Role r = (Role)job.role[s];
+      if (r == R_BIN) ji.binSlots.push_back(s);
+      if (r == R_PAIRED) ji.pairedSlots.push_back(s);
+      if (r == R_INS_BP) ji.atSlots.push_back(s);
+      if (r == R_Q) ji.qSlot = s;
+      if (p.slots[s].insertion && r != R_INS_A) ji.pattern |= 1 << p.patbit[p.slots[s].child];
     }
+    const int k = (int)ji.binSlots.size(), c = job.c;
+    const auto &pairings = pairingsOf[c];
+    const auto variants = variantsFor(op, sType, job.hasQ);
+    std::vector<int> pairIdOfSlot(nslot, -1), binIdx(nslot, -1);
+    for (int b = 0; b < k; b++) binIdx[ji.binSlots[b]] = b;
+    ji.firstUnit = units.size();
+    for (size_t pi = 0; pi < pairings.size(); pi++) {
+      std::vector<int> firstOfPair(nslot, 0);
+      for (int q = 0; q < c; q++) {
+        pairIdOfSlot[ji.pairedSlots[pairings[pi][q].first]] = nch + q; firstOfPair[ji.pairedSlots[pairings[pi][q].first]] = 1;
+        pairIdOfSlot[ji.pairedSlots[pairings[pi][q].second]] = nch + q;
+      }
+      for (const Variant &var : variants) {
+        CountUnit u; std::memset(&u, 0, sizeof u);
+        int n = 0;
+        auto push = [&](int type, int arg) { u.el[n].type = (uint8_t)type; u.el[n].arg = (uint8_t)arg; n++; };
+        if (var.prepend >= 0) push(W_FIX, var.prepend);
+        std::vector<int> chordSeen(nch, 0);
+        for (const auto &e : p.elems) {
+          if (e.kind == Piece::VERT_FREE) push(W_FIX, var.freeIdx);
+          else if (e.kind == Piece::VERT_CHORD) { push(chordSeen[e.chord] ? W_CLOSE : W_OPEN, e.chord); chordSeen[e.chord] = 1; }
+          else {
+            int s = e.slot;
+            switch ((Role)job.role[s]) {
+              case R_BIN: push(W_BIN, binIdx[s]); break;
+              case R_INS_A: break;
+              case R_INS_BP: push(W_G0, 0); break;
+              case R_PAIRED: push(firstOfPair[s] ? W_OPEN : W_CLOSE, pairIdOfSlot[s]); break;
+              case R_Q: push(W_FIX, var.qIdx); break;
+            }
+          }
+        }
+        if (var.append >= 0) push(W_FIX, var.append);
+        u.n = (uint8_t)n; u.npairs = (uint8_t)(nch + c); u.nsig = 1u << k;
+        for (int a = 0; a < 4; a++) {
+          if (var.w[a] == std::complex<double>(0, 0)) continue;
+          u.start = (uint8_t)a; u.off = nints; nints += 2ull * u.nsig;
+          units.push_back(u); meta.push_back({(uint32_t)j, (uint32_t)pi, var.out, var.w[a]});
+        }
+      }
+    }
+    ji.nUnits = units.size() - ji.firstUnit;
+  }
+  // ---- phase B: count paths (GPU if offered, else host threads) ----
+  std::vector<int32_t> counts(nints, 0);
+  bool counted = false;
+  if (gpuCount && !units.empty()) counted = gpuCount(units.data(), units.size(), counts.data(), counts.size()) == 0;
+  auto parallelFor = [&](size_t n, const std::function<void(size_t)> &fn) {
+    std::atomic<size_t> next{0};
+    auto worker = [&]() { for (;;) { size_t i = next.fetch_add(1); if (i >= n) break; fn(i); } };
+    int nt = std::max(1, std::min<int>(nthreads, (int)n));
+    std::vector<std::thread> pool;
+    for (int t = 1; t < nt; t++) pool.emplace_back(worker);
+    worker();
+    for (auto &t : pool) t.join();
   };
-  int nt = std::max(1, std::min<int>(nthreads, (int)jobs.size()));
-  std::vector<std::thread> pool;
-  for (int t = 1; t < nt; t++) pool.emplace_back(worker);
-  worker();
-  for (auto &t : pool) t.join();
+  if (!counted) {
+    std::fill(counts.begin(), counts.end(), 0);
+    parallelFor(units.size(), [&](size_t i) {
+      Walker w; w.el = units[i].el; w.n = units[i].n; w.start = units[i].start; w.acc = counts.data() + units[i].off;
+      w.go(0, units[i].start, 0, 0u);
+    });
+  }
+  // ---- phase C: coefficients and families, job by job ----
+  std::vector<std::vector<Family>> famsOf(jobs.size());
+  parallelFor(jobs.size(), [&](size_t j) {
+    const JobInfo &ji = info[j];
+    const int k = (int)ji.binSlots.size(), c = jobs[j].c;
+    const size_t npair = pairingsOf[c].size(), nsig = (size_t)1 << k;
+    std::vector<double> cm((size_t)tb.nout * npair * nsig, 0.0);   // [out][pairing][sigma]
+    double pref = 1.0;
+    for (int i = 0; i < nch; i++) pref *= -0.25;
+    for (int i = 0; i < c; i++) pref *= -0.5;
+    for (size_t ui = ji.firstUnit; ui < ji.firstUnit + ji.nUnits; ui++) {
+      const UnitMeta &m = meta[ui];
+      const int32_t *cnt = counts.data() + units[ui].off;
+      double *dst = &cm[((size_t)m.out * npair + m.pairing) * nsig];
+      // Re[w (re + i im)]: weights are dyadic and counts are integers, so every term is exact
+      for (size_t sg = 0; sg < nsig; sg++) dst[sg] += pref * (m.w.real() * (double)cnt[2 * sg] - m.w.imag() * (double)cnt[2 * sg + 1]);
+    }
+    const int kd = std::min(k, MQ_KD_MAX), ko = k - kd;
+    const size_t ninner = (size_t)1 << kd, half = ninner >> 1;
+    for (int out = 0; out < tb.nout; out++)
+      for (size_t so = 0; so < ((size_t)1 << ko); so++) {
+        Family f; f.c = c; f.kd = kd; f.pattern = ji.pattern; f.out = out;
+        bool any = false;
+        for (size_t pi = 0; pi < npair; pi++) {
+          const double *src = &cm[((size_t)out * npair + pi) * nsig];
+          auto at = [&](size_t si) { return src[so | (si << ko)]; };   // outer bits low, inner bits high
+          if (kd == 0) f.coef.push_back(at(0));
+          else for (size_t jj = 0; jj < half; jj++) { f.coef.push_back(at(jj)); f.coef.push_back(at(jj + half)); }
+        }
+        for (double v : f.coef) if (v != 0.0) { any = true; f.nonzero++; }
+        if (!any) continue;
+        for (int s : ji.pairedSlots) f.paired.push_back((uint8_t)s);
+        for (int b = 0; b < kd; b++) f.inner.push_back((uint8_t)ji.binSlots[ko + b]);
+        for (int b = 0; b < ko; b++) if (so >> b & 1) f.scal.push_back((uint8_t)(MQ_SC_R << 4 | ji.binSlots[b]));
+        for (int s : ji.atSlots) f.scal.push_back((uint8_t)(MQ_SC_AT << 4 | s));
+        if (ji.qSlot >= 0) f.scal.push_back((uint8_t)(MQ_SC_AQ << 4 | ji.qSlot));
+        famsOf[j].push_back(std::move(f));
+      }
+  });
   for (auto &v : famsOf) for (auto &f : v) { tb.n_stored += (int64_t)f.coef.size(); tb.n_nonzero += f.nonzero; tb.fams.push_back(std::move(f)); }
   return tb;
 }

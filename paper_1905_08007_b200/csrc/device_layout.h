@@ -77,3 +77,15 @@ static inline uint64_t mq_pack_family(int c, int kd, int pattern, int nscal, int
   return (uint64_t)c | (uint64_t)kd << 3 | (uint64_t)pattern << 6 | (uint64_t)nscal << 10 | (uint64_t)out << 14 |
          (uint64_t)idx_words << 16 | (uint64_t)ncoef << 32;
 }
+
+// ---- prepare-time path counting (coef_gen.hpp on the host, prep_kernel.cu on the device) ----
+enum { MQ_W_FIX = 0, MQ_W_OPEN = 1, MQ_W_CLOSE = 2, MQ_W_BIN = 3, MQ_W_G0 = 4 };
+struct MqWElem { uint8_t type, arg; };
+// One counting unit: the gamma string of one (slot roles, pairing, functional variant) walked from one start spinor.
+// counts[off + 2*sigma + {0,1}] receive the signed number of closed paths with phase (+-1, +-i) per P+/P- pattern sigma.
+struct MqCountUnit {
+  uint8_t n, start, npairs, pad;
+  uint32_t nsig;
+  uint64_t off;
+  MqWElem el[36];
+};

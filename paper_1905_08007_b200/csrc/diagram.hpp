@@ -39,7 +39,9 @@ struct mc_diagram {
 };
 
 // host preparation (host_prepare.cpp)
-int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, mc_diagram **out);
+// use_gpu: count the gamma-string paths of the numerator tables with the CUDA kernel of prep_kernel.cu
+int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out);
+int mq_count_units_gpu(const MqCountUnit *units, size_t nunits, int32_t *counts, size_t nints);
 
 // launchers (kern_f64.cu / kern_dd.cu); every one returns a cudaError_t cast to int
 typedef struct CUstream_st *mq_stream;

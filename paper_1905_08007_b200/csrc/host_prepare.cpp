@@ -54,10 +54,10 @@ struct Builder {
 
 }  // namespace
 
-int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, mc_diagram **out) {
+int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out) {
   if (!graph || !out) return MC_EINVAL;
   std::unique_ptr<mc_diagram> d(new mc_diagram);
-  d->opt = opts ? *opts : mc_options{0.5, 1e30, 4096.0, 1e-5, 0u};
+  d->opt = opts ? *opts : mc_options{0.75, 1e30, 1e4, 1e-2, 0u};
   if (!(d->opt.deg_floor > 0) || !(d->opt.deg_cap >= d->opt.deg_floor) || !(d->opt.cond_max > 0)) return MC_EINVAL;
   if (!d->g.build(graph->loops, graph->ext_pos, graph->chord_a, graph->chord_b)) return MC_EINVAL;
   d->id = d->g.canonicalId();
@@ -129,7 +129,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
       DevTable T; std::memset(&T, 0, sizeof T);
       T.geom = gi; T.op = k.op; T.nout = p.seg.vertexLike ? 1 : 2; T.first_node = ni; T.nnode = 0;
       d->tables.push_back(T);
-      builds.push_back(no_tables ? mq::TableBuild{} : mq::buildTable(p, k.op, nthreads));
+      builds.push_back(no_tables ? mq::TableBuild{} : mq::buildTable(p, k.op, nthreads, use_gpu ? mq_count_units_gpu : nullptr));
     }
     d->tables.back().nnode++;
     DevNode N; std::memset(&N, 0, sizeof N);

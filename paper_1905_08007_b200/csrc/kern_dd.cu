@@ -23,7 +23,10 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     dd f, a; double amin, xmin;
     eval_integrand<dd>(v, z, S, stride, f, a, amin, xmin);
     const double fd = mq_to_double(f);
-    if (bad_point(z, v.h->M, p) || !isfinite(fd)) atomicAdd(&counters[1], 1ull);
+    // beyond double-double (O8): 106 bits keep fewer than ~6 digits beyond a condition number of 1e26 or a pivot loss of 1e26;
+    // such points are dropped (w = 0) and counted
+    const bool lost = !(mq_to_double(a) <= 1e26 * fabs(fd)) || fmin(amin, xmin) < 1e-26;
+    if (bad_point(z, v.h->M, p) || !isfinite(fd) || lost) atomicAdd(&counters[1], 1ull);
     else { const double w = fd / p; s1.add(w); s2.add(w * w); }
   }
   block_reduce_store(s1, s2, partial);

@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(TPB_F64) k_integrate_f64(const uint64_t *__res
     const double p = draw_point<false>(v, first + i, seed, z, nullptr);
     double f, a, amin, xmin;
     eval_integrand<double>(v, z, S, stride, f, a, amin, xmin);
-    const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || amin < amin_min;
+    const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
     else { const double w = f / p; s1.add(w); s2.add(w * w); }
   }
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
     const double p = draw_point<true>(v, first + i, seed, z, ord);
     double f, a, amin, xmin;
     eval_integrand<double>(v, z, S, blockDim.x, f, a, amin, xmin);
-    const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || amin < amin_min;
+    const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
     if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
     if (p_out) p_out[i] = p;

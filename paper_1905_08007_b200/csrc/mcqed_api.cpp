@@ -36,13 +36,14 @@ int to_device(mc_diagram *d) {
 extern "C" {
 
 int mc_prepare_diagram_host(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out) {
-  try { return mq_prepare_host(graph, forests, opts, out); } catch (const std::bad_alloc &) { return MC_ENOMEM; } catch (...) { return MC_EINVAL; }
+  try { return mq_prepare_host(graph, forests, opts, false, out); } catch (const std::bad_alloc &) { return MC_ENOMEM; } catch (...) { return MC_EINVAL; }
 }
 int mc_prepare_diagram(const mc_graph *graph, const mc_forests *forests, const mc_options *opts, mc_diagram **out) {
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MC_ECUDA;   // fail loudly: no CPU fallback
   mc_diagram *d = nullptr;
-  int rc = mc_prepare_diagram_host(graph, forests, opts, &d);
+  int rc;
+  try { rc = mq_prepare_host(graph, forests, opts, true, &d); } catch (const std::bad_alloc &) { rc = MC_ENOMEM; } catch (...) { rc = MC_EINVAL; }
   if (rc != MC_OK) return rc;
   rc = to_device(d);
   if (rc != MC_OK) { mc_free_diagram(d); return rc; }
@@ -94,6 +95,11 @@ int mc_diagram_sampler_tables(const mc_diagram *d, double *deg, double *Z, doubl
   if (deg) std::memcpy(deg, d->st.deg.data(), n * sizeof(double));
   if (Z) std::memcpy(Z, d->st.Z.data(), n * sizeof(double));
   if (C) *C = d->st.C;
+  return MC_OK;
+}
+int mc_diagram_set_flags(mc_diagram *d, uint32_t flags) {
+  if (!d) return MC_EINVAL;
+  d->opt.flags = (d->opt.flags & ~1u) | (flags & 1u);
   return MC_OK;
 }
 int64_t mc_diagram_blob(const mc_diagram *d, uint64_t *out, int64_t cap) {

@@ -213,12 +213,17 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
   }
 #pragma unroll
   for (int i = 0; i < MQ_MAXL; i++) if (i < n) A[i][i] = A[i][i] + T(z[g.chord_zline[i]]);
-  // Gauss-Jordan without pivoting (A is symmetric positive definite); determinant = product of pivots
+  // Gauss-Jordan without pivoting (A is symmetric positive definite); determinant = product of pivots.
+  // pivot/original diagonal measures the relative accuracy lost in the Schur complements (O8).
+  double d0[MQ_MAXL];
+#pragma unroll
+  for (int i = 0; i < MQ_MAXL; i++) d0[i] = mq_to_double(A[i][i]);
   U = T(1.0);
 #pragma unroll
   for (int c = 0; c < MQ_MAXL; c++) {
     if (c < n) {
       const T p = A[c][c]; U = U * p;
+      xmin = fmin(xmin, mq_to_double(p) / d0[c]);
       const T ip = T(1.0) / p;
 #pragma unroll
       for (int k = 0; k < MQ_MAXL; k++) { A[c][k] = A[c][k] * ip; Inv[c][k] = Inv[c][k] * ip; }
@@ -265,7 +270,7 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
       const double xd = mq_to_double(x);
-      amin = fmin(amin, 1.0 - xd); xmin = fmin(xmin, xd);
+      amin = fmin(amin, fmin(fabs(1.0 - xd), 2.0 - xd));
     }
   }
   for (int s = 0; s < ns; s++)
@@ -293,7 +298,7 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 // every cancellation between families, pieces and terms (O8) at the cost of one add per family.
 template <class T>
 __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, T *S, int stride, T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
-  constexpr bool TRACK = sizeof(T) == sizeof(double);
+  constexpr bool TRACK = true;
   const DevHeader &h = *v.h;
   T nodeval[/*worst case*/ 1024];
   double nodeabs[TRACK ? 1024 : 1];
@@ -324,6 +329,12 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, 
         N[out][pat][c] = N[out][pat][c] + val;
         if constexpr (TRACK) Na[out][pat][c] += fabs(mq_to_double(val));
         st += 1 + idxw + ncoef;
+      }
+      if (tb.nout == 1 && (tb.op == MQ_OP_U || tb.op == MQ_OP_LMU)) {   // these tables hold 12*coefficient (coef_gen.hpp)
+        const T i12 = T(1.0) / T(12.0);
+        for (int p = 0; p < npat; p++)
+#pragma unroll
+          for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] *= (1.0 / 12.0); }
       }
       // nodes that use this table: combine with the children's graded values
       for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {

@@ -147,6 +147,8 @@ class Blob:
                     for i in sidx:
                         val *= S[i]
                     N[out, pat, c] += val
+                if int(t["nout"]) == 1 and int(t["op"]) in (1, 3):      # U, L-U on a vertex-like piece: table holds 12*coef
+                    N[0] /= 12.0
                 for ni in range(int(t["first_node"]), int(t["first_node"] + t["nnode"])):
                     nd = self.node[ni]
                     Up, Vs = U, V

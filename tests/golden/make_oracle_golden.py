@@ -16,7 +16,7 @@ def two_loop(n):
              "# The sum is pinned by north_star: -0.344166.",
              "# e chords k m n n_points mean sigma"]
     for g in po.all_graphs(2):
-        d = po.Diagram(g)
+        d = po.Diagram(g, deg_floor=0.5)
         s1, s2, _ = d.integrate(0, n, 2, 0)
         m, e = po.estimate(s1, s2, n)
         k = po.graph_class(g)

@@ -56,8 +56,12 @@ def test_points_bit_exact_and_integrand_parity(po, mc, L, idxs, n, seed):
         assert unfl.sum() > 0
         rel = np.abs(r["f"] - fw) / np.abs(fw)
         assert np.all(rel[unfl] <= 1e-10), (L, i, rel[unfl].max())
-        # flagged points: the double-double value against the oracle's wide value
-        assert np.all(rel[~unfl] <= 1e-10), (L, i, rel[~unfl].max() if (~unfl).any() else 0)
+        # flagged points: the double-double value against the oracle's wide value. Both carry ~32 digits, so the
+        # comparison is meaningful where the condition number leaves >= 10 of them (O8)
+        sane = (~unfl) & (r["cond"] <= 1e16)
+        assert np.all(rel[sane] <= 1e-10), (L, i, rel[sane].max() if sane.any() else 0)
+        wild = (~unfl) & ~sane
+        assert np.all(np.isfinite(r["f"][wild]))
         # the proxy has no false negatives against the oracle's truth flag (O8)
         truth = np.abs(ref["f64"] - fw) > 1e-10 * np.abs(fw)
         assert not np.any(truth & unfl), "a point that loses precision in binary64 was not flagged"
@@ -137,9 +141,19 @@ def test_eval_z_double_double_agrees_with_oracle_wide(po, mc):
     z, p, _ = o.sample(0, 400, 5)
     zt = torch.tensor(z, device="cuda")
     f64, fdd, cond = (torch.zeros(len(z), dtype=torch.float64, device="cuda") for _ in range(3))
-    d.eval_z(len(z), zt, torch.cuda.current_stream().cuda_stream, f64, fdd, cond)
+    d.eval_z(len(z), zt, torch.cuda.current_stream().cuda_stream, f64, fdd, cond, None)
     torch.cuda.synchronize()
     ref = o.eval_z(z, wide=True)
     rel = np.abs(fdd.cpu().numpy() - ref["fwide"]) / np.abs(ref["fwide"])
-    assert rel.max() <= 1e-10
+    sane = cond.cpu().numpy() <= 1e16
+    assert sane.sum() > 100 and rel[sane].max() <= 1e-10
     d.close()
+
+
+def test_gpu_prepared_tables_equal_host_prepared(mc):
+    """the path-counting kernel of prepare (prep_kernel.cu) gives bit-identical tables to the host walk"""
+    for (L, e, ch) in [(2, 1, [(0, 4), (2, 3)]), (3, 1, [(0, 6), (2, 4), (3, 5)]), (4, 2, [(0, 5), (1, 7), (3, 4), (6, 8)])]:
+        a = mc.Diagram(L, e, ch)
+        b = mc.Diagram(L, e, ch, host_only=True)
+        assert np.array_equal(a.blob(), b.blob())
+        a.close(); b.close()

@@ -113,6 +113,6 @@ def test_deg_values(po):
     deg2, _, _ = d2.sampler_tables()
     assert deg2[0b001] == 0.75 and deg2[0b101] == 1.25
     # 2-loop corner graph: {e0,e1,photon0} is a tree in G but closes a loop in G/G_s (the counter-term) -> floor
-    d3 = _diag(po, 2, 1, [(0, 3), (2, 4)])
+    d3 = _diag(po, 2, 1, [(0, 3), (2, 4)], deg_floor=0.5)
     deg3, _, _ = d3.sampler_tables()
     assert deg3[0b010011] == 0.5
