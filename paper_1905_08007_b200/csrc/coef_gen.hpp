@@ -17,6 +17,7 @@
 #pragma once
 #include <atomic>
 #include <complex>
+#include <cstdlib>
 #include <cstring>
 #include <functional>
 #include <thread>
@@ -124,13 +125,14 @@ struct RoleJob { std::vector<uint8_t> role; int c; bool hasQ; };
 // optional accelerator: counts all units on the GPU (prep_kernel.cu); returns 0 on success
 using GpuCountFn = int (*)(const detail::CountUnit *units, size_t nunits, int32_t *counts, size_t nints);
 
-inline TableBuild buildTable(const Piece &p, int op, int nthreads, GpuCountFn gpuCount = nullptr) {
+// maxGrade: own grades above it can never reach the integrand (only total grades c < L enter O6)
+inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade, GpuCountFn gpuCount = nullptr) {
   using namespace detail;
   TableBuild tb;
   const bool sType = !p.seg.vertexLike;
   tb.nout = sType ? 2 : 1;
   const int nslot = (int)p.slots.size(), nch = (int)p.ownChord.size();
-  int maxc = nslot / 2;
+  int maxc = std::min(nslot / 2, maxGrade);
   if ((op == MQ_OP_A || op == MQ_OP_LMU) && p.nS == 0) maxc = std::min(maxc, nch - 1);  // top grade ~ gamma^mu: killed (O4)
   // ---- enumerate slot roles ----
   std::vector<RoleJob> jobs;
@@ -243,7 +245,9 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, GpuCountFn gp
       // Re[w (re + i im)]: weights are dyadic and counts are integers, so every term is exact
       for (size_t sg = 0; sg < nsig; sg++) dst[sg] += pref * (m.w.real() * (double)cnt[2 * sg] - m.w.imag() * (double)cnt[2 * sg + 1]);
     }
-    const int kd = std::min(k, MQ_KD_MAX), ko = k - kd;
+    int kdcap = mq_kd_max(c);
+    if (const char *env = std::getenv("MCQED_KD_CAP")) kdcap = std::min(kdcap, std::max(0, atoi(env)));   // experiments only
+    const int kd = std::min(k, kdcap), ko = k - kd;
     const size_t ninner = (size_t)1 << kd, half = ninner >> 1;
     for (int out = 0; out < tb.nout; out++)
       for (size_t so = 0; so < ((size_t)1 << ko); so++) {

@@ -34,9 +34,11 @@ __device__ __forceinline__ dd operator+(dd a, dd b) {   // accurate (IEEE-style)
 __device__ __forceinline__ dd operator-(dd a) { return dd(-a.hi, -a.lo); }
 __device__ __forceinline__ dd operator-(dd a, dd b) { return a + (-b); }
 __device__ __forceinline__ dd operator*(dd a, dd b) {
-  dd p = dd_two_prod(a.hi, b.hi);
-  p.lo = __dadd_rn(p.lo, __fma_rn(a.hi, b.lo, __dmul_rn(a.lo, b.hi)));
-  return dd_quick_two_sum(p.hi, p.lo);
+  const double p = __dmul_rn(a.hi, b.hi);
+  double e = __fma_rn(a.hi, b.hi, -p);
+  e = __fma_rn(a.hi, b.lo, e);
+  e = __fma_rn(a.lo, b.hi, e);
+  return dd_quick_two_sum(p, e);
 }
 __device__ __forceinline__ dd operator*(dd a, double b) {
   dd p = dd_two_prod(a.hi, b);
@@ -58,9 +60,28 @@ __device__ __forceinline__ dd &operator*=(dd &a, dd b) { a = a * b; return a; }
 
 // generic helpers so that one templated evaluator serves binary64 and double-double
 __device__ __forceinline__ double mq_fma(double a, double b, double c) { return fma(a, b, c); }
-__device__ __forceinline__ dd mq_fma(dd a, dd b, dd c) { return a * b + c; }
+// a*b + c in 18 flops: exact product of the high parts, exact sum of the two high parts, low-order terms in binary64;
+// error <= ~2^-103 (|a b| + |c|), the same bound relative to the operands as the renormalising a*b + c
+__device__ __forceinline__ dd mq_fma(dd a, dd b, dd c) {
+  const double p = __dmul_rn(a.hi, b.hi);
+  double e = __fma_rn(a.hi, b.hi, -p);
+  e = __fma_rn(a.hi, b.lo, e);
+  e = __fma_rn(a.lo, b.hi, e);
+  const double s = __dadd_rn(p, c.hi), v = __dadd_rn(s, -p);
+  double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c.hi, -v));
+  t = __dadd_rn(__dadd_rn(t, e), c.lo);
+  return dd_two_sum(s, t);           // not quick: after cancellation of the high parts |t| may exceed |s|
+}
 __device__ __forceinline__ double mq_fma_c(double coef, double x, double c0, double) { return fma(coef, x, c0); }   // coef*x + c0
-__device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) { return x * coef + dd(c0); }
+__device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) {   // coef*x + c0, coef and c0 binary64 (exact table entries)
+  const double p = __dmul_rn(coef, x.hi);
+  double e = __fma_rn(coef, x.hi, -p);
+  e = __fma_rn(coef, x.lo, e);
+  const double s = __dadd_rn(p, c0), v = __dadd_rn(s, -p);
+  double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c0, -v));
+  t = __dadd_rn(t, e);
+  return dd_two_sum(s, t);
+}
 __device__ __forceinline__ double mq_to_double(double a) { return a; }
 __device__ __forceinline__ double mq_to_double(dd a) { return a.hi + a.lo; }
 __device__ __forceinline__ double mq_abs(double a) { return fabs(a); }

@@ -15,8 +15,11 @@
 #define MQ_MAXGEOM 96
 #define MQ_MAXNODE 256
 #define MQ_MAXPAT 16      // 2^(max #S-children of a piece)
-#define MQ_KD_MAX 4       // inner dense binary dimensions of a family
+// inner dense binary dimensions of a family, by number of Wick pairs c (bounds the static code and the family size)
+static inline int mq_kd_max(int c) { return c <= 3 ? 4 : 3; }   // larger inner blocks (5, 6) were measured slower (register spills)
 #define MQ_MAXSCAL 12
+#define MQ_CHUNK_WORDS 2048   // staging granule of the family stream (16 KiB)
+#define MQ_PAD_MARK 7        // header field c of a PAD entry
 
 enum { MQ_OP_A = 0, MQ_OP_U = 1, MQ_OP_L = 2, MQ_OP_LMU = 3 };
 enum { MQ_SLOT_LINE = 0, MQ_SLOT_INS = 1 };
@@ -62,10 +65,11 @@ struct DevHeader {
   int32_t max_scal_len, pad0;
   double C, cond_max;
   int64_t off_Z, off_invdeg, off_geom, off_table, off_node, off_term, total_words;
+  int64_t off_stream, stream_chunks;      // the family streams: stream_chunks chunks of MQ_CHUNK_WORDS words
 };
 
 // Family header word (uint64), then index bytes, padded to 8 bytes, then the dense coefficients:
-//   bits  0..2  c   (#Wick pairs)              bits  3..5  kd (#inner binary slots)
+//   bits  0..2  c   (#Wick pairs; 7 = PAD entry: skip 1+idx_words words, no coefficients)              bits  3..5  kd (#inner binary slots)
 //   bits  6..9  pattern (compressed)           bits 10..13 nscal (#extra scalar factors)
 //   bits 14     out (0/1: which output of an S-type piece)
 //   bits 16..31 number of 8-byte words of index bytes that follow

@@ -129,7 +129,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
       DevTable T; std::memset(&T, 0, sizeof T);
       T.geom = gi; T.op = k.op; T.nout = p.seg.vertexLike ? 1 : 2; T.first_node = ni; T.nnode = 0;
       d->tables.push_back(T);
-      builds.push_back(no_tables ? mq::TableBuild{} : mq::buildTable(p, k.op, nthreads, use_gpu ? mq_count_units_gpu : nullptr));
+      builds.push_back(no_tables ? mq::TableBuild{} : mq::buildTable(p, k.op, nthreads, d->g.L - 1, use_gpu ? mq_count_units_gpu : nullptr));
     }
     d->tables.back().nnode++;
     DevNode N; std::memset(&N, 0, sizeof N);
@@ -161,8 +161,12 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   H.off_table = off; off += words(sizeof(DevTable) * d->tables.size());
   H.off_node = off; off += words(sizeof(DevNode) * d->nodes.size());
   H.off_term = off; off += words(sizeof(DevTerm) * d->terms.size());
-  // streams: every family = header word | index bytes (padded) | coefficients; the coefficients start on a
-  // 16-byte boundary (the kernel reads them as double2), so the index words are padded to make pos+1+idxw even
+  // streams: every family = header word | index bytes (padded) | coefficients. The kernels stage the stream through
+  // shared memory in chunks of MQ_CHUNK_WORDS (bulk async copies), so (i) the stream starts on a 16-byte boundary,
+  // (ii) no family straddles a chunk boundary (a PAD header, c = 7, fills the rest of a chunk), (iii) coefficients
+  // start on a 16-byte boundary (read as double2), (iv) the stream is consumed strictly in order: tables are laid
+  // out in the order the evaluator visits them, families of a table sorted by (output, pattern, grade).
+  if (off & 1) off++;
   std::vector<uint64_t> streams;
   const int64_t stream_base = off;
   for (size_t ti = 0; ti < d->tables.size(); ti++) {
@@ -170,7 +174,15 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     T.stream_off = stream_base + (int64_t)streams.size(); T.nfam = (int)tb.fams.size(); T.n_monomials = tb.n_stored;
     const int ns = d->geoms[T.geom].nslot;
     auto tri = [&](int a, int b) { if (a > b) std::swap(a, b); return 3 * ns + a * ns - a * (a + 1) / 2 + (b - a - 1); };
-    for (auto &f : tb.fams) {
+    std::vector<const mq::Family *> order;
+    for (auto &f : tb.fams) order.push_back(&f);
+    std::stable_sort(order.begin(), order.end(), [](const mq::Family *a, const mq::Family *b) {
+      if (a->out != b->out) return a->out < b->out;
+      if (a->pattern != b->pattern) return a->pattern < b->pattern;
+      return a->c < b->c;
+    });
+    for (const mq::Family *fp : order) {
+      const mq::Family &f = *fp;
       std::vector<uint8_t> idx;
       const int n2 = 2 * f.c;
       for (int i = 0; i < n2; i++) for (int j = i + 1; j < n2; j++) idx.push_back((uint8_t)tri(f.paired[i], f.paired[j]));
@@ -180,8 +192,19 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
         idx.push_back((uint8_t)(kind == MQ_SC_R ? slot : kind == MQ_SC_AT ? ns + slot : 2 * ns + slot));
       }
       int idxw = (int)words(idx.size());
-      const int64_t pos = stream_base + (int64_t)streams.size();
-      if ((pos + 1 + idxw) & 1) idxw++;
+      if (idxw == 0) idxw = 1;                                                 // the kernel always reads one index word
+      int64_t in_chunk = (int64_t)streams.size() % MQ_CHUNK_WORDS;
+      if ((in_chunk + 1 + idxw) & 1) idxw++;
+      const int64_t need = 1 + idxw + (int64_t)f.coef.size();
+      if (need > MQ_CHUNK_WORDS) return MC_ELIMIT;
+      if (in_chunk + need > MQ_CHUNK_WORDS) {                                  // PAD to the chunk boundary
+        const int64_t rest = MQ_CHUNK_WORDS - in_chunk;
+        streams.push_back(mq_pack_family(7, 0, 0, 0, 0, (int)(rest - 1), 0u));
+        streams.resize(streams.size() + (size_t)(rest - 1), 0ull);
+        in_chunk = 0;
+        idxw = std::max<int>(1, (int)words(idx.size()));
+        if ((1 + idxw) & 1) idxw++;
+      }
       streams.push_back(mq_pack_family(f.c, f.kd, f.pattern, (int)f.scal.size(), f.out, idxw, (uint32_t)f.coef.size()));
       const size_t at = streams.size();
       streams.resize(at + idxw + f.coef.size(), 0ull);
@@ -191,6 +214,15 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     T.stream_words = stream_base + (int64_t)streams.size() - T.stream_off;
     d->n_stored += tb.n_stored; d->n_nonzero += tb.n_nonzero;
   }
+  {                                                                            // close the last chunk
+    const int64_t in_chunk = (int64_t)streams.size() % MQ_CHUNK_WORDS;
+    if (in_chunk || streams.empty()) {
+      const int64_t rest = MQ_CHUNK_WORDS - in_chunk;
+      streams.push_back(mq_pack_family(7, 0, 0, 0, 0, (int)(rest - 1), 0u));
+      streams.resize(streams.size() + (size_t)(rest - 1), 0ull);
+    }
+  }
+  H.off_stream = stream_base; H.stream_chunks = (int64_t)streams.size() / MQ_CHUNK_WORDS;
   off += (int64_t)streams.size();
   H.total_words = off;
   d->blob.assign((size_t)off, 0ull);

@@ -38,4 +38,16 @@ __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   
   return bad;
 }
 
+// dynamic shared memory layout of every evaluating kernel: [ S: scal_len x blockDim x sizeof(T) | 2 stream chunks | 2 mbarriers ]
+__host__ __device__ inline size_t smem_bytes(int scal_len, int threads, size_t elem) {
+  size_t s = (size_t)scal_len * threads * elem;
+  s = (s + 127) & ~(size_t)127;
+  return s + 2 * MQ_CHUNK_WORDS * 8 + 16 + 32;   // + slack: the header prefetch may read up to 24 bytes past a chunk
+}
+__device__ __forceinline__ void setup_reader(StreamReader &rd, unsigned char *smem, int scal_len, size_t elem) {
+  size_t s = (size_t)scal_len * blockDim.x * elem;
+  s = (s + 127) & ~(size_t)127;
+  rd.init(reinterpret_cast<uint64_t *>(smem + s), reinterpret_cast<uint64_t *>(smem + s + 2 * MQ_CHUNK_WORDS * 8));
+}
+
 }  // namespace mqk

@@ -11,17 +11,20 @@ namespace mqk {
 // a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
 __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
                                                          const unsigned long long *flag_list, unsigned long long *counters) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  dd *S = reinterpret_cast<dd *>(smem) + threadIdx.x;
+  dd *S = reinterpret_cast<dd *>(smem_raw) + threadIdx.x;
   const int stride = blockDim.x;
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (unsigned long long)gridDim.x * blockDim.x) {
+  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < cnt; base += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned long long i = base + threadIdx.x; const bool live = i < cnt;
     double z[MQ_MAXM];
-    const double p = draw_point<false>(v, flag_list[i], seed, z, nullptr);
+    const double p = draw_point<false>(v, flag_list[live ? i : cnt - 1], seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, z, S, stride, f, a, amin, xmin);
+    eval_integrand<dd>(v, rd, z, S, stride, f, a, amin, xmin);
+    if (!live) continue;
     const double fd = mq_to_double(f);
     // beyond double-double (O8): 106 bits keep fewer than ~6 digits beyond a condition number of 1e26 or a pivot loss of 1e26;
     // such points are dropped (w = 0) and counted
@@ -34,30 +37,35 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
 
 __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
                                                            const unsigned long long *flag_list, const unsigned long long *counters) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  dd *S = reinterpret_cast<dd *>(smem) + threadIdx.x;
+  dd *S = reinterpret_cast<dd *>(smem_raw) + threadIdx.x;
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (unsigned long long)gridDim.x * blockDim.x) {
+  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < cnt; base += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned long long i = base + threadIdx.x; const bool live = i < cnt;
     double z[MQ_MAXM];
-    const unsigned long long rel = flag_list[i];
+    const unsigned long long rel = flag_list[live ? i : cnt - 1];
     draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, z, S, blockDim.x, f, a, amin, xmin);
-    f_out[rel] = mq_to_double(f);
+    eval_integrand<dd>(v, rd, z, S, blockDim.x, f, a, amin, xmin);
+    if (live) f_out[rel] = mq_to_double(f);
   }
 }
 
 __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in, double *fdd_out) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+    const bool live = base + threadIdx.x < n;
+    const uint64_t i = live ? base + threadIdx.x : n - 1;
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, z, reinterpret_cast<dd *>(smem) + threadIdx.x, blockDim.x, f, a, amin, xmin);
-    fdd_out[i] = mq_to_double(f);
+    eval_integrand<dd>(v, rd, z, reinterpret_cast<dd *>(smem_raw) + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    if (live) fdd_out[i] = mq_to_double(f);
   }
 }
 
@@ -66,7 +74,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
 using namespace mqk;
 
 int mq_config_dd(mc_diagram *d) {
-  d->smem_dd = (size_t)d->max_scal_len * 2 * sizeof(double) * TPB_DD;
+  d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd));
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_integrate_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
   if ((e = cudaFuncSetAttribute(k_eval_points_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;

@@ -12,16 +12,21 @@ namespace mqk {
 __global__ void __launch_bounds__(TPB_F64) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
                                                            double cond_max, double amin_min, double *partial,
                                                            unsigned long long *flag_list, unsigned long long *counters) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  double *S = smem + threadIdx.x;
+  double *S = reinterpret_cast<double *>(smem_raw) + threadIdx.x;
   const int stride = blockDim.x;
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+  // the evaluator is CTA-collective (it stages the table stream through shared memory): every thread of the CTA
+  // runs the same number of iterations; threads past the end re-evaluate the last point and discard it
+  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t i = base + threadIdx.x; const bool live = i < n;
     double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + i, seed, z, nullptr);
+    const double p = draw_point<false>(v, first + (live ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
-    eval_integrand<double>(v, z, S, stride, f, a, amin, xmin);
+    eval_integrand<double>(v, rd, z, S, stride, f, a, amin, xmin);
+    if (!live) continue;
     const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
     else { const double w = f / p; s1.add(w); s2.add(w * w); }
@@ -50,15 +55,18 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
                                                           double cond_max, double amin_min,
                                                           double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out,
                                                           double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  double *S = smem + threadIdx.x;
+  double *S = reinterpret_cast<double *>(smem_raw) + threadIdx.x;
   const int M = v.h->M;
-  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t i = base + threadIdx.x; const bool live = i < n;
     double z[MQ_MAXM]; int32_t ord[MQ_MAXM];
-    const double p = draw_point<true>(v, first + i, seed, z, ord);
+    const double p = draw_point<true>(v, first + (live ? i : n - 1), seed, z, ord);
     double f, a, amin, xmin;
-    eval_integrand<double>(v, z, S, blockDim.x, f, a, amin, xmin);
+    eval_integrand<double>(v, rd, z, S, blockDim.x, f, a, amin, xmin);
+    if (!live) continue;
     const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
     if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
@@ -73,14 +81,16 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
 
 __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in,
                                                          double *f64_out, double *cond_out, double *aux_out) {
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t i = base + threadIdx.x < n ? base + threadIdx.x : n - 1;   // surplus threads redo the last point
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     double f, a, amin, xmin;
-    eval_integrand<double>(v, z, smem + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    eval_integrand<double>(v, rd, z, reinterpret_cast<double *>(smem_raw) + threadIdx.x, blockDim.x, f, a, amin, xmin);
     if (f64_out) f64_out[i] = f;
     if (cond_out) cond_out[i] = a / fabs(f);
     if (aux_out) { aux_out[2 * i] = amin; aux_out[2 * i + 1] = xmin; }
@@ -106,8 +116,8 @@ __global__ void k_fp64_peak(int iters, double *sink) {
 using namespace mqk;
 
 int mq_config_f64(mc_diagram *d) {
-  d->smem_f64 = (size_t)d->max_scal_len * sizeof(double) * TPB_F64;
-  d->smem_eval = (size_t)d->max_scal_len * sizeof(double) * TPB_EVAL;
+  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double));
+  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double));
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_integrate_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_f64)) != cudaSuccess) return (int)e;
   if ((e = cudaFuncSetAttribute(k_eval_points, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;

@@ -118,18 +118,81 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
   return __ddiv_rn(__dmul_rn(v.h->C, pu), pz);
 }
 
+// ------------------------------------------------------------------ shared-memory helpers (explicit LDS) and the stream reader
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint64_t lds_u64(uint32_t a) { uint64_t v; asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds_u8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ double2 lds_f64x2(uint32_t a) { double2 v; asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ double lds_f64(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+template <class T> __device__ __forceinline__ T lds_T(uint32_t a);
+template <> __device__ __forceinline__ double lds_T<double>(uint32_t a) { return lds_f64(a); }
+template <> __device__ __forceinline__ dd lds_T<dd>(uint32_t a) { double2 v = lds_f64x2(a); return dd(v.x, v.y); }
+
+// The family stream of a diagram is staged through shared memory in chunks of MQ_CHUNK_WORDS words by bulk
+// asynchronous copies (cp.async.bulk + mbarrier, the TMA engine; SASS UBLKCP), two chunks in flight, so that
+// headers, index bytes and coefficients are read at shared-memory latency by every warp of the CTA.
+// All methods are CTA-collective: every thread of the CTA calls them in the same order.
+struct StreamReader {
+  const uint64_t *gsrc;   // first chunk in global memory
+  uint32_t s_buf;         // shared address of the two chunk buffers
+  uint32_t s_bar;         // shared address of the two mbarriers
+  int nchunks, chunk, pos;
+  uint32_t phase;         // bit b: parity the next wait on buffer b expects
+
+  __device__ __forceinline__ void init(uint64_t *buf, uint64_t *bar) {
+    s_buf = smem_u32(buf); s_bar = smem_u32(bar); phase = 0;
+    if (threadIdx.x == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s_bar));
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s_bar + 8));
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+  }
+  __device__ __forceinline__ void issue(int k) {   // thread 0 only
+    const uint32_t bar = s_bar + 8 * (k & 1), dst = s_buf + (k & 1) * (MQ_CHUNK_WORDS * 8);
+    const uint32_t bytes = MQ_CHUNK_WORDS * 8;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(gsrc + (size_t)k * MQ_CHUNK_WORDS), "r"(bytes), "r"(bar) : "memory");
+  }
+  __device__ __forceinline__ void wait(int k) {
+    const uint32_t bar = s_bar + 8 * (k & 1), par = (phase >> (k & 1)) & 1u;
+    uint32_t ok;
+    do {
+      asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(bar), "r"(par) : "memory");
+    } while (!ok);
+    phase ^= 1u << (k & 1);
+  }
+  __device__ __forceinline__ void begin(const uint64_t *src, int n) {
+    gsrc = src; nchunks = n; chunk = 0; pos = 0;
+    __syncthreads();                                   // nobody still reads the buffers of the previous point
+    if (threadIdx.x == 0) { issue(0); if (n > 1) issue(1); }
+    wait(0);
+  }
+  __device__ __forceinline__ void advance() {          // the current chunk is used up
+    __syncthreads();
+    if (threadIdx.x == 0 && chunk + 2 < nchunks) issue(chunk + 2);
+    chunk++; pos = 0;
+    wait(chunk);
+  }
+  __device__ __forceinline__ uint32_t addr() const { return s_buf + (chunk & 1) * (MQ_CHUNK_WORDS * 8) + pos * 8; }
+};
+
 // ------------------------------------------------------------------ a5: one family, static code per (c, kd)
+// coefficients and index bytes come from the staged stream (shared memory, broadcast reads); the per-point
+// operands r_t and beta~_tu are gathered once per family from S[index][thread] into registers
 template <class T, int KD>
-__device__ __forceinline__ T horner(const double *__restrict__ c, const T *r) {
-  if constexpr (KD == 0) { return T(__ldg(c)); }
+__device__ __forceinline__ T horner(uint32_t &s_coef, const T *r) {
+  if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8; return v; }
   else {
     constexpr int H = 1 << (KD - 1);
     T v[H];
 #pragma unroll
     for (int j = 0; j < H; j++) {
-      double2 cc = __ldg(reinterpret_cast<const double2 *>(c) + j);      // (c[j], c[j+H])
+      const double2 cc = lds_f64x2(s_coef + 16 * j);                       // (c[j], c[j+H])
       v[j] = mq_fma_c(cc.y, r[KD - 1], cc.x, T());
     }
+    s_coef += 16 * H;
 #pragma unroll
     for (int i = KD - 2; i >= 0; i--) {
 #pragma unroll
@@ -144,52 +207,57 @@ constexpr int ctz_c(unsigned x) { int n = 0; while (!(x & 1u)) { x >>= 1; n++; }
 
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec;
 template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> struct PairStep {
-  static __device__ __forceinline__ void run(const T *b, T w, const double *__restrict__ &coef, const T *r, T &sum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum) {
     if constexpr (S < N2) {
       if constexpr (!((USED >> S) & 1u)) {
-        if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], coef, r, sum);
-        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, w * b[pair_index<N2>(F, S)], coef, r, sum);
+        if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], s_coef, r, sum);
+        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, w * b[pair_index<N2>(F, S)], s_coef, r, sum);
       }
-      PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, coef, r, sum);
+      PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, s_coef, r, sum);
     }
   }
 };
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
-  static __device__ __forceinline__ void run(const T *b, T w, const double *__restrict__ &coef, const T *r, T &sum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum) {
     if constexpr (USED == ((1u << N2) - 1u)) {
-      T h = horner<T, KD>(coef, r);
-      coef += (1 << KD);
+      T h = horner<T, KD>(s_coef, r);
       if constexpr (FIRST) sum = sum + h; else sum = mq_fma(w, h, sum);
     } else {
       constexpr int F = ctz_c(~USED);
-      PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, coef, r, sum);
+      PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, s_coef, r, sum);
     }
   }
 };
 
-// S: per-point scalar array of the piece in shared memory, S[index * stride]
+// s_idx: shared address of the index bytes; s_coef: of the coefficients; s_S: of this thread's S[0]; sstride: bytes per S index
 template <class T, int C, int KD>
-__device__ __forceinline__ T family_eval(const uint8_t *__restrict__ idx, const double *__restrict__ coef, const T *S, int stride) {
-  constexpr int N2 = 2 * C, NB = C * (2 * C - 1);
+__device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+  constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
+  uint64_t iw[NW > 2 ? NW : 2];
+  iw[0] = w0; iw[1] = w1;                          // the first 16 index bytes were prefetched with the header
+#pragma unroll
+  for (int k = 2; k < NW; k++) iw[k] = lds_u64(s_idx + 8 * k);
   T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
 #pragma unroll
-  for (int i = 0; i < NB; i++) b[i] = S[(int)idx[i] * stride];
+  for (int i = 0; i < NB; i++) b[i] = lds_T<T>(s_S + (uint32_t)((iw[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
 #pragma unroll
-  for (int i = 0; i < KD; i++) r[i] = S[(int)idx[NB + i] * stride];
+  for (int i = 0; i < KD; i++) r[i] = lds_T<T>(s_S + (uint32_t)((iw[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
   T sum = T(0.0);
-  PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), coef, r, sum);
+  PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum);
   return sum;
 }
 
 template <class T>
-__device__ __noinline__ T family_dispatch(int c, int kd, const uint8_t *__restrict__ idx, const double *__restrict__ coef, const T *S, int stride) {
-  switch (c * 8 + kd) {
-#define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(idx, coef, S, stride);
-#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
+__device__ __noinline__ T family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+  switch (ckd) {     // key = c*8 + kd; the inner dimension kd is capped per c by mq_kd_max (device_layout.h)
+#define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(w0, w1, s_idx, s_coef, s_S, sstride);
+#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3)
     MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_ROW(4)
+    MQ_CASE(0, 4) MQ_CASE(0, 5) MQ_CASE(0, 6) MQ_CASE(1, 4) MQ_CASE(1, 5) MQ_CASE(1, 6) MQ_CASE(2, 4) MQ_CASE(2, 5) MQ_CASE(3, 4)
 #undef MQ_ROW
 #undef MQ_CASE
   }
+  __trap();          // a family shape the tables must never contain
   return T(0.0);
 }
 
@@ -297,13 +365,15 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 // (|family value| summed, |child value| multiplied): abs_out = sum over terms and grades of that bound. It measures
 // every cancellation between families, pieces and terms (O8) at the cost of one add per family.
 template <class T>
-__device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, T *S, int stride, T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
   constexpr bool TRACK = true;
   const DevHeader &h = *v.h;
   T nodeval[/*worst case*/ 1024];
   double nodeabs[TRACK ? 1024 : 1];
   T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
   double amin = 1.0, xmin = 1.0;
+  const uint32_t s_S = smem_u32(S), sstride = (uint32_t)(stride * sizeof(T));
+  rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
     T U, V, G;
@@ -316,20 +386,37 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, const double *z, 
       for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = 0.0; }
-      const uint64_t *st = v.blob + tb.stream_off;
-      for (int fi = 0; fi < tb.nfam; fi++) {
-        const uint64_t hd = __ldg(st);
-        const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7), pat = (int)(hd >> 6 & 15), nscal = (int)(hd >> 10 & 15), out = (int)(hd >> 14 & 1);
-        const int idxw = (int)(hd >> 16 & 0xFFFF); const uint32_t ncoef = (uint32_t)(hd >> 32);
-        const uint8_t *idx = reinterpret_cast<const uint8_t *>(st + 1);
-        const double *coef = reinterpret_cast<const double *>(st + 1 + idxw);
-        T val = family_dispatch<T>(c, kd, idx, coef, S, stride);
+      // families of this table from the staged stream; a run of families with the same (output, pattern, grade)
+      // accumulates in registers and is flushed when the key changes (families are sorted by that key)
+      int key = -1; T racc = T(0.0); double racca = 0.0;
+      bool have = false; uint32_t a0 = 0; uint64_t hd = 0, w0 = 0, w1 = 0;   // header + first index words of the current entry
+      for (int left = tb.nfam; left > 0;) {
+        if (!have) {
+          if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
+          a0 = rd.addr(); hd = lds_u64(a0); w0 = lds_u64(a0 + 8); w1 = lds_u64(a0 + 16);
+        }
+        const int idxw = (int)(hd >> 16 & 0xFFFF);
+        const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7);
+        if (c == MQ_PAD_MARK) { rd.pos += 1 + idxw; have = false; continue; }
+        const int nscal = (int)(hd >> 10 & 15), kk = (int)((hd & 7) | ((hd >> 6 & 15) << 3) | ((hd >> 14 & 1) << 7));
+        const int size = 1 + idxw + (int)(uint32_t)(hd >> 32), npos = rd.pos + size;
+        // software pipeline: fetch the next entry's header and index words before this family's arithmetic
+        uint32_t an = a0 + 8 * size; uint64_t hdn = 0, n0 = 0, n1 = 0;
+        const bool havenext = npos < MQ_CHUNK_WORDS;
+        if (havenext) { hdn = lds_u64(an); n0 = lds_u64(an + 8); n1 = lds_u64(an + 16); }
+        T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
         const int nb = c * (2 * c - 1) + kd;
-        for (int i = 0; i < nscal; i++) val = val * S[(int)idx[nb + i] * stride];
-        N[out][pat][c] = N[out][pat][c] + val;
-        if constexpr (TRACK) Na[out][pat][c] += fabs(mq_to_double(val));
-        st += 1 + idxw + ncoef;
+        for (int i = 0; i < nscal; i++) val = val * lds_T<T>(s_S + lds_u8(a0 + 8 + nb + i) * sstride);
+        if (kk != key) {
+          if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
+          key = kk; racc = T(0.0); racca = 0.0;
+        }
+        racc = racc + val;
+        if constexpr (TRACK) racca += fabs(mq_to_double(val));
+        rd.pos = npos; left--;
+        have = havenext; a0 = an; hd = hdn; w0 = n0; w1 = n1;
       }
+      if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
       if (tb.nout == 1 && (tb.op == MQ_OP_U || tb.op == MQ_OP_LMU)) {   // these tables hold 12*coefficient (coef_gen.hpp)
         const T i12 = T(1.0) / T(12.0);
         for (int p = 0; p < npat; p++)

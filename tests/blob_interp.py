@@ -10,7 +10,8 @@ import numpy as np
 MAXL, MAXSLOT, MAXCHILD, NGRADE = 5, 14, 5, 6
 HDR = np.dtype([("L", "<i4"), ("M", "<i4"), ("diag_id", "<i4"), ("ngeom", "<i4"), ("ntable", "<i4"), ("nnode", "<i4"), ("nterm", "<i4"),
                 ("nodeval_len", "<i4"), ("max_scal_len", "<i4"), ("pad0", "<i4"), ("C", "<f8"), ("cond_max", "<f8"),
-                ("off_Z", "<i8"), ("off_invdeg", "<i8"), ("off_geom", "<i8"), ("off_table", "<i8"), ("off_node", "<i8"), ("off_term", "<i8"), ("total_words", "<i8")])
+                ("off_Z", "<i8"), ("off_invdeg", "<i8"), ("off_geom", "<i8"), ("off_table", "<i8"), ("off_node", "<i8"), ("off_term", "<i8"), ("total_words", "<i8"),
+                ("off_stream", "<i8"), ("stream_chunks", "<i8")])
 SLOT = np.dtype([("kind", "i1"), ("zline", "i1"), ("sgn", "i1"), ("child", "i1"), ("eps", "<u4")])
 GEOM = np.dtype([("nch", "<i4"), ("nslot", "<i4"), ("nchild", "<i4"), ("nS", "<i4"), ("chord_zline", "<i4", (MAXL,)), ("slot", SLOT, (MAXSLOT,)),
                  ("child_type", "i1", (MAXCHILD,)), ("child_patbit", "i1", (MAXCHILD,)), ("pad", "<i2"), ("first_table", "<i4"), ("ntable", "<i4")])
@@ -18,7 +19,7 @@ TABLE = np.dtype([("geom", "<i4"), ("op", "<i4"), ("nout", "<i4"), ("nfam", "<i4
                   ("stream_off", "<i8"), ("stream_words", "<i8"), ("n_monomials", "<i8")])
 NODE = np.dtype([("table", "<i4"), ("geom", "<i4"), ("nchild", "<i4"), ("nout", "<i4"), ("child", "<i4", (MAXCHILD,)), ("val_off", "<i4"), ("ngr", "<i4")])
 TERM = np.dtype([("root", "<i4"), ("sign", "<i4")])
-assert GEOM.itemsize == 168 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 112
+assert GEOM.itemsize == 168 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 128
 
 
 def pairings(n2):
@@ -53,10 +54,15 @@ class Blob:
         t = self.table[ti]
         pos = int(t["stream_off"])
         raw = self.w.view(np.uint8)
-        for _ in range(int(t["nfam"])):
+        nleft = int(t["nfam"])
+        while nleft:
             hd = int(self.w[pos])
             c, kd, pat, nscal, out = hd & 7, hd >> 3 & 7, hd >> 6 & 15, hd >> 10 & 15, hd >> 14 & 1
             idxw, ncoef = hd >> 16 & 0xFFFF, hd >> 32
+            if c == 7:                      # PAD entry up to the chunk boundary
+                pos += 1 + idxw
+                continue
+            nleft -= 1
             nb = c * (2 * c - 1)
             idx = raw[(pos + 1) * 8:(pos + 1) * 8 + nb + kd + nscal].astype(int)
             coef = self.w[pos + 1 + idxw:pos + 1 + idxw + ncoef].view(np.float64)

@@ -123,3 +123,20 @@ def test_info_counts(po, mc):
     info = d.info()
     assert info["n_terms"] == po.Diagram(g, level=0).nterm == 8
     assert info["flop_per_sample"] > 0 and info["table_bytes"] == 8 * len(d.blob())
+
+
+@pytest.mark.parametrize("L,idx,npts", [(2, 1, 6), (2, 3, 6), (3, 7, 3), (3, 18, 2)])
+def test_oracle_wide_value_equals_exact_rational_value(po, mc, L, idx, npts):
+    """exact pin: Fraction arithmetic on the product's tables at points drawn from Eq.(1) (deep corners,
+    condition numbers up to 1e9) reproduces the oracle's binary128 value to the last binary64 digit"""
+    from fractions import Fraction as Fr
+    from exact_interp import ExactBlob
+    g = po.graph_get(L, idx)
+    o = po.Diagram(g)
+    d = mc.Diagram(L, g.ext_pos, g.chords(), host_only=True)
+    b = ExactBlob(d.blob())
+    z, _, _ = o.sample(0, npts, 5)
+    ref = o.eval_z(z, wide=True)
+    for k in range(npts):
+        fe = float(b.integrand([Fr(float(v)) for v in z[k]]))
+        assert abs(ref["fwide"][k] - fe) <= 2e-16 * abs(fe), (k, fe, ref["fwide"][k])
