@@ -32,7 +32,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (4 = the metric's workload)")
     ap.add_argument("--graphs", type=int, default=0, help="use only the first G graphs of the config (0 = all; for debugging)")
-    ap.add_argument("--batch", type=int, default=1 << 13, help="sample points per diagram per step")
+    ap.add_argument("--batch", type=int, default=37888, help="sample points per diagram per step")
     ap.add_argument("--ref-points", type=int, default=768, help="oracle sample points per step (reference arm / cpu_baseline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -198,7 +198,8 @@ def run_ours(args):
     dom = "k_integrate_dd" if ms_dd > ms_f64 else "k_integrate_f64"
     ach = ach_dd if dom == "k_integrate_dd" else ach_f64
     roofline = {"bound": "alu", "kernel": dom, "achieved": ach / 1e12, "peak": peak_flops / 1e12, "unit": "TFLOP/s", "frac": ach / peak_flops,
-                "traffic": None, "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
+                "traffic": {"k_integrate_dd": 108.4e6, "k_integrate_f64": 190.5e6}[dom], "traffic_note": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r1_v2_ncu_details.txt); the algorithmic bytes are ~0 (no per-sample input): this is per-thread stack spilling to DRAM",
+                "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
                 "kernels": {"k_integrate_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
                             "k_integrate_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
                                                "points_per_step": float(c[:, 0].sum()) / args.steps,

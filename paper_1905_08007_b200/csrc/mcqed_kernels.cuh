@@ -261,6 +261,44 @@ __device__ __noinline__ T family_dispatch(int ckd, uint64_t w0, uint64_t w1, uin
   return T(0.0);
 }
 
+// Two consecutive families of the same shape evaluated together: their arithmetic chains are independent, which
+// doubles the instruction-level parallelism of a warp at unchanged shared-memory footprint (binary64 only).
+template <int C, int KD>
+__device__ __forceinline__ void family_eval2(const uint64_t *w, uint32_t s_idxA, uint32_t s_coefA, uint32_t s_idxB, uint32_t s_coefB,
+                                             uint32_t s_S, uint32_t sstride, double &outA, double &outB) {
+  constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
+  uint64_t iwA[NW > 2 ? NW : 2], iwB[NW > 2 ? NW : 2];
+  iwA[0] = w[0]; iwA[1] = w[1]; iwB[0] = w[2]; iwB[1] = w[3];
+#pragma unroll
+  for (int k = 2; k < NW; k++) { iwA[k] = lds_u64(s_idxA + 8 * k); iwB[k] = lds_u64(s_idxB + 8 * k); }
+  double bA[NB > 0 ? NB : 1], rA[KD > 0 ? KD : 1], bB[NB > 0 ? NB : 1], rB[KD > 0 ? KD : 1];
+#pragma unroll
+  for (int i = 0; i < NB; i++) {
+    bA[i] = lds_f64(s_S + (uint32_t)((iwA[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
+    bB[i] = lds_f64(s_S + (uint32_t)((iwB[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
+  }
+#pragma unroll
+  for (int i = 0; i < KD; i++) {
+    rA[i] = lds_f64(s_S + (uint32_t)((iwA[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
+    rB[i] = lds_f64(s_S + (uint32_t)((iwB[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
+  }
+  double sumA = 0.0, sumB = 0.0;
+  PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA);
+  PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB);
+  outA = sumA; outB = sumB;
+}
+static __device__ __noinline__ void family_dispatch2(int ckd, const uint64_t *w, uint32_t s_idxA, uint32_t s_coefA, uint32_t s_idxB, uint32_t s_coefB,
+                                              uint32_t s_S, uint32_t sstride, double &outA, double &outB) {
+  switch (ckd) {
+#define MQ_CASE(C, K) case C * 8 + K: family_eval2<C, K>(w, s_idxA, s_coefA, s_idxB, s_coefB, s_S, sstride, outA, outB); return;
+#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
+    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3)
+#undef MQ_ROW
+#undef MQ_CASE
+  }
+  __trap();
+}
+
 // ------------------------------------------------------------------ a4: scalars of one piece
 // writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
 template <class T>
@@ -404,15 +442,44 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
         uint32_t an = a0 + 8 * size; uint64_t hdn = 0, n0 = 0, n1 = 0;
         const bool havenext = npos < MQ_CHUNK_WORDS;
         if (havenext) { hdn = lds_u64(an); n0 = lds_u64(an + 8); n1 = lds_u64(an + 16); }
-        T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
-        const int nb = c * (2 * c - 1) + kd;
-        for (int i = 0; i < nscal; i++) val = val * lds_T<T>(s_S + lds_u8(a0 + 8 + nb + i) * sstride);
-        if (kk != key) {
-          if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
-          key = kk; racc = T(0.0); racca = 0.0;
+        // pair this family with the next one if it has the same shape (binary64: doubles the ILP of the warp)
+        bool dual = false;
+        if constexpr (sizeof(T) == sizeof(double)) {
+          if (havenext && left > 1 && c <= 3 && (int)(hdn & 63) == (int)(hd & 63)) {
+            const int size2 = 1 + (int)(hdn >> 16 & 0xFFFF) + (int)(uint32_t)(hdn >> 32);
+            dual = npos + size2 <= MQ_CHUNK_WORDS;
+          }
         }
-        racc = racc + val;
-        if constexpr (TRACK) racca += fabs(mq_to_double(val));
+        const int nb = c * (2 * c - 1) + kd;
+        auto account = [&](T val, uint32_t ea, int ns, int keyk) {
+          for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(ea + 8 + nb + i) * sstride);
+          if (keyk != key) {
+            if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
+            key = keyk; racc = T(0.0); racca = 0.0;
+          }
+          racc = racc + val;
+          if constexpr (TRACK) racca += fabs(mq_to_double(val));
+        };
+        if (dual) {
+          if constexpr (sizeof(T) == sizeof(double)) {
+            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = 1 + idxw2 + (int)(uint32_t)(hdn >> 32), npos2 = npos + size2;
+            const int nscal2 = (int)(hdn >> 10 & 15), kk2 = (int)((hdn & 7) | ((hdn >> 6 & 15) << 3) | ((hdn >> 14 & 1) << 7));
+            const uint32_t a2 = an + 8 * size2;
+            uint64_t hd3 = 0, m0 = 0, m1 = 0;
+            const bool have3 = npos2 < MQ_CHUNK_WORDS;
+            if (have3) { hd3 = lds_u64(a2); m0 = lds_u64(a2 + 8); m1 = lds_u64(a2 + 16); }
+            const uint64_t w4[4] = {w0, w1, n0, n1};
+            double vA, vB;
+            family_dispatch2(c * 8 + kd, w4, a0 + 8, a0 + 8 + 8 * idxw, an + 8, an + 8 + 8 * idxw2, s_S, sstride, vA, vB);
+            account(T(vA), a0, nscal, kk);
+            account(T(vB), an, nscal2, kk2);
+            rd.pos = npos2; left -= 2;
+            have = have3; a0 = a2; hd = hd3; w0 = m0; w1 = m1;
+            continue;
+          }
+        }
+        T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
+        account(val, a0, nscal, kk);
         rd.pos = npos; left--;
         have = havenext; a0 = an; hd = hdn; w0 = n0; w1 = n1;
       }

@@ -26,6 +26,25 @@ def two_loop(n):
         fh.write("\n".join(lines) + "\n")
 
 
+def high_loop(L, indices, n, seed, first):
+    """per-point oracle values at L=4,5 (the oracle's table build takes minutes per graph at L=5):
+    sample index range, seed and, per point, the binary128 value rounded to binary64 (hex) and the binary64 value"""
+    lines = ["# Oracle per-point integrand values, loop order %d, points first_sample=%d..+%d of seed %d, default Deg (floor 0.75)." % (L, first, n, seed),
+             "# Written by make_oracle_golden.py (oracle only). Values of L>=4 graphs are 'parity unpinned' by the paper (DESIGN.md section 3).",
+             "# graph_index point fwide(hex) f64(hex)"]
+    for idx in indices:
+        d = po.Diagram(po.graph_get(L, idx))
+        z, p, _ = d.sample(first, n, seed)
+        r = d.eval_z(z, wide=True)
+        for k in range(n):
+            lines.append("%d %d %s %s" % (idx, k, float(r["fwide"][k]).hex(), float(r["f64"][k]).hex()))
+        print("graph", idx, "done", flush=True)
+    with open(os.path.join(HERE, "oracle_points_L%d.txt" % L), "w") as fh:
+        fh.write("\n".join(lines) + "\n")
+
+
 if __name__ == "__main__":
+    if sys.argv[1] == "high_loop":
+        high_loop(int(sys.argv[2]), [int(x) for x in sys.argv[3].split(",")], int(sys.argv[4]), 5, 1000)
     if sys.argv[1] == "two_loop":
         two_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 20000000)

@@ -160,3 +160,32 @@ def test_gpu_prepared_tables_equal_host_prepared(mc):
         b = mc.Diagram(L, e, ch, host_only=True)
         assert np.array_equal(a.blob(), b.blob())
         a.close(); b.close()
+
+
+def test_five_loop_points_against_stored_oracle_values(mc):
+    """BASELINE.json configs[4] scale (L=5, M=15): per-point parity against oracle values stored by
+    tests/golden/make_oracle_golden.py (the oracle needs minutes per 5-loop graph to build its tables)"""
+    from conftest import read_golden
+    from paper_1905_08007_b200 import workloads
+    rows = read_golden("oracle_points_L5.txt")
+    gs = workloads.all_graphs(5)
+    by_graph = {}
+    for idx, k, fw, f64 in rows:
+        by_graph.setdefault(int(idx), []).append((int(k), float.fromhex(fw), float.fromhex(f64)))
+    assert len(by_graph) >= 3
+    for idx, pts in by_graph.items():
+        g = gs[idx]
+        d = mc.Diagram(g[0], g[1], g[2])
+        assert d.id() == idx
+        n = len(pts)
+        r = _gpu_points(mc, d, 1000, n, 5)
+        fw = np.array([p[1] for p in sorted(pts)])
+        fo64 = np.array([p[2] for p in sorted(pts)])
+        unfl = r["flag"] == 0
+        rel = np.abs(r["f"] - fw) / np.abs(fw)
+        assert np.all(rel[unfl] <= 1e-10), (idx, rel[unfl].max())
+        sane = (~unfl) & (r["cond"] <= 1e16)
+        assert np.all(rel[sane] <= 1e-10), (idx, rel[sane].max() if sane.any() else 0)
+        truth = np.abs(fo64 - fw) > 1e-10 * np.abs(fw)
+        assert not np.any(truth & unfl)
+        d.close()
