@@ -16,6 +16,8 @@
 // binary lines, as one dense coefficient block the kernel evaluates with static register indexing.
 #pragma once
 #include <atomic>
+#include <chrono>
+#include <cstdio>
 #include <complex>
 #include <cstdlib>
 #include <cstring>
@@ -150,6 +152,9 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
   std::vector<std::vector<std::vector<std::pair<int, int>>>> pairingsOf(maxc + 1);
   for (int c = 0; c <= maxc; c++) allPairings(2 * c, pairingsOf[c]);
 
+  const bool timing = std::getenv("MCQED_PREPARE_TIMING") != nullptr;
+  auto tick = std::chrono::steady_clock::now();
+  auto lap = [&](const char *what) { if (timing) { auto now = std::chrono::steady_clock::now(); std::fprintf(stderr, "[mcqed prepare] %s %.1f ms\n", what, std::chrono::duration<double, std::milli>(now - tick).count()); tick = now; } };
   // ---- phase A: one counting unit per (job, pairing, variant, start spinor) ----
   struct UnitMeta { uint32_t job, pairing; int out; std::complex<double> w; };
   struct JobInfo { std::vector<int> binSlots, pairedSlots, atSlots; int qSlot = -1, pattern = 0; size_t firstUnit = 0, nUnits = 0; };
@@ -208,6 +213,7 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
     }
     ji.nUnits = units.size() - ji.firstUnit;
   }
+  lap("units");
   // ---- phase B: count paths (GPU if offered, else host threads) ----
   std::vector<int32_t> counts(nints, 0);
   bool counted = false;
@@ -228,6 +234,7 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
       w.go(0, units[i].start, 0, 0u);
     });
   }
+  lap(counted ? "count(gpu)" : "count(host)");
   // ---- phase C: coefficients and families, job by job ----
   std::vector<std::vector<Family>> famsOf(jobs.size());
   parallelFor(jobs.size(), [&](size_t j) {
@@ -270,6 +277,7 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
       }
   });
   for (auto &v : famsOf) for (auto &f : v) { tb.n_stored += (int64_t)f.coef.size(); tb.n_nonzero += f.nonzero; tb.fams.push_back(std::move(f)); }
+  lap("families");
   return tb;
 }
 

@@ -16,9 +16,9 @@
 #define MQ_MAXNODE 256
 #define MQ_MAXPAT 16      // 2^(max #S-children of a piece)
 // inner dense binary dimensions of a family, by number of Wick pairs c (bounds the static code and the family size)
-static inline int mq_kd_max(int c) { return c <= 3 ? 4 : 3; }   // larger inner blocks (5, 6) were measured slower (register spills)
+static inline int mq_kd_max(int c) { return c <= 3 ? 4 : 2; }   // keeps every family below one chunk;   // larger inner blocks (5, 6) were measured slower (register spills)
 #define MQ_MAXSCAL 12
-#define MQ_CHUNK_WORDS 2048   // staging granule of the family stream (16 KiB)
+#define MQ_CHUNK_WORDS 512    // staging granule of the family stream (4 KiB): small, so that three CTAs fit an SM
 #define MQ_PAD_MARK 7        // header field c of a PAD entry
 
 enum { MQ_OP_A = 0, MQ_OP_U = 1, MQ_OP_L = 2, MQ_OP_LMU = 3 };
@@ -42,6 +42,9 @@ struct DevGeom {
   int8_t child_patbit[MQ_MAXCHILD];       // bit position of an S-child in the compressed pattern, -1 for V
   int16_t pad;
   int32_t first_table, ntable;            // tables of this geom are consecutive
+  // per-point scalar array S of this piece: r_t at [0,nslot); A_t at off_at (only pieces with insertions, else -1);
+  // A'_t/g_t at off_aq (only pieces evaluated under operator A, else -1); beta~_tu (t<u, triangular) at off_bt
+  int32_t off_at, off_aq, off_bt, scal_len;
 };
 
 struct DevTable {

@@ -112,7 +112,6 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     }
     for (int c = 0; c < G.nchild; c++) { G.child_type[c] = p.kids[c].vertexLike ? 1 : 0; G.child_patbit[c] = (int8_t)p.patbit[c]; }
     d->geoms[gi] = G;
-    d->max_scal_len = std::max(d->max_scal_len, 3 * G.nslot + G.nslot * (G.nslot - 1) / 2);
   }
   // nodes + tables
   const bool no_tables = d->opt.flags & 2u;
@@ -148,6 +147,17 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     G.ntable++;
   }
   for (size_t t = 0; t < d->ft.terms.size(); t++) d->terms.push_back({nnew[roots[t]], d->ft.terms[t].sign});
+  // layout of the per-point scalar array of every piece (only what its tables can reference)
+  for (auto &G : d->geoms) {
+    bool needAq = false;
+    for (int ti = G.first_table; ti < G.first_table + G.ntable; ti++) needAq |= d->tables[ti].op == MQ_OP_A;
+    int o = G.nslot;
+    G.off_at = G.nS > 0 ? o : -1; if (G.nS > 0) o += G.nslot;
+    G.off_aq = needAq ? o : -1; if (needAq) o += G.nslot;
+    G.off_bt = o; o += G.nslot * (G.nslot - 1) / 2;
+    G.scal_len = o;
+    d->max_scal_len = std::max(d->max_scal_len, o);
+  }
 
   // ---- blob ----
   auto words = [](size_t bytes) { return (int64_t)((bytes + 7) / 8); };
@@ -173,7 +183,8 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     DevTable &T = d->tables[ti]; const mq::TableBuild &tb = builds[ti];
     T.stream_off = stream_base + (int64_t)streams.size(); T.nfam = (int)tb.fams.size(); T.n_monomials = tb.n_stored;
     const int ns = d->geoms[T.geom].nslot;
-    auto tri = [&](int a, int b) { if (a > b) std::swap(a, b); return 3 * ns + a * ns - a * (a + 1) / 2 + (b - a - 1); };
+    const DevGeom &GG = d->geoms[T.geom];
+    auto tri = [&](int a, int b) { if (a > b) std::swap(a, b); return GG.off_bt + a * ns - a * (a + 1) / 2 + (b - a - 1); };
     std::vector<const mq::Family *> order;
     for (auto &f : tb.fams) order.push_back(&f);
     std::stable_sort(order.begin(), order.end(), [](const mq::Family *a, const mq::Family *b) {
@@ -189,7 +200,9 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
       for (uint8_t sl : f.inner) idx.push_back(sl);                            // r_t lives at S[t]
       for (uint8_t sc : f.scal) {
         const int kind = sc >> 4, slot = sc & 15;
-        idx.push_back((uint8_t)(kind == MQ_SC_R ? slot : kind == MQ_SC_AT ? ns + slot : 2 * ns + slot));
+        const int base = kind == MQ_SC_R ? 0 : kind == MQ_SC_AT ? GG.off_at : GG.off_aq;
+        if (base < 0) return MC_ELIMIT;                                          // a table references a scalar its piece does not carry
+        idx.push_back((uint8_t)(base + slot));
       }
       int idxw = (int)words(idx.size());
       if (idxw == 0) idxw = 1;                                                 // the kernel always reads one index word

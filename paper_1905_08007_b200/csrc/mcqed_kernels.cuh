@@ -344,7 +344,7 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
   // beta_su = eps_s^T Inv eps_u ; x_s = sum_lines z_u beta_su ; A'_s = (sgn_s - sum_lines z_u beta_su sgn_u)/2
   T ig[MQ_MAXSLOT];
   V = T(0.0); G = T(1.0);
-  const int off_at = ns, off_aq = 2 * ns, off_bt = 3 * ns;
+  const int off_at = g.off_at, off_aq = g.off_aq, off_bt = g.off_bt;
   for (int s = 0; s < ns; s++) {
     const uint32_t es = g.slot[s].eps;
     T w[MQ_MAXL];
@@ -370,9 +370,9 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
     const T igs = line ? T(1.0) / gs : T(1.0);
     ig[s] = igs;
     S[s * stride] = x * igs;                                  // r_t = x_t / g_t   (lines)
-    S[(off_at + s) * stride] = T(1.0) - x;                    // A_t
+    if (off_at >= 0) S[(off_at + s) * stride] = T(1.0) - x;   // A_t
     const T sg = T((double)g.slot[s].sgn);
-    S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);       // A'_t / g_t
+    if (off_aq >= 0) S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);   // A'_t / g_t
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
       const double xd = mq_to_double(x);

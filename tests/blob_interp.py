@@ -14,12 +14,13 @@ HDR = np.dtype([("L", "<i4"), ("M", "<i4"), ("diag_id", "<i4"), ("ngeom", "<i4")
                 ("off_stream", "<i8"), ("stream_chunks", "<i8")])
 SLOT = np.dtype([("kind", "i1"), ("zline", "i1"), ("sgn", "i1"), ("child", "i1"), ("eps", "<u4")])
 GEOM = np.dtype([("nch", "<i4"), ("nslot", "<i4"), ("nchild", "<i4"), ("nS", "<i4"), ("chord_zline", "<i4", (MAXL,)), ("slot", SLOT, (MAXSLOT,)),
-                 ("child_type", "i1", (MAXCHILD,)), ("child_patbit", "i1", (MAXCHILD,)), ("pad", "<i2"), ("first_table", "<i4"), ("ntable", "<i4")])
+                 ("child_type", "i1", (MAXCHILD,)), ("child_patbit", "i1", (MAXCHILD,)), ("pad", "<i2"), ("first_table", "<i4"), ("ntable", "<i4"),
+                 ("off_at", "<i4"), ("off_aq", "<i4"), ("off_bt", "<i4"), ("scal_len", "<i4")])
 TABLE = np.dtype([("geom", "<i4"), ("op", "<i4"), ("nout", "<i4"), ("nfam", "<i4"), ("first_node", "<i4"), ("nnode", "<i4"),
                   ("stream_off", "<i8"), ("stream_words", "<i8"), ("n_monomials", "<i8")])
 NODE = np.dtype([("table", "<i4"), ("geom", "<i4"), ("nchild", "<i4"), ("nout", "<i4"), ("child", "<i4", (MAXCHILD,)), ("val_off", "<i4"), ("ngr", "<i4")])
 TERM = np.dtype([("root", "<i4"), ("sign", "<i4")])
-assert GEOM.itemsize == 168 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 128
+assert GEOM.itemsize == 184 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 128
 
 
 def pairings(n2):
@@ -84,7 +85,8 @@ class Blob:
         Inv = np.linalg.inv(A)
         E = np.array(eps, float).reshape(ns, n)
         beta = E @ Inv @ E.T
-        S = np.zeros(3 * ns + ns * (ns - 1) // 2)
+        oat, oaq, obt = int(g["off_at"]), int(g["off_aq"]), int(g["off_bt"])
+        S = np.zeros(int(g["scal_len"]))
         ig = np.ones(ns)
         V, G = 0.0, 1.0
         for s in range(ns):
@@ -98,14 +100,16 @@ class Blob:
             gs = 2.0 - x
             ig[s] = 1.0 / gs if line else 1.0
             S[s] = x * ig[s]
-            S[ns + s] = 1.0 - x
-            S[2 * ns + s] = (g["slot"][s]["sgn"] - q) * ig[s] * 0.5
+            if oat >= 0:
+                S[oat + s] = 1.0 - x
+            if oaq >= 0:
+                S[oaq + s] = (g["slot"][s]["sgn"] - q) * ig[s] * 0.5
             if line:
                 V += x * z[g["slot"][s]["zline"]]
                 G *= gs
         for s in range(ns):
             for u in range(s + 1, ns):
-                S[3 * ns + s * ns - s * (s + 1) // 2 + (u - s - 1)] = beta[s, u] * ig[s] * ig[u]
+                S[obt + s * ns - s * (s + 1) // 2 + (u - s - 1)] = beta[s, u] * ig[s] * ig[u]
         return S, U, V, G
 
     def family_value(self, c, kd, bidx, ridx, coef, S):

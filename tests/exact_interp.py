@@ -30,7 +30,8 @@ class ExactBlob(Blob):
                     f = M[r][c]; M[r] = [a - f*b for a,b in zip(M[r], M[c])]
         Inv = [row[n:] for row in M]
         beta = [[sum(Inv[i][j] for i in range(n) if eps[s][i] for j in range(n) if eps[u][j]) for u in range(ns)] for s in range(ns)]
-        S = [Fr(0)]*(3*ns + ns*(ns-1)//2); ig=[Fr(1)]*ns; V=Fr(0); G=Fr(1)
+        oat, oaq, obt = int(g["off_at"]), int(g["off_aq"]), int(g["off_bt"])
+        S = [Fr(0)]*int(g["scal_len"]); ig=[Fr(1)]*ns; V=Fr(0); G=Fr(1)
         for s in range(ns):
             x=q=Fr(0)
             for u in range(ns):
@@ -38,10 +39,12 @@ class ExactBlob(Blob):
                     zb = beta[s][u]*z[g["slot"][u]["zline"]]; x+=zb; q+=zb*int(g["slot"][u]["sgn"])
             line = g["slot"][s]["kind"]==0
             gs = 2-x; ig[s] = 1/gs if line else Fr(1)
-            S[s]=x*ig[s]; S[ns+s]=1-x; S[2*ns+s]=(int(g["slot"][s]["sgn"])-q)*ig[s]/2
+            S[s]=x*ig[s]
+            if oat >= 0: S[oat+s]=1-x
+            if oaq >= 0: S[oaq+s]=(int(g["slot"][s]["sgn"])-q)*ig[s]/2
             if line: V+=x*z[g["slot"][s]["zline"]]; G*=gs
         for s in range(ns):
-            for u in range(s+1,ns): S[3*ns+s*ns-s*(s+1)//2+(u-s-1)] = beta[s][u]*ig[s]*ig[u]
+            for u in range(s+1,ns): S[obt+s*ns-s*(s+1)//2+(u-s-1)] = beta[s][u]*ig[s]*ig[u]
         return S, det, V, G
     def family_value(self, c, kd, bidx, ridx, coef, S):
         n2=2*c
