@@ -13,17 +13,16 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
                                                          const unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  dd *S = reinterpret_cast<dd *>(smem_raw) + threadIdx.x;
-  const int stride = blockDim.x;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < cnt; base += (unsigned long long)gridDim.x * blockDim.x) {
-    const unsigned long long i = base + threadIdx.x; const bool live = i < cnt;
-    double z[MQ_MAXM];
-    const double p = draw_point<false>(v, flag_list[live ? i : cnt - 1], seed, z, nullptr);
+  for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    double z[MQ_MAXM]; double p = 1.0;
+    if (ro.gw == 0) p = draw_point<false>(v, flag_list[i < cnt ? i : cnt - 1], seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, rd, z, S, stride, f, a, amin, xmin);
+    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
     // beyond double-double (O8): 106 bits keep fewer than ~6 digits beyond a condition number of 1e26 or a pivot loss of 1e26;
@@ -39,16 +38,16 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
                                                            const unsigned long long *flag_list, const unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  dd *S = reinterpret_cast<dd *>(smem_raw) + threadIdx.x;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
-  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < cnt; base += (unsigned long long)gridDim.x * blockDim.x) {
-    const unsigned long long i = base + threadIdx.x; const bool live = i < cnt;
+  for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
     double z[MQ_MAXM];
-    const unsigned long long rel = flag_list[live ? i : cnt - 1];
-    draw_point<false>(v, first + rel, seed, z, nullptr);
+    const unsigned long long rel = flag_list[i < cnt ? i : cnt - 1];
+    if (ro.gw == 0) draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, rd, z, S, blockDim.x, f, a, amin, xmin);
+    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (live) f_out[rel] = mq_to_double(f);
   }
 }
@@ -57,14 +56,15 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
-  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
-    const bool live = base + threadIdx.x < n;
-    const uint64_t i = live ? base + threadIdx.x : n - 1;
+  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
+    const bool live = base + ro.slot < n && ro.gw == 0;
+    const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     dd f, a; double amin, xmin;
-    eval_integrand<dd>(v, rd, z, reinterpret_cast<dd *>(smem_raw) + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (live) fdd_out[i] = mq_to_double(f);
   }
 }
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
 using namespace mqk;
 
 int mq_config_dd(mc_diagram *d) {
-  d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd));
+  d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd), W_DD);
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_integrate_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
   if ((e = cudaFuncSetAttribute(k_eval_points_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;

@@ -9,23 +9,23 @@
 namespace mqk {
 
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
-__global__ void __launch_bounds__(TPB_F64) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
+__global__ void __launch_bounds__(TPB_F64, 4) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
                                                            double cond_max, double amin_min, double *partial,
                                                            unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  double *S = reinterpret_cast<double *>(smem_raw) + threadIdx.x;
-  const int stride = blockDim.x;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-  // the evaluator is CTA-collective (it stages the table stream through shared memory): every thread of the CTA
-  // runs the same number of iterations; threads past the end re-evaluate the last point and discard it
-  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t i = base + threadIdx.x; const bool live = i < n;
-    double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + (live ? i : n - 1), seed, z, nullptr);
+  // the evaluator is CTA-collective (it stages the table stream through shared memory and splits the families of a
+  // point group over W warps): every thread of the CTA runs the same number of iterations; slots past the end
+  // re-evaluate the last point and discard it; only the owner warp (gw = 0) of a group draws and accumulates
+  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
+    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0;
+    double z[MQ_MAXM]; double p = 1.0;
+    if (ro.gw == 0) p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
-    eval_integrand<double>(v, rd, z, S, stride, f, a, amin, xmin);
+    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (!live) continue;
     const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
@@ -57,15 +57,15 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
                                                           double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  double *S = reinterpret_cast<double *>(smem_raw) + threadIdx.x;
+  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
   const int M = v.h->M;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
-  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t i = base + threadIdx.x; const bool live = i < n;
-    double z[MQ_MAXM]; int32_t ord[MQ_MAXM];
-    const double p = draw_point<true>(v, first + (live ? i : n - 1), seed, z, ord);
+  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
+    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0;
+    double z[MQ_MAXM]; int32_t ord[MQ_MAXM]; double p = 1.0;
+    if (ro.gw == 0) p = draw_point<true>(v, first + (i < n ? i : n - 1), seed, z, ord);
     double f, a, amin, xmin;
-    eval_integrand<double>(v, rd, z, S, blockDim.x, f, a, amin, xmin);
+    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (!live) continue;
     const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
@@ -84,13 +84,16 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  StreamReader rd; setup_reader(rd, smem_raw, v.h->max_scal_len, sizeof(double));
-  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t i = base + threadIdx.x < n ? base + threadIdx.x : n - 1;   // surplus threads redo the last point
+  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
+    const bool live = base + ro.slot < n && ro.gw == 0;
+    const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;           // surplus slots redo the last point
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     double f, a, amin, xmin;
-    eval_integrand<double>(v, rd, z, reinterpret_cast<double *>(smem_raw) + threadIdx.x, blockDim.x, f, a, amin, xmin);
+    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    if (!live) continue;
     if (f64_out) f64_out[i] = f;
     if (cond_out) cond_out[i] = a / fabs(f);
     if (aux_out) { aux_out[2 * i] = amin; aux_out[2 * i + 1] = xmin; }
@@ -116,8 +119,8 @@ __global__ void k_fp64_peak(int iters, double *sink) {
 using namespace mqk;
 
 int mq_config_f64(mc_diagram *d) {
-  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double));
-  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double));
+  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double), W_F64);
+  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double), W_F64);
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_integrate_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_f64)) != cudaSuccess) return (int)e;
   if ((e = cudaFuncSetAttribute(k_eval_points, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;

@@ -116,7 +116,7 @@ int mc_integrate(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples,
   const bool no_dd = d->opt.flags & 1u;
   for (uint64_t done = 0; done < n_samples; done += mqk::CHUNK) {
     const uint64_t n = std::min<uint64_t>(mqk::CHUNK, n_samples - done);
-    const int g1 = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + mqk::TPB_F64 - 1) / mqk::TPB_F64);
+    const int g1 = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + mqk::PTS_F64 - 1) / mqk::PTS_F64);
     mq_launch_integrate_f64(d, g1, first_sample + done, n, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min, st);
     int g2 = 0;
     if (!no_dd) { g2 = d->grid_dd; mq_launch_integrate_dd(d, seed, st); g_launches++; }
@@ -154,7 +154,7 @@ int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint6
   const int M = d->g.M;
   for (uint64_t done = 0; done < n; done += mqk::CHUNK) {
     const uint64_t m = std::min<uint64_t>(mqk::CHUNK, n - done);
-    const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (m + mqk::TPB_EVAL - 1) / mqk::TPB_EVAL);
+    const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (m + mqk::PTS_EVAL - 1) / mqk::PTS_EVAL);
     const bool list = f_out && !no_dd;
     mq_launch_reset(d, st);
     mq_launch_eval_points(d, g1, first_sample + done, m, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min,
@@ -174,9 +174,10 @@ int mc_eval_z(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda_st
   if (!d || !d->on_device || !z_in) return MC_EINVAL;
   if (n == 0) return MC_OK;
   mq_stream st = (mq_stream)cuda_stream;
-  const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (n + mqk::TPB_EVAL - 1) / mqk::TPB_EVAL);
+  const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (n + mqk::PTS_EVAL - 1) / mqk::PTS_EVAL);
+  const int g2 = (int)std::min<uint64_t>(mqk::MAXGRID, (n + mqk::PTS_DD - 1) / mqk::PTS_DD);
   if (f64_out || cond_out || aux_out) { mq_launch_eval_z_f64(d, g1, n, z_in, f64_out, cond_out, aux_out, st); g_launches++; }
-  if (fdd_out) { mq_launch_eval_z_dd(d, g1, n, z_in, fdd_out, st); g_launches++; }
+  if (fdd_out) { mq_launch_eval_z_dd(d, g2, n, z_in, fdd_out, st); g_launches++; }
   MQ_CK(cudaGetLastError());
   return MC_OK;
 }

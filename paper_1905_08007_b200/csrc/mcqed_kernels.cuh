@@ -402,8 +402,15 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 // For T = double a second, sign-free copy of the whole computation is carried along at family granularity
 // (|family value| summed, |child value| multiplied): abs_out = sum over terms and grades of that bound. It measures
 // every cancellation between families, pieces and terms (O8) at the cost of one add per family.
-template <class T>
-__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
+//
+// Warp split: W warps share one group of 32 points. Warp gw = 0 of the group owns the points (scalars, node
+// values, terms); the families of every table are dealt round-robin to the W warps, which all read the same
+// S[index][point] in shared memory; their partial graded sums are added through the exchange area xT/xA.
+// This multiplies the warps per SM at constant shared memory per point (occupancy is otherwise capped by S).
+// CTA-collective: contains __syncthreads; every thread of the CTA must call it.
+template <class T, int W>
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T *xT, double *xA, int gw,
+                                            T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
   constexpr bool TRACK = true;
   const DevHeader &h = *v.h;
   T nodeval[/*worst case*/ 1024];
@@ -414,8 +421,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
   rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
-    T U, V, G;
-    piece_scalars<T>(g, z, S, stride, U, V, G, amin, xmin);
+    T U = T(1.0), V = T(0.0), G = T(1.0);
+    if (gw == 0) piece_scalars<T>(g, z, S, stride, U, V, G, amin, xmin);
+    if constexpr (W > 1) __syncthreads();              // S of this piece is complete before any warp gathers from it
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
       const DevTable &tb = v.tab[ti];
@@ -428,6 +436,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
       // accumulates in registers and is flushed when the key changes (families are sorted by that key)
       int key = -1; T racc = T(0.0); double racca = 0.0;
       bool have = false; uint32_t a0 = 0; uint64_t hd = 0, w0 = 0, w1 = 0;   // header + first index words of the current entry
+      int unit = 0;                                                          // evaluation units are dealt round-robin to the W warps
       for (int left = tb.nfam; left > 0;) {
         if (!have) {
           if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
@@ -468,18 +477,24 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
             uint64_t hd3 = 0, m0 = 0, m1 = 0;
             const bool have3 = npos2 < MQ_CHUNK_WORDS;
             if (have3) { hd3 = lds_u64(a2); m0 = lds_u64(a2 + 8); m1 = lds_u64(a2 + 16); }
-            const uint64_t w4[4] = {w0, w1, n0, n1};
-            double vA, vB;
-            family_dispatch2(c * 8 + kd, w4, a0 + 8, a0 + 8 + 8 * idxw, an + 8, an + 8 + 8 * idxw2, s_S, sstride, vA, vB);
-            account(T(vA), a0, nscal, kk);
-            account(T(vB), an, nscal2, kk2);
+            if (W == 1 || unit % W == gw) {
+              const uint64_t w4[4] = {w0, w1, n0, n1};
+              double vA, vB;
+              family_dispatch2(c * 8 + kd, w4, a0 + 8, a0 + 8 + 8 * idxw, an + 8, an + 8 + 8 * idxw2, s_S, sstride, vA, vB);
+              account(T(vA), a0, nscal, kk);
+              account(T(vB), an, nscal2, kk2);
+            }
+            unit++;
             rd.pos = npos2; left -= 2;
             have = have3; a0 = a2; hd = hd3; w0 = m0; w1 = m1;
             continue;
           }
         }
-        T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
-        account(val, a0, nscal, kk);
+        if (W == 1 || unit % W == gw) {
+          T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
+          account(val, a0, nscal, kk);
+        }
+        unit++;
         rd.pos = npos; left--;
         have = havenext; a0 = an; hd = hdn; w0 = n0; w1 = n1;
       }
@@ -490,7 +505,23 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] *= (1.0 / 12.0); }
       }
-      // nodes that use this table: combine with the children's graded values
+      if constexpr (W > 1) {                           // add the partial sums of the other warps of the group into warp 0
+        for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++) {
+          if (gw > 0) {
+#pragma unroll
+            for (int c = 0; c < MQ_NGRADE; c++) { xT[((gw - 1) * MQ_NGRADE + c) * stride] = N[o][p][c]; xA[((gw - 1) * MQ_NGRADE + c) * stride] = Na[o][p][c]; }
+          }
+          __syncthreads();
+          if (gw == 0) {
+            for (int w = 0; w < W - 1; w++)
+#pragma unroll
+              for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = N[o][p][c] + xT[(w * MQ_NGRADE + c) * stride]; Na[o][p][c] += xA[(w * MQ_NGRADE + c) * stride]; }
+          }
+          __syncthreads();
+        }
+      }
+      // nodes that use this table: combine with the children's graded values (owner warp only)
+      if (gw == 0)
       for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {
         const DevNode &nd = v.node[ni];
         T Up = U, Vs = V;
@@ -522,6 +553,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
   // a6: terms.  f = sum sign * sum_{c<L} (L-c-1)! N_c / (Uprod^2 Vsum^(L-c))
   const int L = h.L;
   T f = T(0.0), asum = T(0.0);
+  if (gw == 0)
   for (int t = 0; t < h.nterm; t++) {
     const DevTerm tm = v.term[t];
     const DevNode &nd = v.node[tm.root];
