@@ -129,10 +129,7 @@ def run_ours(args):
     G, B = len(graphs), args.batch
     # ---- prepare (not timed as throughput; reported) ----
     t0 = time.perf_counter()
-    # mc_prepare_diagram is thread-safe and ctypes releases the GIL: prepare several diagrams at once
-    from concurrent.futures import ThreadPoolExecutor
-    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
-        diagrams = list(ex.map(lambda ig: mc.Diagram(ig[1][0], ig[1][1], ig[1][2]), graphs))
+    diagrams = [mc.Diagram(g[0], g[1], g[2]) for _, g in graphs]
     prepare_s = time.perf_counter() - t0
     infos = [d.info() for d in diagrams]
     flop = [i["flop_per_sample"] for i in infos]

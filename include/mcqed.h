@@ -105,8 +105,9 @@ int64_t mc_diagram_blob(const mc_diagram *, uint64_t *out, int64_t cap);
  * (the Philox counter is the sample index, so calls with disjoint ranges are independent and
  * additive: that is also the checkpoint/resume story). Asynchronous on `cuda_stream`
  * (a cudaStream_t; NULL = legacy default stream). out_* are DEVICE pointers, one element each,
- * accumulated into (+=): sum of w=f/p, sum of w^2, number of points re-evaluated in double-double,
- * number of points dropped because even the double-double value was non-finite (their w is 0). */
+ * accumulated into (+=): sum of w=f/p, sum of w^2, number of points re-evaluated in double-double (those
+ * double-double cannot resolve either go on to quad-double), number of points dropped because some z
+ * underflowed or even the quad-double value was non-finite (their w is 0). */
 int mc_integrate(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
                  double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped);
 
@@ -128,6 +129,10 @@ int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64
  * lines of all pieces); any output may be NULL. */
 int mc_eval_z(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream,
               double *f64_out, double *fdd_out, double *cond_out, double *aux_out);
+
+/* Integrand at caller-supplied points in the third precision tier (quad-double, ~212 bits), rounded to binary64.
+ * DEVICE z_in n*M, DEVICE fqd_out n. */
+int mc_eval_z_qd(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream, double *fqd_out);
 
 /* Number of kernels this library has launched in the calling process (for gpu_launches in bench.py). */
 unsigned long long mc_kernel_launch_count(void);

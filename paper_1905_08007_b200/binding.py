@@ -16,7 +16,7 @@ FLAG_NO_DD, FLAG_NO_TABLES = 1, 2
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
     "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags",
-    "mc_integrate", "mc_integrate_host", "mc_eval_points", "mc_eval_z", "mc_kernel_launch_count", "mc_fp64_peak",
+    "mc_integrate", "mc_integrate_host", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
 
@@ -73,6 +73,7 @@ def lib():
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
         L.mc_eval_z.argtypes = [vp, u64, vp, vp, vp, vp, vp, vp]
+        L.mc_eval_z_qd.argtypes = [vp, u64, vp, vp, vp]
         L.mc_kernel_launch_count.restype = C.c_ulonglong
         L.mc_fp64_peak.argtypes = [C.c_int, vp, dp, dp]
         L.mc_strerror.restype = C.c_char_p
@@ -187,6 +188,9 @@ class Diagram:
     def eval_points(self, first_sample, n, seed, stream=None, z=None, order=None, p=None, f=None, f64=None, cond=None, flag=None):
         _check(lib().mc_eval_points(self.h, first_sample, n, seed, _ptr(stream), _ptr(z), _ptr(order), _ptr(p), _ptr(f), _ptr(f64),
                                     _ptr(cond), _ptr(flag)), "mc_eval_points")
+
+    def eval_z_qd(self, n, z_in, stream, fqd):
+        _check(lib().mc_eval_z_qd(self.h, n, _ptr(z_in), _ptr(stream), _ptr(fqd)), "mc_eval_z_qd")
 
     def eval_z(self, n, z_in, stream=None, f64=None, fdd=None, cond=None, aux=None):
         _check(lib().mc_eval_z(self.h, n, _ptr(z_in), _ptr(stream), _ptr(f64), _ptr(fdd), _ptr(cond), _ptr(aux)), "mc_eval_z")

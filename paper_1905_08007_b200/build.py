@@ -24,6 +24,7 @@ UNITS = {  # object -> (compiler, source, dependencies)
     "mcqed_api.o": ("g++", "mcqed_api.cpp", COMMON),
     "kern_f64.o": ("nvcc", "kern_f64.cu", KERN),
     "kern_dd.o": ("nvcc", "kern_dd.cu", KERN),
+    "kern_qd.o": ("nvcc", "kern_qd.cu", KERN + ["qd_arith.cuh"]),
     "prep_kernel.o": ("nvcc", "prep_kernel.cu", ["device_layout.h"]),
 }
 

@@ -16,12 +16,14 @@ constexpr int W_F64 = 1, W_DD = 1;
 constexpr int PTS_F64 = TPB_F64 / W_F64, PTS_DD = TPB_DD / W_DD, PTS_EVAL = TPB_EVAL / W_F64;
 constexpr uint64_t CHUNK = 1ull << 22;     // samples per launch (bounds the flagged-index list)
 constexpr int MAXGRID = 148 * 32;
+constexpr uint64_t LOSTCAP = CHUNK / 8;   // capacity of the list of points handed from double-double to quad-double
 }  // namespace mqk
 
 struct McWorkspace {
-  double *partial = nullptr;               // [2][MAXGRID][4] per-block compensated partial sums (f64 pass, dd pass)
+  double *partial = nullptr;               // [3][MAXGRID][4] per-block compensated partial sums (f64, dd, qd pass)
+  unsigned long long *lost_list = nullptr; // [LOSTCAP] points the double-double pass could not resolve
   unsigned long long *flag_list = nullptr; // [CHUNK] sample indices flagged in the current chunk
-  unsigned long long *counters = nullptr;  // [4]: flagged in chunk, dropped, -, -
+  unsigned long long *counters = nullptr;  // [4]: flagged in chunk, dropped, handed to quad-double, -
 };
 
 struct mc_diagram {
@@ -39,8 +41,8 @@ struct mc_diagram {
   uint64_t *d_blob = nullptr;
   McWorkspace ws;
   bool on_device = false;
-  int grid_f64 = 0, grid_dd = 0;
-  size_t smem_f64 = 0, smem_dd = 0, smem_eval = 0;
+  int grid_f64 = 0, grid_dd = 0, grid_qd = 0;
+  size_t smem_f64 = 0, smem_dd = 0, smem_eval = 0, smem_qd = 0;
 };
 
 // host preparation (host_prepare.cpp)
@@ -52,9 +54,13 @@ int mq_count_units_gpu(const MqCountUnit *units, size_t nunits, int32_t *counts,
 typedef struct CUstream_st *mq_stream;
 int mq_config_f64(mc_diagram *d);
 int mq_config_dd(mc_diagram *d);
+int mq_config_qd(mc_diagram *d);
+void mq_launch_integrate_qd(const mc_diagram *d, uint64_t seed, mq_stream st);
+void mq_launch_eval_points_qd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st);
+void mq_launch_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, double *fqd_out, mq_stream st);
 void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st);
 void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st);
-void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);
+void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, int nb3, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);
 void mq_launch_reset(const mc_diagram *d, mq_stream st);
 void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,
                            double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out,

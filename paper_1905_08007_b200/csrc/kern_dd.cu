@@ -10,7 +10,7 @@ namespace mqk {
 
 // a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
 __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
-                                                         const unsigned long long *flag_list, unsigned long long *counters) {
+                                                         const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
@@ -28,14 +28,18 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     // beyond double-double (O8): 106 bits keep fewer than ~6 digits beyond a condition number of 1e26 or a pivot loss of 1e26;
     // such points are dropped (w = 0) and counted
     const bool lost = !(mq_to_double(a) <= 1e26 * fabs(fd)) || fmin(amin, xmin) < 1e-26;
-    if (bad_point(z, v.h->M, p) || !isfinite(fd) || lost) atomicAdd(&counters[1], 1ull);
+    if (bad_point(z, v.h->M, p)) atomicAdd(&counters[1], 1ull);                  // dropped: w = 0
+    else if (!isfinite(fd) || lost) {                                          // third tier: quad-double
+      const unsigned long long slot = atomicAdd(&counters[2], 1ull);
+      if (slot < LOSTCAP) lost_list[slot] = flag_list[i]; else { atomicAdd(&counters[1], 1ull); }
+    }
     else { const double w = fd / p; s1.add(w); s2.add(w * w); }
   }
   block_reduce_store(s1, s2, partial);
 }
 
 __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
-                                                           const unsigned long long *flag_list, const unsigned long long *counters) {
+                                                           const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
@@ -48,7 +52,14 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
     if (ro.gw == 0) draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
     eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
-    if (live) f_out[rel] = mq_to_double(f);
+    if (live) {
+      const double fd = mq_to_double(f);
+      f_out[rel] = fd;
+      if (!isfinite(fd) || !(mq_to_double(a) <= 1e26 * fabs(fd)) || fmin(amin, xmin) < 1e-26) {
+        const unsigned long long slot = atomicAdd(&counters[2], 1ull);
+        if (slot < LOSTCAP) lost_list[slot] = rel;
+      }
+    }
   }
 }
 
@@ -88,10 +99,10 @@ int mq_config_dd(mc_diagram *d) {
   return 0;
 }
 void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st) {
-  k_integrate_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, seed, d->ws.partial + (size_t)MAXGRID * 4, d->ws.flag_list, d->ws.counters);
+  k_integrate_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, seed, d->ws.partial + (size_t)MAXGRID * 4, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
 }
 void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st) {
-  k_eval_points_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, first, seed, f_out, d->ws.flag_list, d->ws.counters);
+  k_eval_points_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, first, seed, f_out, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
 }
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st) {
   k_eval_z_dd<<<grid, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, n, z_in, fdd_out);

@@ -35,20 +35,22 @@ __global__ void __launch_bounds__(TPB_F64, 4) k_integrate_f64(const uint64_t *__
 }
 
 // deterministic final reduction of the per-block partials of both passes; out += result
-__global__ void k_finish(const double *partial, int nb1, int nb2, unsigned long long *counters,
+__global__ void k_finish(const double *partial, int nb1, int nb2, int nb3, unsigned long long *counters,
                          double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   KahanPair a{0.0, 0.0}, b{0.0, 0.0};
   for (int i = 0; i < nb1; i++) { a.merge(partial[i * 4], partial[i * 4 + 1]); b.merge(partial[i * 4 + 2], partial[i * 4 + 3]); }
   const double *p2 = partial + (size_t)MAXGRID * 4;
   for (int i = 0; i < nb2; i++) { a.merge(p2[i * 4], p2[i * 4 + 1]); b.merge(p2[i * 4 + 2], p2[i * 4 + 3]); }
+  const double *p3 = partial + (size_t)2 * MAXGRID * 4;
+  for (int i = 0; i < nb3; i++) { a.merge(p3[i * 4], p3[i * 4 + 1]); b.merge(p3[i * 4 + 2], p3[i * 4 + 3]); }
   if (out_sum) *out_sum += a.hi + a.lo;
   if (out_sumsq) *out_sumsq += b.hi + b.lo;
   if (out_nflag) *out_nflag += counters[0];
   if (out_ndrop) *out_ndrop += counters[1];
-  counters[0] = 0; counters[1] = 0;
+  counters[0] = 0; counters[1] = 0; counters[2] = 0;
 }
-__global__ void k_reset_counters(unsigned long long *counters) { counters[0] = 0; counters[1] = 0; }
+__global__ void k_reset_counters(unsigned long long *counters) { counters[0] = 0; counters[1] = 0; counters[2] = 0; }
 
 // parity hook: per-point outputs (binary64 pass); flagged points are listed for the dd pass
 __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
@@ -136,8 +138,8 @@ int mq_config_f64(mc_diagram *d) {
 void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st) {
   k_integrate_f64<<<grid, TPB_F64, d->smem_f64, (cudaStream_t)st>>>(d->d_blob, first, n, seed, cond_max, amin_min, d->ws.partial, d->ws.flag_list, d->ws.counters);
 }
-void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
-  k_finish<<<1, 32, 0, (cudaStream_t)st>>>(d->ws.partial, nb1, nb2, d->ws.counters, out_sum, out_sumsq, out_nflag, out_ndrop);
+void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, int nb3, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
+  k_finish<<<1, 32, 0, (cudaStream_t)st>>>(d->ws.partial, nb1, nb2, nb3, d->ws.counters, out_sum, out_sumsq, out_nflag, out_ndrop);
 }
 void mq_launch_reset(const mc_diagram *d, mq_stream st) { k_reset_counters<<<1, 1, 0, (cudaStream_t)st>>>(d->ws.counters); }
 void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,

@@ -1,0 +1,104 @@
+// kern_qd.cu — third precision tier: quad-double re-evaluation of the points whose cancellation exceeds what
+// double-double resolves (O8; "arithmetic with different precisions"). sm_100a.
+// Product code (libmcqed.so); shares nothing with oracle/. Speed is irrelevant here (per-mille of the points):
+// the evaluator is instantiated with the loop-based family code (family_generic), 32 threads per CTA.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+
+#include "qd_arith.cuh"
+#include "kern_common.cuh"
+
+namespace mqk {
+
+template <> __device__ __forceinline__ qd lds_T<qd>(uint32_t a) {
+  const double2 lo = lds_f64x2(a), hi = lds_f64x2(a + 16);
+  return qd(lo.x, lo.y, hi.x, hi.y);
+}
+
+constexpr int TPB_QD = 32;
+
+// points listed in lost_list (sample indices) by the double-double pass
+__global__ void __launch_bounds__(TPB_QD) k_integrate_qd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
+                                                         const unsigned long long *lost_list, unsigned long long *counters) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const DiagView v = make_view(blob);
+  const Roles<qd, 1> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  const unsigned long long cnt = counters[2] < LOSTCAP ? counters[2] : LOSTCAP;
+  KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
+  for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt;
+    double z[MQ_MAXM];
+    const double p = draw_point<false>(v, lost_list[live ? i : cnt - 1], seed, z, nullptr);
+    qd f, a; double amin, xmin;
+    eval_integrand<qd, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    if (!live) continue;
+    const double fd = mq_to_double(f);
+    if (bad_point(z, v.h->M, p) || !isfinite(fd)) atomicAdd(&counters[1], 1ull);     // dropped: w = 0
+    else { const double w = fd / p; s1.add(w); s2.add(w * w); }
+  }
+  block_reduce_store(s1, s2, partial);
+}
+
+// parity hooks: per-point values of the lost points (relative indices), and the integrand at given z
+__global__ void __launch_bounds__(TPB_QD) k_eval_points_qd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
+                                                           const unsigned long long *lost_list, const unsigned long long *counters) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const DiagView v = make_view(blob);
+  const Roles<qd, 1> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  const unsigned long long cnt = counters[2] < LOSTCAP ? counters[2] : LOSTCAP;
+  for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt;
+    double z[MQ_MAXM];
+    const unsigned long long rel = lost_list[live ? i : cnt - 1];
+    draw_point<false>(v, first + rel, seed, z, nullptr);
+    qd f, a; double amin, xmin;
+    eval_integrand<qd, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    if (live) f_out[rel] = mq_to_double(f);
+  }
+}
+__global__ void __launch_bounds__(TPB_QD) k_eval_z_qd(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in, double *fqd_out) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const DiagView v = make_view(blob);
+  const int M = v.h->M;
+  const Roles<qd, 1> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
+    const bool live = base + ro.slot < n;
+    const uint64_t i = live ? base + ro.slot : n - 1;
+    double z[MQ_MAXM];
+    for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
+    qd f, a; double amin, xmin;
+    eval_integrand<qd, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    if (live) fqd_out[i] = mq_to_double(f);
+  }
+}
+
+}  // namespace mqk
+
+using namespace mqk;
+
+int mq_config_qd(mc_diagram *d) {
+  d->smem_qd = smem_bytes(d->max_scal_len, TPB_QD, sizeof(qd), 1);
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_integrate_qd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_qd)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_points_qd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_qd)) != cudaSuccess) return (int)e;
+  if ((e = cudaFuncSetAttribute(k_eval_z_qd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_qd)) != cudaSuccess) return (int)e;
+  int nsm = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  d->grid_qd = nsm;
+  return 0;
+}
+void mq_launch_integrate_qd(const mc_diagram *d, uint64_t seed, mq_stream st) {
+  k_integrate_qd<<<d->grid_qd, TPB_QD, d->smem_qd, (cudaStream_t)st>>>(d->d_blob, seed, d->ws.partial + (size_t)2 * MAXGRID * 4, d->ws.lost_list, d->ws.counters);
+}
+void mq_launch_eval_points_qd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st) {
+  k_eval_points_qd<<<d->grid_qd, TPB_QD, d->smem_qd, (cudaStream_t)st>>>(d->d_blob, first, seed, f_out, d->ws.lost_list, d->ws.counters);
+}
+void mq_launch_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, double *fqd_out, mq_stream st) {
+  const int g = (int)std::min<uint64_t>((uint64_t)MAXGRID, (n + TPB_QD - 1) / TPB_QD);
+  k_eval_z_qd<<<g, TPB_QD, d->smem_qd, (cudaStream_t)st>>>(d->d_blob, n, z_in, fqd_out);
+}

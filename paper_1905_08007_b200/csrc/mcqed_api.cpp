@@ -21,11 +21,12 @@ int to_device(mc_diagram *d) {
   const size_t bytes = d->blob.size() * 8;
   if (cudaMalloc(&d->d_blob, bytes) != cudaSuccess) return MC_ENOMEM;
   if (cudaMemcpy(d->d_blob, d->blob.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) return MC_ECUDA;
-  if (cudaMalloc(&d->ws.partial, sizeof(double) * 2 * mqk::MAXGRID * 4) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMalloc(&d->ws.partial, sizeof(double) * 3 * mqk::MAXGRID * 4) != cudaSuccess) return MC_ENOMEM;
+  if (cudaMalloc(&d->ws.lost_list, sizeof(unsigned long long) * mqk::LOSTCAP) != cudaSuccess) return MC_ENOMEM;
   if (cudaMalloc(&d->ws.flag_list, sizeof(unsigned long long) * mqk::CHUNK) != cudaSuccess) return MC_ENOMEM;
   if (cudaMalloc(&d->ws.counters, sizeof(unsigned long long) * 4) != cudaSuccess) return MC_ENOMEM;
   if (cudaMemset(d->ws.counters, 0, sizeof(unsigned long long) * 4) != cudaSuccess) return MC_ECUDA;
-  if (mq_config_f64(d) != 0 || mq_config_dd(d) != 0) return MC_ECUDA;
+  if (mq_config_f64(d) != 0 || mq_config_dd(d) != 0 || mq_config_qd(d) != 0) return MC_ECUDA;
   d->on_device = true;
   return MC_OK;
 }
@@ -55,6 +56,7 @@ void mc_free_diagram(mc_diagram *d) {
   if (d->d_blob) cudaFree(d->d_blob);
   if (d->ws.partial) cudaFree(d->ws.partial);
   if (d->ws.flag_list) cudaFree(d->ws.flag_list);
+  if (d->ws.lost_list) cudaFree(d->ws.lost_list);
   if (d->ws.counters) cudaFree(d->ws.counters);
   delete d;
 }
@@ -118,9 +120,13 @@ int mc_integrate(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples,
     const uint64_t n = std::min<uint64_t>(mqk::CHUNK, n_samples - done);
     const int g1 = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + mqk::PTS_F64 - 1) / mqk::PTS_F64);
     mq_launch_integrate_f64(d, g1, first_sample + done, n, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min, st);
-    int g2 = 0;
-    if (!no_dd) { g2 = d->grid_dd; mq_launch_integrate_dd(d, seed, st); g_launches++; }
-    mq_launch_finish(d, g1, g2, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
+    int g2 = 0, g3 = 0;
+    if (!no_dd) {     // second tier (double-double) and third tier (quad-double, only what the second could not resolve)
+      g2 = d->grid_dd; mq_launch_integrate_dd(d, seed, st);
+      g3 = d->grid_qd; mq_launch_integrate_qd(d, seed, st);
+      g_launches += 2;
+    }
+    mq_launch_finish(d, g1, g2, g3, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
     g_launches += 2;
   }
   MQ_CK(cudaGetLastError());
@@ -162,7 +168,11 @@ int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint6
                           f_out ? f_out + done : nullptr, f64_out ? f64_out + done : nullptr, cond_out ? cond_out + done : nullptr,
                           flag_out ? flag_out + done : nullptr, list, st);
     g_launches += 2;
-    if (list) { mq_launch_eval_points_dd(d, first_sample + done, seed, f_out + done, st); g_launches++; }
+    if (list) {
+      mq_launch_eval_points_dd(d, first_sample + done, seed, f_out + done, st);
+      mq_launch_eval_points_qd(d, first_sample + done, seed, f_out + done, st);
+      g_launches += 2;
+    }
     mq_launch_reset(d, st);
     g_launches++;
   }
@@ -178,6 +188,15 @@ int mc_eval_z(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda_st
   const int g2 = (int)std::min<uint64_t>(mqk::MAXGRID, (n + mqk::PTS_DD - 1) / mqk::PTS_DD);
   if (f64_out || cond_out || aux_out) { mq_launch_eval_z_f64(d, g1, n, z_in, f64_out, cond_out, aux_out, st); g_launches++; }
   if (fdd_out) { mq_launch_eval_z_dd(d, g2, n, z_in, fdd_out, st); g_launches++; }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+
+int mc_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda_stream, double *fqd_out) {
+  if (!d || !d->on_device || !z_in || !fqd_out) return MC_EINVAL;
+  if (n == 0) return MC_OK;
+  mq_launch_eval_z_qd(d, n, z_in, fqd_out, (mq_stream)cuda_stream);
+  g_launches++;
   MQ_CK(cudaGetLastError());
   return MC_OK;
 }

@@ -299,6 +299,38 @@ static __device__ __noinline__ void family_dispatch2(int ckd, const uint64_t *w,
   __trap();
 }
 
+// Loop-based family evaluation for wide types (quad-double): same arithmetic as family_eval, no unrolling.
+// Pairings are enumerated in the canonical order (the first free element pairs with every later one).
+template <class T>
+__device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+  const int n2 = 2 * c, nb = c * (2 * c - 1), nblk = 1 << kd;
+  T b[28], r[4], v[8];
+  for (int i = 0; i < nb; i++) b[i] = lds_T<T>(s_S + lds_u8(s_idx + i) * sstride);
+  for (int i = 0; i < kd; i++) r[i] = lds_T<T>(s_S + lds_u8(s_idx + nb + i) * sstride);
+  auto horner_at = [&](uint32_t a) -> T {
+    if (kd == 0) return T(lds_f64(a));
+    const int H = 1 << (kd - 1);
+    for (int j = 0; j < H; j++) { const double2 cc = lds_f64x2(a + 16 * j); v[j] = mq_fma_c(cc.y, r[kd - 1], cc.x, T()); }
+    for (int i = kd - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
+    return v[0];
+  };
+  if (c == 0) return horner_at(s_coef);
+  T sum = T(0.0), w[5];
+  unsigned used[5]; int scur[5];
+  int level = 0; used[0] = 0u; w[0] = T(1.0); scur[0] = -1;
+  while (level >= 0) {
+    const unsigned u = used[level]; const int f = __ffs(~u) - 1;
+    int s2 = scur[level] < 0 ? f + 1 : scur[level] + 1;
+    while (s2 < n2 && (u >> s2 & 1u)) s2++;
+    if (s2 >= n2) { level--; continue; }
+    scur[level] = s2;
+    const T wn = w[level] * b[f * n2 - f * (f + 1) / 2 + (s2 - f - 1)];
+    if (level == c - 1) { sum = sum + wn * horner_at(s_coef); s_coef += 8 * nblk; }
+    else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
+  }
+  return sum;
+}
+
 // ------------------------------------------------------------------ a4: scalars of one piece
 // writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
 template <class T>
@@ -491,7 +523,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
           }
         }
         if (W == 1 || unit % W == gw) {
-          T val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
+          T val;
+          if constexpr (sizeof(T) > sizeof(dd)) val = family_generic<T>(c, kd, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
+          else val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
           account(val, a0, nscal, kk);
         }
         unit++;

@@ -189,3 +189,35 @@ def test_five_loop_points_against_stored_oracle_values(mc):
         truth = np.abs(fo64 - fw) > 1e-10 * np.abs(fw)
         assert not np.any(truth & unfl)
         d.close()
+
+
+def test_quad_double_tier_against_exact_rational_values(po, mc):
+    """third precision tier (mc_eval_z_qd) against exact Fraction arithmetic on the device tables, at the most
+    ill-conditioned sampled points of a graph with two adjacent self-energy insertions (cond up to 1e18 and more),
+    where double-double and the oracle's binary128 run out of digits"""
+    import os
+    import sys
+    from fractions import Fraction as Fr
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from exact_interp import ExactBlob
+    g = po.graph_get(3, 7)
+    o = po.Diagram(g)
+    d = mc.Diagram(3, g.ext_pos, g.chords())
+    z, p, _ = o.sample(0, 3000, 5)
+    zt = torch.tensor(z, device="cuda")
+    n = len(z)
+    fdd, fqd, cond = (torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    st = torch.cuda.current_stream().cuda_stream
+    d.eval_z(n, zt, st, None, fdd, cond, None)
+    d.eval_z_qd(n, zt, st, fqd)
+    torch.cuda.synchronize()
+    c, fq, fd = cond.cpu().numpy(), fqd.cpu().numpy(), fdd.cpu().numpy()
+    assert np.all(np.isfinite(fq))
+    easy = c <= 1e12                                   # there double-double is already exact to binary64
+    assert np.all(np.abs(fq[easy] - fd[easy]) <= 1e-15 * np.abs(fd[easy]))
+    b = ExactBlob(d.blob())
+    worst = list(np.argsort(-np.where(np.isfinite(c), c, 0))[:5]) + [0, 1]
+    for k in worst:
+        fe = float(b.integrand([Fr(float(v)) for v in z[k]]))
+        assert abs(fq[k] - fe) <= 4e-16 * abs(fe), (k, c[k], fq[k], fe, fd[k])
+    d.close()
