@@ -134,14 +134,14 @@ def run_ours(args):
     infos = [d.info() for d in diagrams]
     flop = [i["flop_per_sample"] for i in infos]
     stream = torch.cuda.current_stream().cuda_stream
-    sums = torch.zeros(G, 2, dtype=torch.float64, device="cuda")
-    cnts = torch.zeros(G, 2, dtype=torch.int64, device="cuda")
-    state = {"first": rank * (1 << 44)}        # disjoint sample-index ranges per rank (weak scaling, no collective)
+    batch = mc.Batch(diagrams, B)                # one persistent launch per precision tier for the whole diagram set
+    sums = torch.zeros(2, G, dtype=torch.float64, device="cuda")
+    cnts = torch.zeros(2, G, dtype=torch.int64, device="cuda")
+    state = {"first": rank * (1 << 44), "flags": 0}        # disjoint sample-index ranges per rank (weak scaling, no collective)
 
     def step():
         f = state["first"]
-        for i, d in enumerate(diagrams):
-            d.integrate(f, B, seed, stream, sums[i, 0:1], sums[i, 1:2], cnts[i, 0:1], cnts[i, 1:2])
+        batch.integrate(f, B, seed, stream, sums[0], sums[1], cnts[0], cnts[1], flags=state["flags"])
         state["first"] = f + B
 
     def barrier():
@@ -179,38 +179,45 @@ def run_ours(args):
     value = world * G * n_tot / (ms * 1e-3)
     var_sum = 0.0
     for i in range(G):
-        mean = s[i, 0] / n_tot
-        var_sum += max(s[i, 1] / n_tot - mean * mean, 0.0) / n_tot
-    flagged_frac = float(c[:, 0].sum()) / (G * n_tot)
-    # ---- per-kernel times: the same steps with the double-double pass switched off time k_integrate_f64 alone ----
-    for d in diagrams:
-        d.set_flags(mc.FLAG_NO_DD)
+        mean = s[0, i] / n_tot
+        var_sum += max(s[1, i] / n_tot - mean * mean, 0.0) / n_tot
+    flagged_frac = float(c[0].sum()) / (G * n_tot)
+    # ---- per-kernel times: the same steps with the higher tiers switched off (flags bit 0: binary64 kernel alone;
+    #      bit 1: no quad-double pass); the double-double and quad-double kernels are timed as the differences ----
+    state["flags"] = mc.FLAG_NO_DD
     step()
     ms_f64 = timed(args.steps)
-    for d in diagrams:
-        d.set_flags(0)
-    ms_dd = max(ms - ms_f64, 0.0)
+    state["flags"] = mc.FLAG_NO_QD
+    keep = (sums.clone(), cnts.clone())
+    step()
+    cnts.zero_()
+    ms_noqd = timed(args.steps)
+    n_qd = float(cnts[1].sum().item())           # with the quad-double pass skipped its points are counted as dropped
+    sums.copy_(keep[0]); cnts.copy_(keep[1])
+    state["flags"] = 0
+    ms_dd = max(ms_noqd - ms_f64, 0.0)
+    ms_qd = max(ms - ms_noqd, 0.0)
     peak_flops, _ = mc.fp64_peak(4096)
     flops_f64 = sum(flop) * n_tot                                    # every point goes through the binary64 kernel
-    flops_dd = float(sum(fl * cc for fl, cc in zip(flop, c[:, 0])))  # flagged points are re-evaluated (same algorithmic flop)
+    flops_dd = float(sum(fl * cc for fl, cc in zip(flop, c[0])))     # flagged points are re-evaluated (same algorithmic flop)
     ach_f64 = flops_f64 / (ms_f64 * 1e-3) if ms_f64 > 0 else 0.0
     ach_dd = flops_dd / (ms_dd * 1e-3) if ms_dd > 0 else 0.0
-    dom = "k_integrate_dd" if ms_dd > ms_f64 else "k_integrate_f64"
-    ach = ach_dd if dom == "k_integrate_dd" else ach_f64
+    dom = "k_batch_dd" if ms_dd > ms_f64 else "k_batch_f64"
+    ach = ach_dd if dom == "k_batch_dd" else ach_f64
     roofline = {"bound": "alu", "kernel": dom, "achieved": ach / 1e12, "peak": peak_flops / 1e12, "unit": "TFLOP/s", "frac": ach / peak_flops,
-                "traffic": {"k_integrate_dd": 108.4e6, "k_integrate_f64": 190.5e6}[dom], "traffic_note": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r1_v2_ncu_details.txt); the algorithmic bytes are ~0 (no per-sample input): this is per-thread stack spilling to DRAM",
+                "traffic": None,
                 "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
-                "kernels": {"k_integrate_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
-                            "k_integrate_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
-                                               "points_per_step": float(c[:, 0].sum()) / args.steps,
-                                               "note": "double-double: ~20 binary64 flop per algorithmic flop, so frac is bounded by ~0.05"}}}
-    # ---- end to end through the public host-pointer API (mc_integrate_host: results copied back every call) ----
+                "kernels": {"k_batch_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
+                            "k_batch_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
+                                           "points_per_step": float(c[0].sum()) / args.steps,
+                                           "note": "double-double: one algorithmic flop costs 5-6 binary64 instructions (pair arithmetic), so frac is bounded by ~0.18"},
+                            "k_batch_qd": {"ms_per_step": ms_qd / args.steps, "points_per_step": n_qd / args.steps}}}
+    # ---- end to end through the public host-pointer API (mc_batch_integrate_host: results copied back every call) ----
     barrier()
     t0 = time.perf_counter()
     f = state["first"]
     for _ in range(args.steps):
-        for d in diagrams:
-            d.integrate_host(f, B, seed, stream)
+        batch.integrate_host(f, B, seed, stream)
         f += B
     barrier()
     e2e_s = time.perf_counter() - t0
@@ -225,8 +232,8 @@ def run_ours(args):
             "config": {"workload": "configs[%d]: %d seeded 5-loop graphs without lepton loops, %d points per graph per step" % (args.config, G, B) if args.config == 4
                        else "configs[%d]: %d graphs, %d points per graph per step" % (args.config, G, B),
                        "n_graphs": G, "batch": B, "seed": seed, "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
-                       "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "dropped": int(c[:, 1].sum()),
-                       "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[:, 0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
+                       "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "dropped": int(c[1].sum()),
+                       "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
                        "algorithmic_flop_per_sample_mean": sum(flop) / G},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

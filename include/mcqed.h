@@ -116,6 +116,31 @@ int mc_integrate(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, 
 int mc_integrate_host(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
                       double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
 
+/* Batched form of the hot path: the same computation as mc_integrate for EVERY diagram of a set, with one
+ * persistent kernel launch per precision tier for the whole set instead of three launches per diagram. The
+ * paper's workload is a sum over thousands of graphs (Table 1 :112-124): per-diagram launches
+ * leave the GPU idle in the tail of every launch (a point costs up to milliseconds in double-double), a set-wide
+ * work queue has one tail per call. Work items are CTA-loads of points of one diagram; results do not depend on
+ * which CTA ran which item (per-item compensated partial sums, added in item order).
+ *   mc_batch_create: diagrams = HOST array of n_diagrams device-prepared handles (they must outlive the batch);
+ *     max_samples_per_call bounds n_samples of one pass (longer calls are split); allocates the device work space
+ *     (about 8 bytes per diagram and sample of one pass).
+ *   mc_batch_integrate: sample indices first_sample .. first_sample+n_samples-1 of every diagram (each with its own
+ *     diagram id in the Philox counter, as in mc_integrate). out_* are DEVICE arrays of n_diagrams elements,
+ *     accumulated into (+=); any may be NULL. flags bit 0: skip the double-double / quad-double passes (flagged
+ *     points then contribute 0; used to time the binary64 kernel alone); bit 1: skip the quad-double pass only (its
+ *     points contribute 0 and are counted as dropped). Asynchronous on cuda_stream.
+ *   mc_batch_integrate_host: same with HOST output arrays (n_diagrams each; overwritten, not accumulated);
+ *     synchronises the stream.
+ * Errors: MC_EINVAL (NULL / host-only handle, n_diagrams < 1, max_samples_per_call 0 or > 2^30), MC_ENOMEM, MC_ECUDA. */
+typedef struct mc_batch mc_batch;
+int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint64_t max_samples_per_call, mc_batch **out);
+int mc_batch_integrate(mc_batch *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
+                       double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped);
+int mc_batch_integrate_host(mc_batch *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
+                            double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
+void mc_batch_free(mc_batch *);
+
 /* Parity hook: per-point values for comparison with the oracle. DEVICE outputs, any may be NULL:
  * z_out n*M (row = point, column = line index), order_out n*M (the Hepp sector j_1..j_M),
  * p_out n (density), f_out n (value used by mc_integrate: binary64, or double-double rounded to

@@ -11,12 +11,13 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ELIMIT = 0, -1, -2, -3, -4
-FLAG_NO_DD, FLAG_NO_TABLES = 1, 2
+FLAG_NO_DD, FLAG_NO_TABLES = 1, 2    # mc_options.flags
+FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
     "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags",
-    "mc_integrate", "mc_integrate_host", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
+    "mc_integrate", "mc_integrate_host", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
 
@@ -71,6 +72,11 @@ def lib():
         L.mc_diagram_set_flags.argtypes = [vp, C.c_uint32]
         L.mc_integrate.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
+        L.mc_batch_create.argtypes = [C.POINTER(vp), C.c_int32, u64, C.POINTER(vp)]
+        L.mc_batch_integrate.argtypes = [vp, u64, u64, u64, C.c_uint32, vp, vp, vp, vp, vp]
+        L.mc_batch_integrate_host.argtypes = [vp, u64, u64, u64, C.c_uint32, vp, vp, vp, vp, vp]
+        L.mc_batch_free.argtypes = [vp]
+        L.mc_batch_free.restype = None
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
         L.mc_eval_z.argtypes = [vp, u64, vp, vp, vp, vp, vp, vp]
         L.mc_eval_z_qd.argtypes = [vp, u64, vp, vp, vp]
@@ -194,6 +200,35 @@ class Diagram:
 
     def eval_z(self, n, z_in, stream=None, f64=None, fdd=None, cond=None, aux=None):
         _check(lib().mc_eval_z(self.h, n, _ptr(z_in), _ptr(stream), _ptr(f64), _ptr(fdd), _ptr(cond), _ptr(aux)), "mc_eval_z")
+
+
+class Batch:
+    """RAII handle around mc_batch*: a set of device-prepared Diagrams integrated by one launch per precision tier"""
+
+    def __init__(self, diagrams, max_samples_per_call):
+        self.diagrams = list(diagrams)                   # keeps the handles alive
+        arr = (C.c_void_p * len(self.diagrams))(*[d.h.value for d in self.diagrams])
+        self.h = C.c_void_p()
+        _check(lib().mc_batch_create(arr, len(self.diagrams), max_samples_per_call, C.byref(self.h)), "mc_batch_create")
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().mc_batch_free(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def integrate(self, first_sample, n_samples, seed, stream, out_sum, out_sumsq, out_n_flagged, out_n_dropped, flags=0):
+        """mc_batch_integrate: out_* are device tensors/pointers of len(diagrams) elements (accumulated into)"""
+        _check(lib().mc_batch_integrate(self.h, first_sample, n_samples, seed, flags, _ptr(stream), _ptr(out_sum), _ptr(out_sumsq),
+                                        _ptr(out_n_flagged), _ptr(out_n_dropped)), "mc_batch_integrate")
+
+    def integrate_host(self, first_sample, n_samples, seed, stream=None, flags=0):
+        n = len(self.diagrams)
+        s, s2, nf, nd = np.zeros(n), np.zeros(n), np.zeros(n, np.uint64), np.zeros(n, np.uint64)
+        _check(lib().mc_batch_integrate_host(self.h, first_sample, n_samples, seed, flags, _ptr(stream), _ptr(s), _ptr(s2), _ptr(nf), _ptr(nd)),
+               "mc_batch_integrate_host")
+        return s, s2, nf, nd
 
 
 def kernel_launch_count():

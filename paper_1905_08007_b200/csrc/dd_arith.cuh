@@ -60,28 +60,41 @@ __device__ __forceinline__ dd &operator*=(dd &a, dd b) { a = a * b; return a; }
 
 // generic helpers so that one templated evaluator serves binary64 and double-double
 __device__ __forceinline__ double mq_fma(double a, double b, double c) { return fma(a, b, c); }
-// a*b + c in 18 flops: exact product of the high parts, exact sum of the two high parts, low-order terms in binary64;
-// error <= ~2^-103 (|a b| + |c|), the same bound relative to the operands as the renormalising a*b + c
+// Pair arithmetic (no renormalisation of the result): a*b + c in 12 flops. The product of the high parts and the sum
+// of the two high parts are exact (error-free transformations); every low-order term is binary64. The pair
+// (s, lo) need not satisfy |lo| <= ulp(s)/2: after cancellation of the high parts |lo| may even exceed |s|, so
+// nothing downstream may assume an ordering (two_sum, never quick_two_sum, on values that come from here).
+// Error <= ~2^-103 (|a b| + |c|): the bound is relative to the operands, which is all a renormalising a*b + c gives
+// after a cancellation as well; the evaluator renormalises once per family (mq_norm in account()).
 __device__ __forceinline__ dd mq_fma(dd a, dd b, dd c) {
   const double p = __dmul_rn(a.hi, b.hi);
   double e = __fma_rn(a.hi, b.hi, -p);
   e = __fma_rn(a.hi, b.lo, e);
   e = __fma_rn(a.lo, b.hi, e);
   const double s = __dadd_rn(p, c.hi), v = __dadd_rn(s, -p);
-  double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c.hi, -v));
-  t = __dadd_rn(__dadd_rn(t, e), c.lo);
-  return dd_two_sum(s, t);           // not quick: after cancellation of the high parts |t| may exceed |s|
+  const double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c.hi, -v));
+  return dd(s, __dadd_rn(__dadd_rn(e, c.lo), t));
 }
 __device__ __forceinline__ double mq_fma_c(double coef, double x, double c0, double) { return fma(coef, x, c0); }   // coef*x + c0
-__device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) {   // coef*x + c0, coef and c0 binary64 (exact table entries)
+__device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) {   // coef*x + c0, coef and c0 binary64 (exact table entries); 10 flops
   const double p = __dmul_rn(coef, x.hi);
   double e = __fma_rn(coef, x.hi, -p);
   e = __fma_rn(coef, x.lo, e);
   const double s = __dadd_rn(p, c0), v = __dadd_rn(s, -p);
-  double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c0, -v));
-  t = __dadd_rn(t, e);
-  return dd_two_sum(s, t);
+  const double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c0, -v));
+  return dd(s, __dadd_rn(t, e));
 }
+// product of two pairs without renormalisation (5 flops); same remark as mq_fma
+__device__ __forceinline__ dd mq_mul(dd a, dd b) {
+  const double p = __dmul_rn(a.hi, b.hi);
+  double e = __fma_rn(a.hi, b.hi, -p);
+  e = __fma_rn(a.hi, b.lo, e);
+  e = __fma_rn(a.lo, b.hi, e);
+  return dd(p, e);
+}
+__device__ __forceinline__ double mq_mul(double a, double b) { return a * b; }
+__device__ __forceinline__ dd mq_norm(dd a) { return dd_two_sum(a.hi, a.lo); }
+__device__ __forceinline__ double mq_norm(double a) { return a; }
 __device__ __forceinline__ double mq_to_double(double a) { return a; }
 __device__ __forceinline__ double mq_to_double(dd a) { return a.hi + a.lo; }
 __device__ __forceinline__ double mq_abs(double a) { return fabs(a); }

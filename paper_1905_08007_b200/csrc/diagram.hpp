@@ -45,6 +45,37 @@ struct mc_diagram {
   size_t smem_f64 = 0, smem_dd = 0, smem_eval = 0, smem_qd = 0;
 };
 
+// the object behind mc_batch*: a set of prepared diagrams integrated together by one persistent launch per precision tier
+namespace mqk {
+struct BatchDiag {
+  const uint64_t *blob;
+  double cond_max, amin_min;
+};
+struct BatchView {
+  const BatchDiag *dg;             // [nd]
+  int nd; uint32_t cap;            // diagrams; capacity (points per diagram per call, multiple of PTS_F64)
+  uint32_t ipd;                    // binary64 items per diagram in this call
+  uint32_t *item_cnt;              // [nd*cap/PTS_F64] flagged points of a binary64 item
+  uint32_t *flag_raw;              // [nd*cap] item-local lists (relative sample indices), entry b*PTS_F64+k of diagram d
+  uint32_t *flag_list;             // [nd*cap] compacted, ascending
+  uint32_t *lost_list;             // [nd*lostcap] handed from double-double to quad-double
+  uint32_t lostcap;
+  unsigned long long *nflag, *nlost, *ndrop;   // [nd]
+  uint32_t *dd_start, *qd_start;   // [nd+1] first item of diagram d in the double-double / quad-double pass
+  double *part_f64, *part_dd, *part_qd;        // [items][4]
+  unsigned long long *queue;       // [4] heads of the three work queues
+};
+}  // namespace mqk
+struct mc_batch {
+  std::vector<const mc_diagram *> diags;
+  uint32_t cap = 0, lostcap = 0;           // points per diagram per call (multiple of PTS_F64); quad-double list capacity
+  int scal_len = 0;                        // max over the diagrams: fixes the shared-memory layout of the batch kernels
+  int grid_f64 = 0, grid_dd = 0, grid_qd = 0;
+  size_t smem_f64 = 0, smem_dd = 0, smem_qd = 0;
+  void *d_mem = nullptr;                   // one device allocation holding every array of BatchView
+  mqk::BatchView view{};                   // the kernel argument (pointers into d_mem)
+};
+
 // host preparation (host_prepare.cpp)
 // use_gpu: count the gamma-string paths of the numerator tables with the CUDA kernel of prep_kernel.cu
 int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out);
@@ -69,3 +100,12 @@ void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed
 void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st);
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st);
 int mq_fp64_peak(int iters, mq_stream st, double *flops, double *ms);
+// batched path (kern_f64.cu / kern_dd.cu / kern_qd.cu)
+size_t mq_batch_smem_f64(int scal_len); size_t mq_batch_smem_dd(int scal_len); size_t mq_batch_smem_qd(int scal_len);
+int mq_batch_config_f64(size_t smem, int *grid); int mq_batch_config_dd(size_t smem, int *grid); int mq_batch_config_qd(size_t smem, int *grid);
+void mq_launch_batch_f64(const mqk::BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd, mq_stream st);
+void mq_launch_batch_compact(const mqk::BatchView &bv, mq_stream st);
+void mq_launch_batch_ranges(const mqk::BatchView &bv, int tier, mq_stream st);
+void mq_launch_batch_dd(const mqk::BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st);
+void mq_launch_batch_qd(const mqk::BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st);
+void mq_launch_batch_finish(const mqk::BatchView &bv, int tiers, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);

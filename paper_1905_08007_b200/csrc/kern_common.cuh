@@ -13,7 +13,8 @@ struct KahanPair {   // compensated running sum (hi, lo)
 };
 
 // a7: block reduction of two compensated sums (warp shuffles, then shared memory); thread 0 writes partial[block][0..3]
-__device__ __forceinline__ void block_reduce_store(KahanPair a, KahanPair b, double *partial) {
+// dst[0..3] = (sum hi, sum lo, sumsq hi, sumsq lo) of the CTA; callers in a loop must pass a __syncthreads between calls
+__device__ __forceinline__ void block_reduce_to(KahanPair a, KahanPair b, double *dst) {
   __shared__ double red[32][4];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
@@ -27,9 +28,33 @@ __device__ __forceinline__ void block_reduce_store(KahanPair a, KahanPair b, dou
   if (threadIdx.x == 0) {
     KahanPair sa{0.0, 0.0}, sb{0.0, 0.0};
     for (int w = 0; w < nw; w++) { sa.merge(red[w][0], red[w][1]); sb.merge(red[w][2], red[w][3]); }
-    partial[blockIdx.x * 4 + 0] = sa.hi; partial[blockIdx.x * 4 + 1] = sa.lo;
-    partial[blockIdx.x * 4 + 2] = sb.hi; partial[blockIdx.x * 4 + 3] = sb.lo;
+    dst[0] = sa.hi; dst[1] = sa.lo; dst[2] = sb.hi; dst[3] = sb.lo;
   }
+}
+__device__ __forceinline__ void block_reduce_store(KahanPair a, KahanPair b, double *partial) { block_reduce_to(a, b, partial + (size_t)blockIdx.x * 4); }
+
+// Opt every evaluating kernel in to the device's maximum dynamic shared memory once: the attribute is per function, not
+// per launch, and diagrams of different size share the kernels (a smaller diagram prepared later must not lower it).
+template <class K> inline cudaError_t allow_max_smem(K kernel) {
+  cudaFuncAttributes fa; cudaError_t e;
+  if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
+  int dev = 0, optin = 0;
+  cudaGetDevice(&dev);
+  if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+}
+
+// ---- batched path (mc_batch_*): one persistent launch per precision tier serves every diagram of a batch ----
+// A work item is one CTA-load of points of ONE diagram (the evaluator is CTA-collective and its table reads are
+// CTA-uniform). CTAs take items from a global queue head, so diagrams of different cost balance themselves and the
+// only tail is the last item of the whole batch. Every item writes its own compensated partial sums; the final
+// reduction adds them in item order, so the result does not depend on which CTA ran which item.
+// (BatchDiag / BatchView: diagram.hpp)
+// item -> diagram for the passes whose item counts are known only on the device
+__device__ __forceinline__ int batch_find(const uint32_t *start, int nd, uint32_t item) {
+  int lo = 0, hi = nd;             // start[lo] <= item < start[hi]
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (start[mid] <= item) lo = mid; else hi = mid; }
+  return lo;
 }
 
 __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   // DESIGN.md A15

@@ -8,6 +8,10 @@
 
 namespace mqk {
 
+// beyond double-double (O8): pair arithmetic carries ~2^-103 relative to the operands, so a point whose
+// condition number (or pivot / current loss) exceeds this keeps fewer than ~5 digits and goes on to quad-double
+#define MQ_DD_COND_MAX 1e26
+
 // a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
 __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
                                                          const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
@@ -25,9 +29,7 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
-    // beyond double-double (O8): 106 bits keep fewer than ~6 digits beyond a condition number of 1e26 or a pivot loss of 1e26;
-    // such points are dropped (w = 0) and counted
-    const bool lost = !(mq_to_double(a) <= 1e26 * fabs(fd)) || fmin(amin, xmin) < 1e-26;
+    const bool lost = !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX;
     if (bad_point(z, v.h->M, p)) atomicAdd(&counters[1], 1ull);                  // dropped: w = 0
     else if (!isfinite(fd) || lost) {                                          // third tier: quad-double
       const unsigned long long slot = atomicAdd(&counters[2], 1ull);
@@ -36,6 +38,43 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     else { const double w = fd / p; s1.add(w); s2.add(w * w); }
   }
   block_reduce_store(s1, s2, partial);
+}
+
+// batched path, double-double tier: persistent CTAs; item = PTS_DD consecutive entries of one diagram's flagged list
+__global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ unsigned s_item; __shared__ int s_d;
+  const Roles<dd, 1> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<1>(rd, smem_raw, scal_len, sizeof(dd));
+  const uint32_t total = bv.dd_start[bv.nd];
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) { s_item = (unsigned)atomicAdd(&bv.queue[1], 1ull); s_d = s_item < total ? batch_find(bv.dd_start, bv.nd, s_item) : 0; }
+    __syncthreads();
+    const uint32_t item = s_item;
+    if (item >= total) break;
+    const int d = s_d;
+    const DiagView v = make_view(bv.dg[d].blob);
+    const unsigned long long cnt = bv.nflag[d];
+    const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + threadIdx.x; const bool live = i < cnt;
+    const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (live ? i : cnt - 1)];
+    double z[MQ_MAXM];
+    const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
+    dd f, a; double amin, xmin;
+    eval_integrand<dd, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
+    if (live) {
+      const double fd = mq_to_double(f);
+      const bool lost = !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX;     // same rule as k_integrate_dd
+      if (bad_point(z, v.h->M, p)) atomicAdd(&bv.ndrop[d], 1ull);
+      else if (!isfinite(fd) || lost) {
+        const unsigned long long slot = atomicAdd(&bv.nlost[d], 1ull);
+        if (slot < bv.lostcap) bv.lost_list[(size_t)d * bv.lostcap + slot] = rel; else atomicAdd(&bv.ndrop[d], 1ull);
+      }
+      else { const double w = fd / p; s1.add(w); s2.add(w * w); }
+    }
+    block_reduce_to(s1, s2, bv.part_dd + (size_t)item * 4);
+  }
 }
 
 __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
@@ -55,7 +94,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
     if (live) {
       const double fd = mq_to_double(f);
       f_out[rel] = fd;
-      if (!isfinite(fd) || !(mq_to_double(a) <= 1e26 * fabs(fd)) || fmin(amin, xmin) < 1e-26) {
+      if (!isfinite(fd) || !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX) {
         const unsigned long long slot = atomicAdd(&counters[2], 1ull);
         if (slot < LOSTCAP) lost_list[slot] = rel;
       }
@@ -87,9 +126,9 @@ using namespace mqk;
 int mq_config_dd(mc_diagram *d) {
   d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd), W_DD);
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_integrate_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
-  if ((e = cudaFuncSetAttribute(k_eval_points_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
-  if ((e = cudaFuncSetAttribute(k_eval_z_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_dd)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_integrate_dd)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_eval_points_dd)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_eval_z_dd)) != cudaSuccess) return (int)e;
   int nsm = 0, occ = 0, dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -106,4 +145,21 @@ void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed
 }
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st) {
   k_eval_z_dd<<<grid, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, n, z_in, fdd_out);
+}
+
+// ---- batched path launchers ----
+int mq_batch_config_dd(size_t smem, int *grid) {
+  cudaError_t e;
+  if ((e = allow_max_smem(k_batch_dd)) != cudaSuccess) return (int)e;
+  int nsm = 0, occ = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_batch_dd, TPB_DD, smem)) != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  *grid = nsm * occ;
+  return 0;
+}
+size_t mq_batch_smem_dd(int scal_len) { return smem_bytes(scal_len, TPB_DD, sizeof(dd), 1); }
+void mq_launch_batch_dd(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st) {
+  k_batch_dd<<<grid, TPB_DD, smem, (cudaStream_t)st>>>(bv, first, seed, scal_len);
 }

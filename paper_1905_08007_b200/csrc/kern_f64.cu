@@ -102,6 +102,103 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
   }
 }
 
+// ------------------------------------------------------------------ batched path, binary64 tier (a1-a7 for every diagram of a batch)
+// Persistent CTAs; item = PTS_F64 consecutive sample indices of one diagram, taken from queue[0].
+// Flagged points are compacted inside the item in thread order (ballot + prefix): deterministic lists.
+__global__ void __launch_bounds__(TPB_F64, 4) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ unsigned s_item, s_wcnt[TPB_F64 / 32];
+  const Roles<double, 1> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<1>(rd, smem_raw, scal_len, sizeof(double));
+  const uint32_t total = (uint32_t)bv.nd * bv.ipd;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_item = (unsigned)atomicAdd(&bv.queue[0], 1ull);
+    __syncthreads();
+    const uint32_t item = s_item;
+    if (item >= total) break;
+    const int d = (int)(item / bv.ipd); const uint32_t b = item % bv.ipd;
+    const DiagView v = make_view(bv.dg[d].blob);
+    const double cond_max = no_dd ? INFINITY : bv.dg[d].cond_max, amin_min = no_dd ? -1.0 : bv.dg[d].amin_min;
+    const uint64_t i = (uint64_t)b * PTS_F64 + threadIdx.x; const bool live = i < n;
+    double z[MQ_MAXM];
+    const double p = draw_point<false>(v, first + (live ? i : n - 1), seed, z, nullptr);
+    double f, a, amin, xmin;
+    eval_integrand<double, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    const bool flag = live && (bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min);
+    const unsigned bal = __ballot_sync(0xffffffffu, flag);
+    if (lane == 0) s_wcnt[warp] = __popc(bal);
+    __syncthreads();
+    unsigned before = 0, all = 0;
+#pragma unroll
+    for (int w = 0; w < TPB_F64 / 32; w++) { if (w < warp) before += s_wcnt[w]; all += s_wcnt[w]; }
+    if (flag) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + before + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)i;
+    if (threadIdx.x == 0) bv.item_cnt[(size_t)d * (bv.cap / PTS_F64) + b] = all;
+    KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
+    if (live && !flag) { const double w = f / p; s1.add(w); s2.add(w * w); }
+    block_reduce_to(s1, s2, bv.part_f64 + (size_t)item * 4);
+  }
+}
+
+// one CTA per diagram: concatenates the item-local flagged lists in item order (ascending sample index)
+__global__ void __launch_bounds__(128) k_batch_compact(BatchView bv) {
+  __shared__ unsigned sc[128];
+  __shared__ unsigned s_base;
+  const int d = blockIdx.x, t = threadIdx.x;
+  const uint32_t *cnt = bv.item_cnt + (size_t)d * (bv.cap / PTS_F64);
+  const uint32_t *raw = bv.flag_raw + (size_t)d * bv.cap;
+  uint32_t *out = bv.flag_list + (size_t)d * bv.cap;
+  if (t == 0) s_base = 0;
+  __syncthreads();
+  for (uint32_t b0 = 0; b0 < bv.ipd; b0 += 128) {
+    const uint32_t b = b0 + t;
+    const unsigned c = b < bv.ipd ? cnt[b] : 0u;
+    sc[t] = c;
+    __syncthreads();
+    for (int off = 1; off < 128; off <<= 1) {        // inclusive scan
+      const unsigned x = t >= off ? sc[t - off] : 0u;
+      __syncthreads();
+      sc[t] += x;
+      __syncthreads();
+    }
+    const unsigned o = s_base + sc[t] - c;
+    for (unsigned k = 0; k < c; k++) out[o + k] = raw[(size_t)b * PTS_F64 + k];
+    __syncthreads();
+    if (t == 127) s_base += sc[127];
+    __syncthreads();
+  }
+  if (t == 0) bv.nflag[d] = s_base;
+}
+// item ranges of the next tier: start[d] = sum_{d'<d} ceil(count[d'] / per); resets that tier's queue head
+__global__ void k_batch_ranges(const unsigned long long *count, unsigned long long limit, int nd, unsigned per, uint32_t *start, unsigned long long *queue_head) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  uint32_t acc = 0;
+  for (int d = 0; d < nd; d++) { start[d] = acc; const unsigned long long c = count[d] < limit ? count[d] : limit; acc += (uint32_t)((c + per - 1) / per); }
+  start[nd] = acc;
+  *queue_head = 0ull;
+}
+// one thread per diagram: adds the per-item partial sums of the three tiers in item order; out += result
+__global__ void k_batch_finish(BatchView bv, int tiers, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop) {
+  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+  if (d == 0) bv.queue[0] = 0ull;
+  if (d >= bv.nd) return;
+  KahanPair a{0.0, 0.0}, b{0.0, 0.0};
+  const double *p = bv.part_f64 + (size_t)d * bv.ipd * 4;
+  for (uint32_t i = 0; i < bv.ipd; i++) { a.merge(p[i * 4], p[i * 4 + 1]); b.merge(p[i * 4 + 2], p[i * 4 + 3]); }
+  unsigned long long ndrop = bv.ndrop[d];
+  if (tiers > 1)
+    for (uint32_t i = bv.dd_start[d]; i < bv.dd_start[d + 1]; i++) { const double *q = bv.part_dd + (size_t)i * 4; a.merge(q[0], q[1]); b.merge(q[2], q[3]); }
+  if (tiers > 2)
+    for (uint32_t i = bv.qd_start[d]; i < bv.qd_start[d + 1]; i++) { const double *q = bv.part_qd + (size_t)i * 4; a.merge(q[0], q[1]); b.merge(q[2], q[3]); }
+  else if (tiers == 2) ndrop += bv.nlost[d] < bv.lostcap ? bv.nlost[d] : bv.lostcap;   // quad-double pass skipped: its points count as dropped
+  if (out_sum) out_sum[d] += a.hi + a.lo;
+  if (out_sumsq) out_sumsq[d] += b.hi + b.lo;
+  if (out_nflag) out_nflag[d] += bv.nflag[d];
+  if (out_ndrop) out_ndrop[d] += ndrop;
+  bv.nflag[d] = 0; bv.nlost[d] = 0; bv.ndrop[d] = 0;
+}
+
 // FP64 FMA peak: 8 independent chains per thread
 __global__ void k_fp64_peak(int iters, double *sink) {
   double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3, a4 = a0 + 4e-3, a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
@@ -124,9 +221,9 @@ int mq_config_f64(mc_diagram *d) {
   d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double), W_F64);
   d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double), W_F64);
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_integrate_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_f64)) != cudaSuccess) return (int)e;
-  if ((e = cudaFuncSetAttribute(k_eval_points, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;
-  if ((e = cudaFuncSetAttribute(k_eval_z_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->smem_eval)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_integrate_f64)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_eval_points)) != cudaSuccess) return (int)e;
+  if ((e = allow_max_smem(k_eval_z_f64)) != cudaSuccess) return (int)e;
   int nsm = 0, occ = 0, dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -169,4 +266,29 @@ int mq_fp64_peak(int iters, mq_stream stream, double *flops, double *ms) {
   if (flops) *flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)blocks * tpb / (t * 1e-3);
   cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
   return (int)e;
+}
+
+// ---- batched path launchers ----
+int mq_batch_config_f64(size_t smem, int *grid) {
+  cudaError_t e;
+  if ((e = allow_max_smem(k_batch_f64)) != cudaSuccess) return (int)e;
+  int nsm = 0, occ = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_batch_f64, TPB_F64, smem)) != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  *grid = nsm * occ;
+  return 0;
+}
+size_t mq_batch_smem_f64(int scal_len) { return smem_bytes(scal_len, TPB_F64, sizeof(double), 1); }
+void mq_launch_batch_f64(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd, mq_stream st) {
+  k_batch_f64<<<grid, TPB_F64, smem, (cudaStream_t)st>>>(bv, first, n, seed, scal_len, no_dd);
+}
+void mq_launch_batch_compact(const BatchView &bv, mq_stream st) { k_batch_compact<<<bv.nd, 128, 0, (cudaStream_t)st>>>(bv); }
+void mq_launch_batch_ranges(const BatchView &bv, int tier, mq_stream st) {
+  if (tier == 1) k_batch_ranges<<<1, 1, 0, (cudaStream_t)st>>>(bv.nflag, ~0ull, bv.nd, (unsigned)PTS_DD, bv.dd_start, bv.queue + 1);
+  else k_batch_ranges<<<1, 1, 0, (cudaStream_t)st>>>(bv.nlost, (unsigned long long)bv.lostcap, bv.nd, 32u, bv.qd_start, bv.queue + 2);
+}
+void mq_launch_batch_finish(const BatchView &bv, int tiers, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
+  k_batch_finish<<<(bv.nd + 127) / 128, 128, 0, (cudaStream_t)st>>>(bv, tiers, out_sum, out_sumsq, out_nflag, out_ndrop);
 }

@@ -201,6 +201,103 @@ int mc_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda
   return MC_OK;
 }
 
+// ---- batched path ----
+int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint64_t max_samples_per_call, mc_batch **out) {
+  if (!diagrams || n_diagrams < 1 || !out || max_samples_per_call < 1 || max_samples_per_call > (1ull << 30)) return MC_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MC_ECUDA;
+  mc_batch *b = new (std::nothrow) mc_batch;
+  if (!b) return MC_ENOMEM;
+  for (int i = 0; i < n_diagrams; i++) {
+    if (!diagrams[i] || !diagrams[i]->on_device) { delete b; return MC_EINVAL; }
+    b->diags.push_back(diagrams[i]);
+    b->scal_len = std::max(b->scal_len, diagrams[i]->max_scal_len);
+  }
+  const size_t P = mqk::PTS_F64, nd = (size_t)n_diagrams;
+  b->cap = (uint32_t)((max_samples_per_call + P - 1) / P * P);
+  b->lostcap = std::max<uint32_t>(1024u, b->cap / 8);
+  const size_t ipd = b->cap / P, idd = (size_t)b->cap / mqk::PTS_DD + 1, iqd = (size_t)b->lostcap / 32 + 1;
+  // carve one allocation (every array 256-byte aligned)
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+  const size_t o_dg = take(nd * sizeof(mqk::BatchDiag)), o_cnt = take(nd * ipd * 4), o_raw = take(nd * b->cap * 4), o_list = take(nd * b->cap * 4),
+               o_lost = take(nd * b->lostcap * 4), o_nf = take(nd * 8), o_nl = take(nd * 8), o_ndp = take(nd * 8), o_dds = take((nd + 1) * 4),
+               o_qds = take((nd + 1) * 4), o_p1 = take(nd * ipd * 32), o_p2 = take(nd * idd * 32), o_p3 = take(nd * iqd * 32), o_q = take(32);
+  if (cudaMalloc(&b->d_mem, off) != cudaSuccess) { delete b; return MC_ENOMEM; }
+  if (cudaMemset(b->d_mem, 0, off) != cudaSuccess) { mc_batch_free(b); return MC_ECUDA; }
+  char *base = (char *)b->d_mem;
+  std::vector<mqk::BatchDiag> dg(nd);
+  for (size_t i = 0; i < nd; i++) { dg[i].blob = diagrams[i]->d_blob; dg[i].cond_max = diagrams[i]->opt.cond_max; dg[i].amin_min = diagrams[i]->opt.amin_min; }
+  if (cudaMemcpy(base + o_dg, dg.data(), nd * sizeof(mqk::BatchDiag), cudaMemcpyHostToDevice) != cudaSuccess) { mc_batch_free(b); return MC_ECUDA; }
+  mqk::BatchView &v = b->view;
+  v.dg = (const mqk::BatchDiag *)(base + o_dg); v.nd = n_diagrams; v.cap = b->cap; v.ipd = 0;
+  v.item_cnt = (uint32_t *)(base + o_cnt); v.flag_raw = (uint32_t *)(base + o_raw); v.flag_list = (uint32_t *)(base + o_list);
+  v.lost_list = (uint32_t *)(base + o_lost); v.lostcap = b->lostcap;
+  v.nflag = (unsigned long long *)(base + o_nf); v.nlost = (unsigned long long *)(base + o_nl); v.ndrop = (unsigned long long *)(base + o_ndp);
+  v.dd_start = (uint32_t *)(base + o_dds); v.qd_start = (uint32_t *)(base + o_qds);
+  v.part_f64 = (double *)(base + o_p1); v.part_dd = (double *)(base + o_p2); v.part_qd = (double *)(base + o_p3);
+  v.queue = (unsigned long long *)(base + o_q);
+  b->smem_f64 = mq_batch_smem_f64(b->scal_len); b->smem_dd = mq_batch_smem_dd(b->scal_len); b->smem_qd = mq_batch_smem_qd(b->scal_len);
+  if (mq_batch_config_f64(b->smem_f64, &b->grid_f64) != 0 || mq_batch_config_dd(b->smem_dd, &b->grid_dd) != 0 || mq_batch_config_qd(b->smem_qd, &b->grid_qd) != 0) {
+    mc_batch_free(b); return MC_ECUDA;
+  }
+  *out = b;
+  return MC_OK;
+}
+void mc_batch_free(mc_batch *b) {
+  if (!b) return;
+  if (b->d_mem) cudaFree(b->d_mem);
+  delete b;
+}
+int mc_batch_integrate(mc_batch *b, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
+                       double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
+  if (!b) return MC_EINVAL;
+  mq_stream st = (mq_stream)cuda_stream;
+  const bool no_dd = flags & 1u, no_qd = flags & 2u;
+  for (uint64_t done = 0; done < n_samples; done += b->cap) {
+    const uint64_t n = std::min<uint64_t>(b->cap, n_samples - done);
+    mqk::BatchView v = b->view;
+    v.ipd = (uint32_t)((n + mqk::PTS_F64 - 1) / mqk::PTS_F64);
+    const uint64_t items = (uint64_t)v.ipd * v.nd;
+    mq_launch_batch_f64(v, (int)std::min<uint64_t>((uint64_t)b->grid_f64, items), b->smem_f64, first_sample + done, n, seed, b->scal_len, no_dd ? 1 : 0, st);
+    mq_launch_batch_compact(v, st);
+    g_launches += 2;
+    if (!no_dd) {
+      mq_launch_batch_ranges(v, 1, st);
+      mq_launch_batch_dd(v, b->grid_dd, b->smem_dd, first_sample + done, seed, b->scal_len, st);
+      g_launches += 2;
+      if (!no_qd) {
+        mq_launch_batch_ranges(v, 2, st);
+        mq_launch_batch_qd(v, b->grid_qd, b->smem_qd, first_sample + done, seed, b->scal_len, st);
+        g_launches += 2;
+      }
+    }
+    mq_launch_batch_finish(v, no_dd ? 1 : no_qd ? 2 : 3, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
+    g_launches++;
+  }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+int mc_batch_integrate_host(mc_batch *b, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
+                            double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped) {
+  if (!b) return MC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nd = b->diags.size();
+  char *dev = nullptr;
+  MQ_CK(cudaMallocAsync((void **)&dev, nd * 32, st));
+  MQ_CK(cudaMemsetAsync(dev, 0, nd * 32, st));
+  double *ds = (double *)dev, *ds2 = ds + nd; unsigned long long *dnf = (unsigned long long *)(ds2 + nd), *dnd = dnf + nd;
+  int rc = mc_batch_integrate(b, first_sample, n_samples, seed, flags, cuda_stream, ds, ds2, dnf, dnd);
+  if (rc != MC_OK) { cudaFreeAsync(dev, st); return rc; }
+  if (sum) MQ_CK(cudaMemcpyAsync(sum, ds, nd * 8, cudaMemcpyDeviceToHost, st));
+  if (sumsq) MQ_CK(cudaMemcpyAsync(sumsq, ds2, nd * 8, cudaMemcpyDeviceToHost, st));
+  if (n_flagged) MQ_CK(cudaMemcpyAsync(n_flagged, dnf, nd * 8, cudaMemcpyDeviceToHost, st));
+  if (n_dropped) MQ_CK(cudaMemcpyAsync(n_dropped, dnd, nd * 8, cudaMemcpyDeviceToHost, st));
+  MQ_CK(cudaFreeAsync(dev, st));
+  MQ_CK(cudaStreamSynchronize(st));
+  return MC_OK;
+}
+
 unsigned long long mc_kernel_launch_count(void) { return g_launches.load(); }
 
 int mc_fp64_peak(int iters, void *cuda_stream, double *flops, double *ms) {

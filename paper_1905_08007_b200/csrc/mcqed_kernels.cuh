@@ -211,7 +211,7 @@ template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> stru
     if constexpr (S < N2) {
       if constexpr (!((USED >> S) & 1u)) {
         if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], s_coef, r, sum);
-        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, w * b[pair_index<N2>(F, S)], s_coef, r, sum);
+        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, mq_mul(w, b[pair_index<N2>(F, S)]), s_coef, r, sum);
       }
       PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, s_coef, r, sum);
     }
@@ -221,7 +221,7 @@ template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
   static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum) {
     if constexpr (USED == ((1u << N2) - 1u)) {
       T h = horner<T, KD>(s_coef, r);
-      if constexpr (FIRST) sum = sum + h; else sum = mq_fma(w, h, sum);
+      if constexpr (FIRST) sum = h; else sum = mq_fma(w, h, sum);   // FIRST at a leaf: no pairs, one block
     } else {
       constexpr int F = ctz_c(~USED);
       PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, s_coef, r, sum);
@@ -493,6 +493,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
         }
         const int nb = c * (2 * c - 1) + kd;
         auto account = [&](T val, uint32_t ea, int ns, int keyk) {
+          val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
           for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(ea + 8 + nb + i) * sstride);
           if (keyk != key) {
             if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }

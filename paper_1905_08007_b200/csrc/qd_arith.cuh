@@ -85,6 +85,8 @@ __device__ __forceinline__ qd &operator+=(qd &a, qd b) { a = a + b; return a; }
 
 __device__ __forceinline__ qd mq_fma(qd a, qd b, qd c) { return a * b + c; }
 __device__ __forceinline__ qd mq_fma_c(double coef, qd x, double c0, qd) { return x * qd(coef) + qd(c0); }
+__device__ __forceinline__ qd mq_mul(qd a, qd b) { return a * b; }
+__device__ __forceinline__ qd mq_norm(qd a) { return a; }
 __device__ __forceinline__ double mq_to_double(qd a) { return __dadd_rn(__dadd_rn(a.x[0], a.x[1]), __dadd_rn(a.x[2], a.x[3])); }
 __device__ __forceinline__ qd mq_abs(qd a) { return a.x[0] < 0 ? -a : a; }
 __device__ __forceinline__ bool mq_lt0(qd a) { return a.x[0] < 0; }

@@ -221,3 +221,45 @@ def test_quad_double_tier_against_exact_rational_values(po, mc):
         fe = float(b.integrand([Fr(float(v)) for v in z[k]]))
         assert abs(fq[k] - fe) <= 4e-16 * abs(fe), (k, c[k], fq[k], fe, fd[k])
     d.close()
+
+
+def test_batched_path_equals_per_diagram_path(po, mc):
+    """mc_batch_integrate (one persistent launch per precision tier for the whole set) against mc_integrate per diagram:
+    same flagged counts exactly, same sums up to the order of the compensated additions; ragged sizes, a call longer than
+    max_samples_per_call (split), accumulation over two calls, and run-to-run bit-determinism."""
+    st = torch.cuda.current_stream().cuda_stream
+    graphs = [(2, i) for i in range(6)] + [(3, i) for i in (0, 7, 8, 29)] + [(1, 0)]
+    ds = []
+    for L, i in graphs:
+        g = po.graph_get(L, i)
+        ds.append(mc.Diagram(L, g.ext_pos, g.chords()))
+    n, seed, first = 5000 + 77, 11, (1 << 33) + 5
+    b = mc.Batch(ds, 2048)                       # cap 2048 < n: three passes, the last one ragged (981 = 7*128 + 85 points)
+    G = len(ds)
+    out = torch.zeros(2, G, dtype=torch.float64, device="cuda")
+    cnt = torch.zeros(2, G, dtype=torch.int64, device="cuda")
+    n1 = 1234
+    b.integrate(first, n1, seed, st, out[0], out[1], cnt[0], cnt[1])
+    b.integrate(first + n1, n - n1, seed, st, out[0], out[1], cnt[0], cnt[1])
+    torch.cuda.synchronize()
+    s, c = out.cpu().numpy(), cnt.cpu().numpy()
+    h = b.integrate_host(first, n, seed, st)
+    h2 = b.integrate_host(first, n, seed, st)
+    assert np.array_equal(h[0], h2[0]) and np.array_equal(h[1], h2[1]) and np.array_equal(h[2], h2[2])
+    for k, d in enumerate(ds):
+        r1, r2, nf, nd = d.integrate_host(first, n, seed, st)
+        assert nf == c[0, k] == h[2][k] and nd == c[1, k] == 0
+        scale = math.sqrt(n * r2)
+        assert abs(s[0, k] - r1) <= 1e-12 * scale and abs(h[0][k] - r1) <= 1e-12 * scale
+        assert abs(s[1, k] - r2) <= 1e-12 * r2 and abs(h[1][k] - r2) <= 1e-12 * r2
+    # binary64 tier alone (flags bit 0): flagged points contribute nothing, nothing is counted as flagged
+    hb = b.integrate_host(first, n, seed, st, flags=1)
+    r = _gpu_points(mc, ds[1], first, n, seed)
+    w = (r["f64"] / r["p"])[np.isfinite(r["f64"])]
+    assert abs(hb[0][1] - math.fsum(w)) <= 1e-12 * math.fsum(np.abs(w))
+    # empty call
+    z = b.integrate_host(0, 0, seed, st)
+    assert not z[0].any() and not z[2].any()
+    b.close()
+    for d in ds:
+        d.close()
