@@ -18,7 +18,8 @@
 // inner dense binary dimensions of a family, by number of Wick pairs c (bounds the static code and the family size)
 static inline int mq_kd_max(int c) { return c <= 3 ? 4 : 2; }   // keeps every family below one chunk;   // larger inner blocks (5, 6) were measured slower (register spills)
 #define MQ_MAXSCAL 12
-#define MQ_CHUNK_WORDS 512    // staging granule of the family stream (4 KiB): small, so that three CTAs fit an SM
+#define MQ_CHUNK_WORDS 1024   // staging granule of the family stream (8 KiB): the largest entry (MQ_WL families of c = 4, kd = 2) must fit
+#define MQ_WL 2               // families per stream entry = lanes that share one sample point in the binary64 / double-double kernels
 #define MQ_PAD_MARK 7        // header field c of a PAD entry
 
 enum { MQ_OP_A = 0, MQ_OP_U = 1, MQ_OP_L = 2, MQ_OP_LMU = 3 };
@@ -48,7 +49,7 @@ struct DevGeom {
 };
 
 struct DevTable {
-  int32_t geom, op, nout, nfam;
+  int32_t geom, op, nout, nfam;           // nfam = stream ENTRIES of this table (each holds MQ_WL families)
   int32_t first_node, nnode;              // nodes using this table are consecutive
   int64_t stream_off, stream_words;       // in 8-byte words from the blob start
   int64_t n_monomials;                    // stored (dense) numerator coefficients
@@ -71,17 +72,25 @@ struct DevHeader {
   int64_t off_stream, stream_chunks;      // the family streams: stream_chunks chunks of MQ_CHUNK_WORDS words
 };
 
-// Family header word (uint64), then index bytes, padded to 8 bytes, then the dense coefficients:
-//   bits  0..2  c   (#Wick pairs; 7 = PAD entry: skip 1+idx_words words, no coefficients)              bits  3..5  kd (#inner binary slots)
+// Stream entry = MQ_WL families of the SAME shape (c, kd), evaluated side by side by the MQ_WL lanes that share a
+// sample point (each lane runs the same static code on its own family; a table with an odd number of families of a
+// shape gets a VOID member: zero coefficients). Layout in 8-byte words:
+//   hd[MQ_WL] | idx[MQ_WL][idx_words] | coefficients, interleaved
+// Family header word hd[s] (uint64):
+//   bits  0..2  c   (#Wick pairs; 7 = PAD entry: ONE word, skip 1+idx_words words, no coefficients)      bits  3..5  kd (#inner binary slots)
 //   bits  6..9  pattern (compressed)           bits 10..13 nscal (#extra scalar factors)
-//   bits 14     out (0/1: which output of an S-type piece)
-//   bits 16..31 number of 8-byte words of index bytes that follow
-//   bits 32..63 number of coefficient doubles that follow the index bytes
-// index bytes: 2c paired slot ids | kd inner binary slot ids | nscal x (kind<<4 | slot)
-// coefficients: for every pairing (canonical order) 2^kd values, stored as (lo,hi) pairs for the
-// first Horner level: c[j], c[j+2^(kd-1)], j < 2^(kd-1)   (kd = 0: one value per pairing).
-static inline uint64_t mq_pack_family(int c, int kd, int pattern, int nscal, int out, int idx_words, uint32_t ncoef) {
-  return (uint64_t)c | (uint64_t)kd << 3 | (uint64_t)pattern << 6 | (uint64_t)nscal << 10 | (uint64_t)out << 14 |
+//   bits 14     out (0/1: which output of an S-type piece)                  bit 15  VOID member
+//   bits 16..31 idx_words: 8-byte words of index bytes PER MEMBER
+//   bits 32..63 number of coefficient doubles of the WHOLE entry (MQ_WL x per family)
+//   (c, kd, idx_words and the coefficient count are the same in all MQ_WL header words)
+// index bytes of member s: C(2c,2) beta~ indices of its paired slots (pair (i<j) at i*2c - i(i+1)/2 + j-i-1) | kd inner
+//   binary slot ids | nscal scalar-factor indices; all are direct indices into the per-point scalar array S
+// coefficients: for every pairing (canonical order) 2^kd values per member. kd >= 1: stored as 16-byte units
+//   (c[j], c[j+2^(kd-1)]), j < 2^(kd-1) (the first Horner level); unit j of pairing q of member s sits at unit index
+//   (q*2^(kd-1) + j)*MQ_WL + s. kd = 0: one double per pairing, at double index q*MQ_WL + s.
+//   The lanes of a warp therefore read MQ_WL adjacent units with one shared-memory wavefront.
+static inline uint64_t mq_pack_family(int c, int kd, int pattern, int nscal, int out, int idx_words, uint32_t ncoef, int is_void = 0) {
+  return (uint64_t)c | (uint64_t)kd << 3 | (uint64_t)pattern << 6 | (uint64_t)nscal << 10 | (uint64_t)out << 14 | (uint64_t)is_void << 15 |
          (uint64_t)idx_words << 16 | (uint64_t)ncoef << 32;
 }
 

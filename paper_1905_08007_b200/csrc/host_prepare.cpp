@@ -171,59 +171,83 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   H.off_table = off; off += words(sizeof(DevTable) * d->tables.size());
   H.off_node = off; off += words(sizeof(DevNode) * d->nodes.size());
   H.off_term = off; off += words(sizeof(DevTerm) * d->terms.size());
-  // streams: every family = header word | index bytes (padded) | coefficients. The kernels stage the stream through
+  // streams: a sequence of entries of MQ_WL same-shape families (device_layout.h). The kernels stage the stream through
   // shared memory in chunks of MQ_CHUNK_WORDS (bulk async copies), so (i) the stream starts on a 16-byte boundary,
-  // (ii) no family straddles a chunk boundary (a PAD header, c = 7, fills the rest of a chunk), (iii) coefficients
+  // (ii) no entry straddles a chunk boundary (a PAD header, c = 7, fills the rest of a chunk), (iii) coefficients
   // start on a 16-byte boundary (read as double2), (iv) the stream is consumed strictly in order: tables are laid
-  // out in the order the evaluator visits them, families of a table sorted by (output, pattern, grade).
+  // out in the order the evaluator visits them.
   if (off & 1) off++;
   std::vector<uint64_t> streams;
   const int64_t stream_base = off;
   for (size_t ti = 0; ti < d->tables.size(); ti++) {
     DevTable &T = d->tables[ti]; const mq::TableBuild &tb = builds[ti];
-    T.stream_off = stream_base + (int64_t)streams.size(); T.nfam = (int)tb.fams.size(); T.n_monomials = tb.n_stored;
+    T.stream_off = stream_base + (int64_t)streams.size(); T.n_monomials = tb.n_stored;
     const int ns = d->geoms[T.geom].nslot;
     const DevGeom &GG = d->geoms[T.geom];
     auto tri = [&](int a, int b) { if (a > b) std::swap(a, b); return GG.off_bt + a * ns - a * (a + 1) / 2 + (b - a - 1); };
     std::vector<const mq::Family *> order;
     for (auto &f : tb.fams) order.push_back(&f);
+    // shape-major, so that MQ_WL consecutive families share their static code; inside a shape by (output, pattern): the
+    // evaluator accumulates a run of equal (output, pattern, grade) in registers
     std::stable_sort(order.begin(), order.end(), [](const mq::Family *a, const mq::Family *b) {
+      if (a->c != b->c) return a->c < b->c;
+      if (a->kd != b->kd) return a->kd < b->kd;
       if (a->out != b->out) return a->out < b->out;
-      if (a->pattern != b->pattern) return a->pattern < b->pattern;
-      return a->c < b->c;
+      return a->pattern < b->pattern;
     });
-    for (const mq::Family *fp : order) {
-      const mq::Family &f = *fp;
-      std::vector<uint8_t> idx;
+    auto index_bytes = [&](const mq::Family &f, std::vector<uint8_t> &idx) -> bool {
+      idx.clear();
       const int n2 = 2 * f.c;
       for (int i = 0; i < n2; i++) for (int j = i + 1; j < n2; j++) idx.push_back((uint8_t)tri(f.paired[i], f.paired[j]));
       for (uint8_t sl : f.inner) idx.push_back(sl);                            // r_t lives at S[t]
       for (uint8_t sc : f.scal) {
         const int kind = sc >> 4, slot = sc & 15;
         const int base = kind == MQ_SC_R ? 0 : kind == MQ_SC_AT ? GG.off_at : GG.off_aq;
-        if (base < 0) return MC_ELIMIT;                                          // a table references a scalar its piece does not carry
+        if (base < 0) return false;                                            // a table references a scalar its piece does not carry
         idx.push_back((uint8_t)(base + slot));
       }
-      int idxw = (int)words(idx.size());
-      if (idxw == 0) idxw = 1;                                                 // the kernel always reads one index word
-      int64_t in_chunk = (int64_t)streams.size() % MQ_CHUNK_WORDS;
-      if ((in_chunk + 1 + idxw) & 1) idxw++;
-      const int64_t need = 1 + idxw + (int64_t)f.coef.size();
+      return true;
+    };
+    int nentries = 0;
+    for (size_t at0 = 0; at0 < order.size();) {
+      const mq::Family &f0 = *order[at0];
+      int nm = 1;                                                              // members of this entry (same shape), the rest is VOID
+      while (nm < MQ_WL && at0 + nm < order.size() && order[at0 + nm]->c == f0.c && order[at0 + nm]->kd == f0.kd) nm++;
+      std::vector<uint8_t> idx[MQ_WL];
+      int idxw = 1;                                                            // the kernel always reads two index words per member
+      for (int m = 0; m < MQ_WL; m++) {
+        if (!index_bytes(m < nm ? *order[at0 + m] : f0, idx[m])) return MC_ELIMIT;
+        if (m >= nm) idx[m].resize((size_t)(f0.c * (2 * f0.c - 1) + f0.kd));   // VOID member: no scalar factors
+        idxw = std::max(idxw, (int)words(idx[m].size()));
+      }
+      const size_t ncf = f0.coef.size();
+      const int64_t need = MQ_WL + (int64_t)MQ_WL * idxw + (int64_t)MQ_WL * (int64_t)ncf;    // even: coefficients stay 16-byte aligned
       if (need > MQ_CHUNK_WORDS) return MC_ELIMIT;
+      const int64_t in_chunk = (int64_t)streams.size() % MQ_CHUNK_WORDS;
       if (in_chunk + need > MQ_CHUNK_WORDS) {                                  // PAD to the chunk boundary
         const int64_t rest = MQ_CHUNK_WORDS - in_chunk;
         streams.push_back(mq_pack_family(7, 0, 0, 0, 0, (int)(rest - 1), 0u));
         streams.resize(streams.size() + (size_t)(rest - 1), 0ull);
-        in_chunk = 0;
-        idxw = std::max<int>(1, (int)words(idx.size()));
-        if ((1 + idxw) & 1) idxw++;
       }
-      streams.push_back(mq_pack_family(f.c, f.kd, f.pattern, (int)f.scal.size(), f.out, idxw, (uint32_t)f.coef.size()));
-      const size_t at = streams.size();
-      streams.resize(at + idxw + f.coef.size(), 0ull);
-      std::memcpy(streams.data() + at, idx.data(), idx.size());
-      std::memcpy(streams.data() + at + idxw, f.coef.data(), sizeof(double) * f.coef.size());
+      for (int m = 0; m < MQ_WL; m++) {
+        const mq::Family &f = m < nm ? *order[at0 + m] : f0;
+        if (f.coef.size() != ncf) return MC_ELIMIT;
+        streams.push_back(mq_pack_family(f.c, f.kd, f.pattern, m < nm ? (int)f.scal.size() : 0, f.out, idxw, (uint32_t)(MQ_WL * ncf), m < nm ? 0 : 1));
+      }
+      for (int m = 0; m < MQ_WL; m++) {
+        const size_t at = streams.size();
+        streams.resize(at + idxw, 0ull);
+        std::memcpy(streams.data() + at, idx[m].data(), idx[m].size());
+      }
+      const size_t unit = f0.kd >= 1 ? 2 : 1, nunit = ncf / unit, at = streams.size();
+      streams.resize(at + MQ_WL * ncf, 0ull);
+      for (int m = 0; m < nm; m++) {
+        const double *src = order[at0 + m]->coef.data();
+        for (size_t u = 0; u < nunit; u++) std::memcpy(streams.data() + at + (u * MQ_WL + m) * unit, src + u * unit, sizeof(double) * unit);
+      }
+      at0 += nm; nentries++;
     }
+    T.nfam = nentries;
     T.stream_words = stream_base + (int64_t)streams.size() - T.stream_off;
     d->n_stored += tb.n_stored; d->n_nonzero += tb.n_nonzero;
   }

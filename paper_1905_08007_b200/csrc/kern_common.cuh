@@ -63,31 +63,36 @@ __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   
   return bad;
 }
 
-// Thread roles (mcqed_kernels.cuh "warp split"): a CTA of `threads` threads holds P = threads / W points; warp w
-// works for point group w / W in role gw = w % W. Dynamic shared memory of every evaluating kernel:
+// Thread roles (mcqed_kernels.cuh "lane split" / "warp split"): WLX lanes of a warp share one sample point (WLX = MQ_WL in
+// the binary64 and double-double kernels, 1 in quad-double) and W warps share one group of 32 / WLX points, so a CTA of
+// `threads` threads holds P = threads / (W * WLX) points; warp w works for point group w / W in role gw = w % W, lane l
+// for point l % (32 / WLX) of the group in role sub = l / (32 / WLX) (a quarter warp reads consecutive points: no
+// shared-memory bank conflicts). Dynamic shared memory of every evaluating kernel:
 //   [ S: scal_len x P x elem | xT: (W-1) x NGRADE x P x elem | xA: (W-1) x NGRADE x P x 8 | pad to 128 | 2 stream chunks | 2 mbarriers | slack ]
-__host__ __device__ inline size_t smem_head_bytes(int scal_len, int threads, size_t elem, int W) {
-  const size_t P = (size_t)threads / W;
+__host__ __device__ inline size_t smem_head_bytes(int scal_len, int threads, size_t elem, int W, int WLX) {
+  const size_t P = (size_t)threads / (W * WLX);
   size_t s = (size_t)scal_len * P * elem + (size_t)(W - 1) * MQ_NGRADE * P * (elem + 8);
   return (s + 127) & ~(size_t)127;
 }
-__host__ __device__ inline size_t smem_bytes(int scal_len, int threads, size_t elem, int W) {
-  return smem_head_bytes(scal_len, threads, elem, W) + 2 * MQ_CHUNK_WORDS * 8 + 16 + 32;   // + slack: the header prefetch may read 24 bytes past a chunk
+__host__ __device__ inline size_t smem_bytes(int scal_len, int threads, size_t elem, int W, int WLX) {
+  return smem_head_bytes(scal_len, threads, elem, W, WLX) + 2 * MQ_CHUNK_WORDS * 8 + 16 + 64;   // + slack: the header prefetch may read 8*MQ_WL + 24 bytes past a chunk
 }
-template <class T, int W> struct Roles {
-  int gw, slot, P;          // role of this warp in its group, point slot of this lane in the CTA, points per CTA
+template <class T, int W, int WLX> struct Roles {
+  int gw, sub, slot, P;     // role of this warp in its group, role of this lane for its point, point slot of this lane in the CTA, points per CTA
   T *S, *xT; double *xA;
   __device__ __forceinline__ Roles(unsigned char *smem, int scal_len) {
-    const int w = threadIdx.x >> 5;
-    gw = w % W; P = blockDim.x / W; slot = (w / W) * 32 + (threadIdx.x & 31);
+    constexpr int PPW = 32 / WLX;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    gw = w % W; sub = l / PPW; P = blockDim.x / (W * WLX); slot = (w / W) * PPW + l % PPW;
     S = reinterpret_cast<T *>(smem) + slot;
     xT = reinterpret_cast<T *>(smem) + (size_t)scal_len * P + slot;
     xA = reinterpret_cast<double *>(smem + ((size_t)scal_len * P + (size_t)(W - 1) * MQ_NGRADE * P) * sizeof(T)) + slot;
   }
 };
-template <int W> __device__ __forceinline__ void setup_reader(StreamReader &rd, unsigned char *smem, int scal_len, size_t elem) {
-  const size_t s = smem_head_bytes(scal_len, blockDim.x, elem, W);
+template <int W, int WLX> __device__ __forceinline__ void setup_reader(StreamReader &rd, unsigned char *smem, int scal_len, size_t elem) {
+  const size_t s = smem_head_bytes(scal_len, blockDim.x, elem, W, WLX);
   rd.init(reinterpret_cast<uint64_t *>(smem + s), reinterpret_cast<uint64_t *>(smem + s + 2 * MQ_CHUNK_WORDS * 8));
 }
+
 
 }  // namespace mqk

@@ -17,16 +17,16 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
                                                          const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  const Roles<dd, W_DD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
   for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
-    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<false>(v, flag_list[i < cnt ? i : cnt - 1], seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
     const bool lost = !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX;
@@ -44,8 +44,8 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
 __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item; __shared__ int s_d;
-  const Roles<dd, 1> ro(smem_raw, scal_len);
-  StreamReader rd; setup_reader<1>(rd, smem_raw, scal_len, sizeof(dd));
+  const Roles<dd, 1, MQ_WL> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(dd));
   const uint32_t total = bv.dd_start[bv.nd];
   for (;;) {
     __syncthreads();
@@ -56,12 +56,12 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     const int d = s_d;
     const DiagView v = make_view(bv.dg[d].blob);
     const unsigned long long cnt = bv.nflag[d];
-    const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + threadIdx.x; const bool live = i < cnt;
-    const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (live ? i : cnt - 1)];
+    const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + ro.slot; const bool live = i < cnt && ro.sub == 0;
+    const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (i < cnt ? i : cnt - 1)];
     double z[MQ_MAXM];
     const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    eval_integrand<dd, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
@@ -81,16 +81,16 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
                                                            const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  const Roles<dd, W_DD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   const unsigned long long cnt = counters[0];
   for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
-    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM];
     const unsigned long long rel = flag_list[i < cnt ? i : cnt - 1];
     if (ro.gw == 0) draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) {
       const double fd = mq_to_double(f);
       f_out[rel] = fd;
@@ -106,15 +106,15 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  const Roles<dd, W_DD> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_DD>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
+  const Roles<dd, W_DD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_DD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(dd));
   for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const bool live = base + ro.slot < n && ro.gw == 0;
+    const bool live = base + ro.slot < n && ro.gw == 0 && ro.sub == 0;
     const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) fdd_out[i] = mq_to_double(f);
   }
 }
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
 using namespace mqk;
 
 int mq_config_dd(mc_diagram *d) {
-  d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd), W_DD);
+  d->smem_dd = smem_bytes(d->max_scal_len, TPB_DD, sizeof(dd), W_DD, MQ_WL);
   cudaError_t e;
   if ((e = allow_max_smem(k_integrate_dd)) != cudaSuccess) return (int)e;
   if ((e = allow_max_smem(k_eval_points_dd)) != cudaSuccess) return (int)e;
@@ -159,7 +159,7 @@ int mq_batch_config_dd(size_t smem, int *grid) {
   *grid = nsm * occ;
   return 0;
 }
-size_t mq_batch_smem_dd(int scal_len) { return smem_bytes(scal_len, TPB_DD, sizeof(dd), 1); }
+size_t mq_batch_smem_dd(int scal_len) { return smem_bytes(scal_len, TPB_DD, sizeof(dd), 1, MQ_WL); }
 void mq_launch_batch_dd(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st) {
   k_batch_dd<<<grid, TPB_DD, smem, (cudaStream_t)st>>>(bv, first, seed, scal_len);
 }

@@ -9,23 +9,23 @@
 namespace mqk {
 
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
-__global__ void __launch_bounds__(TPB_F64, 4) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
+__global__ void __launch_bounds__(TPB_F64, 2) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
                                                            double cond_max, double amin_min, double *partial,
                                                            unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
   // the evaluator is CTA-collective (it stages the table stream through shared memory and splits the families of a
   // point group over W warps): every thread of the CTA runs the same number of iterations; slots past the end
   // re-evaluate the last point and discard it; only the owner warp (gw = 0) of a group draws and accumulates
   for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0;
+    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
-    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
@@ -59,15 +59,15 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
                                                           double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
+  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
   const int M = v.h->M;
-  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
   for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0;
+    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM]; int32_t ord[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<true>(v, first + (i < n ? i : n - 1), seed, z, ord);
     double f, a, amin, xmin;
-    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
@@ -86,15 +86,15 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  const Roles<double, W_F64> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_F64>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
   for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const bool live = base + ro.slot < n && ro.gw == 0;
+    const bool live = base + ro.slot < n && ro.gw == 0 && ro.sub == 0;
     const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;           // surplus slots redo the last point
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     double f, a, amin, xmin;
-    eval_integrand<double, W_F64>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, f, a, amin, xmin);
+    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     if (f64_out) f64_out[i] = f;
     if (cond_out) cond_out[i] = a / fabs(f);
@@ -105,11 +105,11 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
 // ------------------------------------------------------------------ batched path, binary64 tier (a1-a7 for every diagram of a batch)
 // Persistent CTAs; item = PTS_F64 consecutive sample indices of one diagram, taken from queue[0].
 // Flagged points are compacted inside the item in thread order (ballot + prefix): deterministic lists.
-__global__ void __launch_bounds__(TPB_F64, 4) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
+__global__ void __launch_bounds__(TPB_F64, 2) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item, s_wcnt[TPB_F64 / 32];
-  const Roles<double, 1> ro(smem_raw, scal_len);
-  StreamReader rd; setup_reader<1>(rd, smem_raw, scal_len, sizeof(double));
+  const Roles<double, 1, MQ_WL> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(double));
   const uint32_t total = (uint32_t)bv.nd * bv.ipd;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (;;) {
@@ -121,11 +121,11 @@ __global__ void __launch_bounds__(TPB_F64, 4) k_batch_f64(BatchView bv, uint64_t
     const int d = (int)(item / bv.ipd); const uint32_t b = item % bv.ipd;
     const DiagView v = make_view(bv.dg[d].blob);
     const double cond_max = no_dd ? INFINITY : bv.dg[d].cond_max, amin_min = no_dd ? -1.0 : bv.dg[d].amin_min;
-    const uint64_t i = (uint64_t)b * PTS_F64 + threadIdx.x; const bool live = i < n;
+    const uint64_t i = (uint64_t)b * PTS_F64 + ro.slot; const bool live = i < n && ro.sub == 0;
     double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + (live ? i : n - 1), seed, z, nullptr);
+    const double p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
-    eval_integrand<double, 1>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, f, a, amin, xmin);
+    eval_integrand<double, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
     const bool flag = live && (bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min);
     const unsigned bal = __ballot_sync(0xffffffffu, flag);
     if (lane == 0) s_wcnt[warp] = __popc(bal);
@@ -218,8 +218,8 @@ __global__ void k_fp64_peak(int iters, double *sink) {
 using namespace mqk;
 
 int mq_config_f64(mc_diagram *d) {
-  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double), W_F64);
-  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double), W_F64);
+  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double), W_F64, MQ_WL);
+  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double), W_F64, MQ_WL);
   cudaError_t e;
   if ((e = allow_max_smem(k_integrate_f64)) != cudaSuccess) return (int)e;
   if ((e = allow_max_smem(k_eval_points)) != cudaSuccess) return (int)e;
@@ -280,7 +280,7 @@ int mq_batch_config_f64(size_t smem, int *grid) {
   *grid = nsm * occ;
   return 0;
 }
-size_t mq_batch_smem_f64(int scal_len) { return smem_bytes(scal_len, TPB_F64, sizeof(double), 1); }
+size_t mq_batch_smem_f64(int scal_len) { return smem_bytes(scal_len, TPB_F64, sizeof(double), 1, MQ_WL); }
 void mq_launch_batch_f64(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd, mq_stream st) {
   k_batch_f64<<<grid, TPB_F64, smem, (cudaStream_t)st>>>(bv, first, n, seed, scal_len, no_dd);
 }

@@ -183,16 +183,16 @@ struct StreamReader {
 // operands r_t and beta~_tu are gathered once per family from S[index][thread] into registers
 template <class T, int KD>
 __device__ __forceinline__ T horner(uint32_t &s_coef, const T *r) {
-  if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8; return v; }
+  if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8 * MQ_WL; return v; }   // the MQ_WL members of an entry are interleaved
   else {
     constexpr int H = 1 << (KD - 1);
     T v[H];
 #pragma unroll
     for (int j = 0; j < H; j++) {
-      const double2 cc = lds_f64x2(s_coef + 16 * j);                       // (c[j], c[j+H])
+      const double2 cc = lds_f64x2(s_coef + 16 * MQ_WL * j);               // (c[j], c[j+H])
       v[j] = mq_fma_c(cc.y, r[KD - 1], cc.x, T());
     }
-    s_coef += 16 * H;
+    s_coef += 16 * MQ_WL * H;
 #pragma unroll
     for (int i = KD - 2; i >= 0; i--) {
 #pragma unroll
@@ -310,7 +310,7 @@ __device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t
   auto horner_at = [&](uint32_t a) -> T {
     if (kd == 0) return T(lds_f64(a));
     const int H = 1 << (kd - 1);
-    for (int j = 0; j < H; j++) { const double2 cc = lds_f64x2(a + 16 * j); v[j] = mq_fma_c(cc.y, r[kd - 1], cc.x, T()); }
+    for (int j = 0; j < H; j++) { const double2 cc = lds_f64x2(a + 16 * MQ_WL * j); v[j] = mq_fma_c(cc.y, r[kd - 1], cc.x, T()); }
     for (int i = kd - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
     return v[0];
   };
@@ -325,7 +325,7 @@ __device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t
     if (s2 >= n2) { level--; continue; }
     scur[level] = s2;
     const T wn = w[level] * b[f * n2 - f * (f + 1) / 2 + (s2 - f - 1)];
-    if (level == c - 1) { sum = sum + wn * horner_at(s_coef); s_coef += 8 * nblk; }
+    if (level == c - 1) { sum = sum + wn * horner_at(s_coef); s_coef += 8 * MQ_WL * nblk; }
     else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
   }
   return sum;
@@ -334,7 +334,7 @@ __device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t
 // ------------------------------------------------------------------ a4: scalars of one piece
 // writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
 template <class T>
-__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, T &U, T &V, T &G, double &amin, double &xmin) {
+__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, bool wr, T &U, T &V, T &G, double &amin, double &xmin) {
   const int n = g.nch, ns = g.nslot;
   T A[MQ_MAXL][MQ_MAXL], Inv[MQ_MAXL][MQ_MAXL];
 #pragma unroll
@@ -395,22 +395,23 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
         const T zb = bsu * T(z[g.slot[u].zline]);
         x = x + zb; if (g.slot[u].sgn < 0) q = q - zb; else q = q + zb;
       }
-      if (u > s) S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride] = bsu;   // raw beta, scaled below
+      if (u > s && wr) S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride] = bsu;   // raw beta, scaled below
     }
     const bool line = g.slot[s].kind == MQ_SLOT_LINE;
     const T gs = T(2.0) - x;
     const T igs = line ? T(1.0) / gs : T(1.0);
     ig[s] = igs;
-    S[s * stride] = x * igs;                                  // r_t = x_t / g_t   (lines)
-    if (off_at >= 0) S[(off_at + s) * stride] = T(1.0) - x;   // A_t
+    if (wr) S[s * stride] = x * igs;                                  // r_t = x_t / g_t   (lines)
+    if (off_at >= 0 && wr) S[(off_at + s) * stride] = T(1.0) - x;   // A_t
     const T sg = T((double)g.slot[s].sgn);
-    if (off_aq >= 0) S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);   // A'_t / g_t
+    if (off_aq >= 0 && wr) S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);   // A'_t / g_t
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
       const double xd = mq_to_double(x);
       amin = fmin(amin, fmin(fabs(1.0 - xd), 2.0 - xd));
     }
   }
+  if (wr)
   for (int s = 0; s < ns; s++)
     for (int u = s + 1; u < ns; u++) {
       T *p = &S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride];
@@ -435,13 +436,22 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 // (|family value| summed, |child value| multiplied): abs_out = sum over terms and grades of that bound. It measures
 // every cancellation between families, pieces and terms (O8) at the cost of one add per family.
 //
-// Warp split: W warps share one group of 32 points. Warp gw = 0 of the group owns the points (scalars, node
-// values, terms); the families of every table are dealt round-robin to the W warps, which all read the same
+// Lane split (LANES = true; binary64 and double-double kernels): MQ_WL lanes of a warp share one sample point. All of
+// them compute the point's scalars (only lane role sub = 0 writes S), then each evaluates ITS member of every stream
+// entry (MQ_WL same-shape families side by side, device_layout.h) from the common S[index][point]; the partial graded
+// sums are added across the lane roles with warp shuffles once per table, so every lane ends with the same totals.
+// This multiplies the warps per SM at constant shared memory per point (occupancy is capped by S), with no
+// duplicated family work. LANES = false (quad-double): one lane per point evaluates the members one after the other.
+// Warp split: W warps share one group of points. Warp gw = 0 of the group owns the points (scalars, node
+// values, terms); the entries of every table are dealt round-robin to the W warps, which all read the same
 // S[index][point] in shared memory; their partial graded sums are added through the exchange area xT/xA.
-// This multiplies the warps per SM at constant shared memory per point (occupancy is otherwise capped by S).
 // CTA-collective: contains __syncthreads; every thread of the CTA must call it.
-template <class T, int W>
-__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T *xT, double *xA, int gw,
+template <class T> __device__ __forceinline__ T mq_shfl_xor(T v, int m);
+template <> __device__ __forceinline__ double mq_shfl_xor<double>(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+template <> __device__ __forceinline__ dd mq_shfl_xor<dd>(dd v, int m) { return dd(__shfl_xor_sync(0xffffffffu, v.hi, m), __shfl_xor_sync(0xffffffffu, v.lo, m)); }
+
+template <class T, int W, bool LANES>
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T *xT, double *xA, int gw, int sub,
                                             T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
   constexpr bool TRACK = true;
   const DevHeader &h = *v.h;
@@ -454,8 +464,10 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
     T U = T(1.0), V = T(0.0), G = T(1.0);
-    if (gw == 0) piece_scalars<T>(g, z, S, stride, U, V, G, amin, xmin);
+    if constexpr (LANES) __syncwarp();                 // every lane role has finished reading S of the previous piece
+    if (gw == 0) piece_scalars<T>(g, z, S, stride, sub == 0, U, V, G, amin, xmin);
     if constexpr (W > 1) __syncthreads();              // S of this piece is complete before any warp gathers from it
+    else if constexpr (LANES) __syncwarp();
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
       const DevTable &tb = v.tab[ti];
@@ -464,37 +476,46 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
       for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = 0.0; }
-      // families of this table from the staged stream; a run of families with the same (output, pattern, grade)
-      // accumulates in registers and is flushed when the key changes (families are sorted by that key)
+      // entries of this table from the staged stream; a run of families with the same (output, pattern, grade)
+      // accumulates in registers and is flushed when the key changes
       int key = -1; T racc = T(0.0); double racca = 0.0;
-      bool have = false; uint32_t a0 = 0; uint64_t hd = 0, w0 = 0, w1 = 0;   // header + first index words of the current entry
-      int unit = 0;                                                          // evaluation units are dealt round-robin to the W warps
+      bool have = false; uint32_t a0 = 0; uint64_t hd = 0, hl = 0, w0 = 0, w1 = 0;   // entry header, this lane's member header + first index words
+      int unit = 0;                                                                  // evaluation units are dealt round-robin to the W warps
+      // this lane's member of the entry at address a with (uniform) header hu: its header word and first two index words
+      auto fetch_member = [&](uint32_t a, uint64_t hu, int m, uint64_t &ml, uint64_t &m0, uint64_t &m1) {
+        const uint32_t iw = (hu & 7) == MQ_PAD_MARK ? 0u : (uint32_t)(hu >> 16 & 0xFFFF);
+        const uint32_t ma = a + 8 * MQ_WL + 8 * iw * (uint32_t)m;
+        ml = lds_u64(a + 8 * (uint32_t)m); m0 = lds_u64(ma); m1 = lds_u64(ma + 8);
+      };
       for (int left = tb.nfam; left > 0;) {
         if (!have) {
           if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
-          a0 = rd.addr(); hd = lds_u64(a0); w0 = lds_u64(a0 + 8); w1 = lds_u64(a0 + 16);
+          a0 = rd.addr(); hd = lds_u64(a0);
+          if constexpr (LANES) fetch_member(a0, hd, sub, hl, w0, w1);
         }
         const int idxw = (int)(hd >> 16 & 0xFFFF);
         const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7);
         if (c == MQ_PAD_MARK) { rd.pos += 1 + idxw; have = false; continue; }
-        const int nscal = (int)(hd >> 10 & 15), kk = (int)((hd & 7) | ((hd >> 6 & 15) << 3) | ((hd >> 14 & 1) << 7));
-        const int size = 1 + idxw + (int)(uint32_t)(hd >> 32), npos = rd.pos + size;
-        // software pipeline: fetch the next entry's header and index words before this family's arithmetic
-        uint32_t an = a0 + 8 * size; uint64_t hdn = 0, n0 = 0, n1 = 0;
+        const int size = MQ_WL * (1 + idxw) + (int)(uint32_t)(hd >> 32), npos = rd.pos + size;
+        // software pipeline: fetch the next entry's header and index words before this entry's arithmetic
+        uint32_t an = a0 + 8 * size; uint64_t hdn = 0, hln = 0, n0 = 0, n1 = 0;
         const bool havenext = npos < MQ_CHUNK_WORDS;
-        if (havenext) { hdn = lds_u64(an); n0 = lds_u64(an + 8); n1 = lds_u64(an + 16); }
-        // pair this family with the next one if it has the same shape (binary64: doubles the ILP of the warp)
+        if (havenext) { hdn = lds_u64(an); if constexpr (LANES) fetch_member(an, hdn, sub, hln, n0, n1); }
+        // pair this entry with the next one if it has the same shape (binary64: doubles the ILP of the warp)
         bool dual = false;
-        if constexpr (sizeof(T) == sizeof(double)) {
+        if constexpr (sizeof(T) == sizeof(double) && LANES) {
           if (havenext && left > 1 && c <= 3 && (int)(hdn & 63) == (int)(hd & 63)) {
-            const int size2 = 1 + (int)(hdn >> 16 & 0xFFFF) + (int)(uint32_t)(hdn >> 32);
+            const int size2 = MQ_WL * (1 + (int)(hdn >> 16 & 0xFFFF)) + (int)(uint32_t)(hdn >> 32);
             dual = npos + size2 <= MQ_CHUNK_WORDS;
           }
         }
         const int nb = c * (2 * c - 1) + kd;
-        auto account = [&](T val, uint32_t ea, int ns, int keyk) {
+        const uint32_t ustride = kd ? 16u : 8u;                        // bytes between the members' coefficient units
+        // member header ml: scalar factors and accumulation key; sidx: shared address of the member's index bytes
+        auto account = [&](T val, uint64_t ml, uint32_t sidx) {
+          const int ns = (int)(ml >> 10 & 15), keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
           val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
-          for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(ea + 8 + nb + i) * sstride);
+          for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(sidx + nb + i) * sstride);
           if (keyk != key) {
             if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
             key = keyk; racc = T(0.0); racca = 0.0;
@@ -503,37 +524,55 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
           if constexpr (TRACK) racca += fabs(mq_to_double(val));
         };
         if (dual) {
-          if constexpr (sizeof(T) == sizeof(double)) {
-            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = 1 + idxw2 + (int)(uint32_t)(hdn >> 32), npos2 = npos + size2;
-            const int nscal2 = (int)(hdn >> 10 & 15), kk2 = (int)((hdn & 7) | ((hdn >> 6 & 15) << 3) | ((hdn >> 14 & 1) << 7));
+          if constexpr (sizeof(T) == sizeof(double) && LANES) {
+            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = MQ_WL * (1 + idxw2) + (int)(uint32_t)(hdn >> 32), npos2 = npos + size2;
             const uint32_t a2 = an + 8 * size2;
-            uint64_t hd3 = 0, m0 = 0, m1 = 0;
+            uint64_t hd3 = 0, hl3 = 0, m0 = 0, m1 = 0;
             const bool have3 = npos2 < MQ_CHUNK_WORDS;
-            if (have3) { hd3 = lds_u64(a2); m0 = lds_u64(a2 + 8); m1 = lds_u64(a2 + 16); }
+            if (have3) { hd3 = lds_u64(a2); fetch_member(a2, hd3, sub, hl3, m0, m1); }
             if (W == 1 || unit % W == gw) {
               const uint64_t w4[4] = {w0, w1, n0, n1};
+              const uint32_t sidxA = a0 + 8 * MQ_WL + 8 * idxw * sub, sidxB = an + 8 * MQ_WL + 8 * idxw2 * sub;
               double vA, vB;
-              family_dispatch2(c * 8 + kd, w4, a0 + 8, a0 + 8 + 8 * idxw, an + 8, an + 8 + 8 * idxw2, s_S, sstride, vA, vB);
-              account(T(vA), a0, nscal, kk);
-              account(T(vB), an, nscal2, kk2);
+              family_dispatch2(c * 8 + kd, w4, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub, sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub,
+                               s_S, sstride, vA, vB);
+              account(T(vA), hl, sidxA);
+              account(T(vB), hln, sidxB);
             }
             unit++;
             rd.pos = npos2; left -= 2;
-            have = have3; a0 = a2; hd = hd3; w0 = m0; w1 = m1;
+            have = have3; a0 = a2; hd = hd3; hl = hl3; w0 = m0; w1 = m1;
             continue;
           }
         }
         if (W == 1 || unit % W == gw) {
-          T val;
-          if constexpr (sizeof(T) > sizeof(dd)) val = family_generic<T>(c, kd, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
-          else val = family_dispatch<T>(c * 8 + kd, w0, w1, a0 + 8, a0 + 8 + 8 * idxw, s_S, sstride);
-          account(val, a0, nscal, kk);
+#pragma unroll 1
+          for (int q = 0; q < (LANES ? 1 : MQ_WL); q++) {
+            const int m = LANES ? sub : q;
+            if constexpr (!LANES) fetch_member(a0, hd, m, hl, w0, w1);
+            const uint32_t sidx = a0 + 8 * MQ_WL + 8 * idxw * m, scoef = a0 + 8 * MQ_WL * (1 + idxw) + ustride * m;
+            T val;
+            if constexpr (sizeof(T) > sizeof(dd)) val = family_generic<T>(c, kd, sidx, scoef, s_S, sstride);
+            else val = family_dispatch<T>(c * 8 + kd, w0, w1, sidx, scoef, s_S, sstride);
+            account(val, hl, sidx);
+          }
         }
         unit++;
         rd.pos = npos; left--;
-        have = havenext; a0 = an; hd = hdn; w0 = n0; w1 = n1;
+        have = havenext; a0 = an; hd = hdn; hl = hln; w0 = n0; w1 = n1;
       }
       if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
+      if constexpr (LANES && MQ_WL > 1) {              // add the partial sums of the lane roles: afterwards every lane holds the totals
+        for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
+#pragma unroll
+          for (int c = 0; c < MQ_NGRADE; c++) {
+#pragma unroll
+            for (int m = 32 / MQ_WL; m < 32; m <<= 1) {
+              N[o][p][c] = N[o][p][c] + mq_shfl_xor<T>(N[o][p][c], m);
+              if constexpr (TRACK) Na[o][p][c] += __shfl_xor_sync(0xffffffffu, Na[o][p][c], m);
+            }
+          }
+      }
       if (tb.nout == 1 && (tb.op == MQ_OP_U || tb.op == MQ_OP_LMU)) {   // these tables hold 12*coefficient (coef_gen.hpp)
         const T i12 = T(1.0) / T(12.0);
         for (int p = 0; p < npat; p++)

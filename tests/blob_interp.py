@@ -52,23 +52,36 @@ class Blob:
         self._pair_cache = {}
 
     def families(self, ti):
+        """yields the families of table ti; a stream entry holds WL same-shape families side by side (device_layout.h)"""
+        WL = 2
         t = self.table[ti]
         pos = int(t["stream_off"])
         raw = self.w.view(np.uint8)
-        nleft = int(t["nfam"])
+        nleft = int(t["nfam"])                       # stream entries
         while nleft:
             hd = int(self.w[pos])
-            c, kd, pat, nscal, out = hd & 7, hd >> 3 & 7, hd >> 6 & 15, hd >> 10 & 15, hd >> 14 & 1
+            c, kd = hd & 7, hd >> 3 & 7
             idxw, ncoef = hd >> 16 & 0xFFFF, hd >> 32
             if c == 7:                      # PAD entry up to the chunk boundary
                 pos += 1 + idxw
                 continue
             nleft -= 1
             nb = c * (2 * c - 1)
-            idx = raw[(pos + 1) * 8:(pos + 1) * 8 + nb + kd + nscal].astype(int)
-            coef = self.w[pos + 1 + idxw:pos + 1 + idxw + ncoef].view(np.float64)
-            yield c, kd, pat, out, idx[:nb], idx[nb:nb + kd], idx[nb + kd:], coef
-            pos += 1 + idxw + ncoef
+            assert ncoef % WL == 0 and (pos + WL * (1 + idxw)) % 2 == 0
+            unit = 2 if kd >= 1 else 1
+            allc = self.w[pos + WL * (1 + idxw):pos + WL * (1 + idxw) + ncoef].view(np.float64).reshape(-1, WL, unit)
+            for m in range(WL):
+                hm = int(self.w[pos + m])
+                assert (hm & 63) == (hd & 63) and (hm >> 16) == (hd >> 16)
+                pat, nscal, out, void = hm >> 6 & 15, hm >> 10 & 15, hm >> 14 & 1, hm >> 15 & 1
+                coef = np.ascontiguousarray(allc[:, m, :]).reshape(-1)
+                if void:
+                    assert not coef.any()
+                    continue
+                at = (pos + WL + m * idxw) * 8
+                idx = raw[at:at + nb + kd + nscal].astype(int)
+                yield c, kd, pat, out, idx[:nb], idx[nb:nb + kd], idx[nb + kd:], coef
+            pos += WL * (1 + idxw) + ncoef
         assert pos == int(t["stream_off"] + t["stream_words"])
 
     def scalars(self, g, z):
