@@ -227,12 +227,25 @@ def run_ours(args):
         e2e_s = float(t.item())
     e2e = {"value": world * G * n_tot / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 32 * G,
            "note": "inputs are (first_sample, n, seed) scalars: no host->device tensor; 4 results (32 B) per diagram come back per step"}
+    # precision-policy mix on a sample (mc_eval_points flag_out: 0 accepted by the relative bound, 1 re-evaluated in
+    # double-double, 2 precision loss detected but accepted by the absolute bound on the weight; O8)
+    mix = [0, 0, 0]
+    ns = 4096
+    for d in diagrams[::max(1, G // 8)][:8]:
+        fl = torch.zeros(ns, dtype=torch.uint8, device="cuda")
+        d.eval_points(state["first"], ns, seed, stream, flag=fl)
+        torch.cuda.synchronize()
+        cts = torch.bincount(fl.long(), minlength=3).cpu().numpy()
+        mix = [mix[i] + int(cts[i]) for i in range(3)]
+    mixn = float(sum(mix))
+    precision = {"cond_max": 1e4, "amin_min": 1e-2, "w_abs_tol": 1e-10, "dd_cond_max": 1e26,
+                 "sample_mix": {"accepted_relative": mix[0] / mixn, "reevaluated_dd": mix[1] / mixn, "accepted_absolute": mix[2] / mixn, "points": int(mixn)}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[%d]: %d seeded 5-loop graphs without lepton loops, %d points per graph per step" % (args.config, G, B) if args.config == 4
                        else "configs[%d]: %d graphs, %d points per graph per step" % (args.config, G, B),
                        "n_graphs": G, "batch": B, "seed": seed, "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
-                       "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "dropped": int(c[1].sum()),
+                       "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "precision": precision, "dropped": int(c[1].sum()),
                        "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
                        "algorithmic_flop_per_sample_mean": sum(flop) / G},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}

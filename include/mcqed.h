@@ -97,6 +97,19 @@ int mc_diagram_sampler_tables(const mc_diagram *, double *deg, double *Z, double
  * pass). Used by bench.py to time the binary64 kernel alone. HOST. */
 int mc_diagram_set_flags(mc_diagram *, uint32_t flags);
 
+/* Precision policy of an existing handle (O8; "interval arithmetic ... with different precisions":
+ * the paper gives no thresholds). Every tier carries a = sum |contribution| next to f and inner = the smallest |A_t|, g_t and
+ * pivot ratio of the point. A tier's value is ACCEPTED if
+ *   (relative) a <= cond * |f| and inner >= inner_min, with (cond, inner_min) = (cond_max, amin_min) in binary64 (then
+ *              |df| <= 1e-10 |f|) and (dd_cond_max, 1/dd_cond_max) in double-double, or
+ *   (absolute) 64 ulp * a / min(1, inner) <= w_abs_tol * p: the round-off bound on the WEIGHT w = f/p is below
+ *              w_abs_tol. The Monte Carlo sums need absolute accuracy of the weights; deep in the corners of the simplex the
+ *              subtracted integrand loses all relative precision while f/p is 1e-20 and smaller.
+ * Otherwise the point goes to the next tier (binary64 -> double-double -> quad-double). Defaults: cond_max, amin_min from
+ * mc_options; dd_cond_max = 1e26; w_abs_tol = 1e-10 (0 switches the absolute criterion off). A batch copies the values
+ * when it is created. HOST. MC_EINVAL on cond_max <= 0, dd_cond_max < 1, w_abs_tol < 0. */
+int mc_diagram_set_precision(mc_diagram *, double cond_max, double amin_min, double dd_cond_max, double w_abs_tol);
+
 /* Host copy of the device table blob (layout: csrc/device_layout.h), for format tests. Returns the
  * number of 8-byte words; copies min(words, cap) words into out (may be NULL). HOST. */
 int64_t mc_diagram_blob(const mc_diagram *, uint64_t *out, int64_t cap);
@@ -144,7 +157,9 @@ void mc_batch_free(mc_batch *);
 /* Parity hook: per-point values for comparison with the oracle. DEVICE outputs, any may be NULL:
  * z_out n*M (row = point, column = line index), order_out n*M (the Hepp sector j_1..j_M),
  * p_out n (density), f_out n (value used by mc_integrate: binary64, or double-double rounded to
- * binary64 if flagged), f64_out n (plain binary64 value), cond_out n (sum|contrib|/|f|), flag_out n. */
+ * binary64 if flagged), f64_out n (plain binary64 value), cond_out n (sum|contrib|/|f|), flag_out n: 0 = accepted by the
+ * relative bound, 1 = re-evaluated in double-double (or beyond), 2 = precision loss detected but accepted by the absolute
+ * bound on the weight (mc_diagram_set_precision). */
 int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
                    double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out,
                    double *cond_out, uint8_t *flag_out);

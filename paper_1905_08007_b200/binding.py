@@ -16,7 +16,7 @@ FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
-    "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags",
+    "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags", "mc_diagram_set_precision",
     "mc_integrate", "mc_integrate_host", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
@@ -70,6 +70,7 @@ def lib():
         L.mc_diagram_blob.argtypes = [vp, C.POINTER(C.c_uint64), C.c_int64]
         L.mc_diagram_blob.restype = C.c_int64
         L.mc_diagram_set_flags.argtypes = [vp, C.c_uint32]
+        L.mc_diagram_set_precision.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_double]
         L.mc_integrate.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.mc_batch_create.argtypes = [C.POINTER(vp), C.c_int32, u64, C.POINTER(vp)]
@@ -173,6 +174,9 @@ class Diagram:
 
     def set_flags(self, flags):
         _check(lib().mc_diagram_set_flags(self.h, flags), "mc_diagram_set_flags")
+
+    def set_dd_limit(self, dd_cond_max):
+        _check(lib().mc_diagram_set_dd_limit(self.h, dd_cond_max), "mc_diagram_set_precision")
 
     def blob(self):
         n = lib().mc_diagram_blob(self.h, None, 0)

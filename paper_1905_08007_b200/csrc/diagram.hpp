@@ -17,6 +17,8 @@ constexpr int W_F64 = 1, W_DD = 1;
 constexpr int PTS_F64 = TPB_F64 / (W_F64 * MQ_WL), PTS_DD = TPB_DD / (W_DD * MQ_WL), PTS_EVAL = TPB_EVAL / (W_F64 * MQ_WL);   // points per CTA (MQ_WL lanes per point)
 constexpr uint64_t CHUNK = 1ull << 22;     // samples per launch (bounds the flagged-index list)
 constexpr int MAXGRID = 148 * 32;
+// precision policy of one diagram as the kernels see it (O8; include/mcqed.h mc_diagram_set_precision)
+struct MqPrec { double cond_max, amin_min, dd_cond_max, w_abs_tol; };
 constexpr uint64_t LOSTCAP = CHUNK / 8;   // capacity of the list of points handed from double-double to quad-double
 }  // namespace mqk
 
@@ -32,6 +34,10 @@ struct mc_diagram {
   mq::ForestTerms ft;
   mq::SamplerTables st;
   mc_options opt{};
+  double dd_cond_max = 1e26, w_abs_tol = 1e-10;   // mc_diagram_set_precision
+  mqk::MqPrec prec(bool no_dd) const {    // no_dd: nothing but non-finite points is handed on
+    return no_dd ? mqk::MqPrec{1e300, -1.0, dd_cond_max, w_abs_tol} : mqk::MqPrec{opt.cond_max, opt.amin_min, dd_cond_max, w_abs_tol};
+  }
   int id = -1;
   std::vector<uint64_t> blob;              // host copy of the device blob (device_layout.h)
   std::vector<DevGeom> geoms; std::vector<DevTable> tables; std::vector<DevNode> nodes; std::vector<DevTerm> terms;
@@ -50,7 +56,7 @@ struct mc_diagram {
 namespace mqk {
 struct BatchDiag {
   const uint64_t *blob;
-  double cond_max, amin_min;
+  MqPrec pr;
 };
 struct BatchView {
   const BatchDiag *dg;             // [nd]
@@ -90,11 +96,11 @@ int mq_config_qd(mc_diagram *d);
 void mq_launch_integrate_qd(const mc_diagram *d, uint64_t seed, mq_stream st);
 void mq_launch_eval_points_qd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st);
 void mq_launch_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, double *fqd_out, mq_stream st);
-void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st);
+void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, mqk::MqPrec pr, mq_stream st);
 void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st);
 void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, int nb3, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);
 void mq_launch_reset(const mc_diagram *d, mq_stream st);
-void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,
+void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, mqk::MqPrec pr,
                            double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out,
                            uint8_t *flag_out, bool list_flagged, mq_stream st);
 void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st);

@@ -63,6 +63,21 @@ __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   
   return bad;
 }
 
+// Precision decision of one tier (O8). a = sum |contribution| carried by the evaluator, inner = min over the
+// electron lines of every piece of (|A_t|, g_t, pivot / diagonal), unit = 64 ulp of the tier's arithmetic.
+//   0: accepted, relative round-off bound met (a <= cond_max |f| and inner >= inner_min): |df| <= 1e-10 |f| in tier 1
+//   2: precision loss detected, but the absolute round-off bound on the WEIGHT w = f/p is below w_abs_tol: the
+//      Monte Carlo sums need absolute, not relative, accuracy of w (PAPER.md:91 controls the round-off error of the result)
+//   1: handed to the next tier
+#define MQ_UNIT_F64 (64.0 * 0x1p-53)
+#define MQ_UNIT_DD (64.0 * 0x1p-103)
+__device__ __forceinline__ int tier_decision(bool hard, double f, double a, double inner, double p, double cond_max, double inner_min, double unit, double w_abs_tol) {
+  if (hard || !isfinite(f) || !isfinite(a)) return 1;
+  if (a <= cond_max * fabs(f) && inner >= inner_min) return 0;
+  if (unit * a <= w_abs_tol * p * fmin(1.0, inner)) return 2;
+  return 1;
+}
+
 // Thread roles (mcqed_kernels.cuh "lane split" / "warp split"): WLX lanes of a warp share one sample point (WLX = MQ_WL in
 // the binary64 and double-double kernels, 1 in quad-double) and W warps share one group of 32 / WLX points, so a CTA of
 // `threads` threads holds P = threads / (W * WLX) points; warp w works for point group w / W in role gw = w % W, lane l

@@ -9,11 +9,11 @@
 namespace mqk {
 
 // beyond double-double (O8): pair arithmetic carries ~2^-103 relative to the operands, so a point whose
-// condition number (or pivot / current loss) exceeds this keeps fewer than ~5 digits and goes on to quad-double
-#define MQ_DD_COND_MAX 1e26
+// condition number (or pivot / current loss) exceeds dd_cond_max (default 1e26: ~5 digits left) goes on to quad-double,
+// unless the absolute round-off bound on its weight is already below w_abs_tol (tier_decision, kern_common.cuh)
 
 // a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
-__global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
+__global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, MqPrec pr, double *partial,
                                                          const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
@@ -29,9 +29,9 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
-    const bool lost = !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX;
+    const bool lost = tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;
     if (bad_point(z, v.h->M, p)) atomicAdd(&counters[1], 1ull);                  // dropped: w = 0
-    else if (!isfinite(fd) || lost) {                                          // third tier: quad-double
+    else if (lost) {                                          // third tier: quad-double
       const unsigned long long slot = atomicAdd(&counters[2], 1ull);
       if (slot < LOSTCAP) lost_list[slot] = flag_list[i]; else { atomicAdd(&counters[1], 1ull); }
     }
@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     if (item >= total) break;
     const int d = s_d;
     const DiagView v = make_view(bv.dg[d].blob);
+    const MqPrec pr = bv.dg[d].pr;
     const unsigned long long cnt = bv.nflag[d];
     const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + ro.slot; const bool live = i < cnt && ro.sub == 0;
     const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (i < cnt ? i : cnt - 1)];
@@ -65,9 +66,9 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
-      const bool lost = !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX;     // same rule as k_integrate_dd
+      const bool lost = tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;     // same rule as k_integrate_dd
       if (bad_point(z, v.h->M, p)) atomicAdd(&bv.ndrop[d], 1ull);
-      else if (!isfinite(fd) || lost) {
+      else if (lost) {
         const unsigned long long slot = atomicAdd(&bv.nlost[d], 1ull);
         if (slot < bv.lostcap) bv.lost_list[(size_t)d * bv.lostcap + slot] = rel; else atomicAdd(&bv.ndrop[d], 1ull);
       }
@@ -77,7 +78,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
   }
 }
 
-__global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, double *f_out,
+__global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, MqPrec pr, double *f_out,
                                                            const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
@@ -86,15 +87,15 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
   const unsigned long long cnt = counters[0];
   for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
     const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
-    double z[MQ_MAXM];
+    double z[MQ_MAXM]; double p = 1.0;
     const unsigned long long rel = flag_list[i < cnt ? i : cnt - 1];
-    if (ro.gw == 0) draw_point<false>(v, first + rel, seed, z, nullptr);
+    if (ro.gw == 0) p = draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
     eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) {
       const double fd = mq_to_double(f);
       f_out[rel] = fd;
-      if (!isfinite(fd) || !(mq_to_double(a) <= MQ_DD_COND_MAX * fabs(fd)) || fmin(amin, xmin) < 1.0 / MQ_DD_COND_MAX) {
+      if (tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1) {
         const unsigned long long slot = atomicAdd(&counters[2], 1ull);
         if (slot < LOSTCAP) lost_list[slot] = rel;
       }
@@ -138,10 +139,10 @@ int mq_config_dd(mc_diagram *d) {
   return 0;
 }
 void mq_launch_integrate_dd(const mc_diagram *d, uint64_t seed, mq_stream st) {
-  k_integrate_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, seed, d->ws.partial + (size_t)MAXGRID * 4, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
+  k_integrate_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, seed, d->prec(false), d->ws.partial + (size_t)MAXGRID * 4, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
 }
 void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed, double *f_out, mq_stream st) {
-  k_eval_points_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, first, seed, f_out, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
+  k_eval_points_dd<<<d->grid_dd, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, first, seed, d->prec(false), f_out, d->ws.flag_list, d->ws.lost_list, d->ws.counters);
 }
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st) {
   k_eval_z_dd<<<grid, TPB_DD, d->smem_dd, (cudaStream_t)st>>>(d->d_blob, n, z_in, fdd_out);

@@ -10,7 +10,7 @@ namespace mqk {
 
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
 __global__ void __launch_bounds__(TPB_F64, 2) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
-                                                           double cond_max, double amin_min, double *partial,
+                                                           MqPrec pr, double *partial,
                                                            unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(TPB_F64, 2) k_integrate_f64(const uint64_t *__
     double f, a, amin, xmin;
     eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
-    const bool flag = bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
+    const bool flag = tier_decision(bad_point(z, v.h->M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
     else { const double w = f / p; s1.add(w); s2.add(w * w); }
   }
@@ -54,7 +54,7 @@ __global__ void k_reset_counters(unsigned long long *counters) { counters[0] = 0
 
 // parity hook: per-point outputs (binary64 pass); flagged points are listed for the dd pass
 __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
-                                                          double cond_max, double amin_min,
+                                                          MqPrec pr,
                                                           double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out,
                                                           double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -69,14 +69,15 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
     double f, a, amin, xmin;
     eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
-    const bool flag = bad_point(z, M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min;
+    const int dec = tier_decision(bad_point(z, M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
+    const bool flag = dec == 1;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
     if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
     if (p_out) p_out[i] = p;
     if (f_out) f_out[i] = f;
     if (f64_out) f64_out[i] = f;
     if (cond_out) cond_out[i] = a / fabs(f);
-    if (flag_out) flag_out[i] = flag ? 1 : 0;
+    if (flag_out) flag_out[i] = (uint8_t)dec;      // 0 accepted (relative), 1 re-evaluated in double-double, 2 accepted by the absolute bound on w
     if (flag && flag_list) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = i; }
   }
 }
@@ -120,13 +121,14 @@ __global__ void __launch_bounds__(TPB_F64, 2) k_batch_f64(BatchView bv, uint64_t
     if (item >= total) break;
     const int d = (int)(item / bv.ipd); const uint32_t b = item % bv.ipd;
     const DiagView v = make_view(bv.dg[d].blob);
-    const double cond_max = no_dd ? INFINITY : bv.dg[d].cond_max, amin_min = no_dd ? -1.0 : bv.dg[d].amin_min;
+    MqPrec pr = bv.dg[d].pr;
+    if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
     const uint64_t i = (uint64_t)b * PTS_F64 + ro.slot; const bool live = i < n && ro.sub == 0;
     double z[MQ_MAXM];
     const double p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
     eval_integrand<double, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
-    const bool flag = live && (bad_point(z, v.h->M, p) || !isfinite(f) || !isfinite(a) || a > cond_max * fabs(f) || fmin(amin, xmin) < amin_min);
+    const bool flag = live && tier_decision(bad_point(z, v.h->M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
     const unsigned bal = __ballot_sync(0xffffffffu, flag);
     if (lane == 0) s_wcnt[warp] = __popc(bal);
     __syncthreads();
@@ -232,17 +234,17 @@ int mq_config_f64(mc_diagram *d) {
   d->grid_f64 = std::min(MAXGRID, nsm * occ);
   return 0;
 }
-void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min, mq_stream st) {
-  k_integrate_f64<<<grid, TPB_F64, d->smem_f64, (cudaStream_t)st>>>(d->d_blob, first, n, seed, cond_max, amin_min, d->ws.partial, d->ws.flag_list, d->ws.counters);
+void mq_launch_integrate_f64(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, MqPrec pr, mq_stream st) {
+  k_integrate_f64<<<grid, TPB_F64, d->smem_f64, (cudaStream_t)st>>>(d->d_blob, first, n, seed, pr, d->ws.partial, d->ws.flag_list, d->ws.counters);
 }
 void mq_launch_finish(const mc_diagram *d, int nb1, int nb2, int nb3, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
   k_finish<<<1, 32, 0, (cudaStream_t)st>>>(d->ws.partial, nb1, nb2, nb3, d->ws.counters, out_sum, out_sumsq, out_nflag, out_ndrop);
 }
 void mq_launch_reset(const mc_diagram *d, mq_stream st) { k_reset_counters<<<1, 1, 0, (cudaStream_t)st>>>(d->ws.counters); }
-void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, double cond_max, double amin_min,
+void mq_launch_eval_points(const mc_diagram *d, int grid, uint64_t first, uint64_t n, uint64_t seed, MqPrec pr,
                            double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out,
                            uint8_t *flag_out, bool list_flagged, mq_stream st) {
-  k_eval_points<<<grid, TPB_EVAL, d->smem_eval, (cudaStream_t)st>>>(d->d_blob, first, n, seed, cond_max, amin_min, z_out, order_out, p_out, f_out, f64_out,
+  k_eval_points<<<grid, TPB_EVAL, d->smem_eval, (cudaStream_t)st>>>(d->d_blob, first, n, seed, pr, z_out, order_out, p_out, f_out, f64_out,
                                                                   cond_out, flag_out, list_flagged ? d->ws.flag_list : nullptr, d->ws.counters);
 }
 void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st) {

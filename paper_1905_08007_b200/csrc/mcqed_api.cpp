@@ -104,6 +104,11 @@ int mc_diagram_set_flags(mc_diagram *d, uint32_t flags) {
   d->opt.flags = (d->opt.flags & ~1u) | (flags & 1u);
   return MC_OK;
 }
+int mc_diagram_set_precision(mc_diagram *d, double cond_max, double amin_min, double dd_cond_max, double w_abs_tol) {
+  if (!d || !(cond_max > 0) || !(dd_cond_max >= 1.0) || !(w_abs_tol >= 0) || !(amin_min <= 1.0)) return MC_EINVAL;
+  d->opt.cond_max = cond_max; d->opt.amin_min = amin_min; d->dd_cond_max = dd_cond_max; d->w_abs_tol = w_abs_tol;
+  return MC_OK;
+}
 int64_t mc_diagram_blob(const mc_diagram *d, uint64_t *out, int64_t cap) {
   if (!d) return MC_EINVAL;
   int64_t n = (int64_t)d->blob.size();
@@ -119,7 +124,7 @@ int mc_integrate(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples,
   for (uint64_t done = 0; done < n_samples; done += mqk::CHUNK) {
     const uint64_t n = std::min<uint64_t>(mqk::CHUNK, n_samples - done);
     const int g1 = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + mqk::PTS_F64 - 1) / mqk::PTS_F64);
-    mq_launch_integrate_f64(d, g1, first_sample + done, n, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min, st);
+    mq_launch_integrate_f64(d, g1, first_sample + done, n, seed, d->prec(no_dd), st);
     int g2 = 0, g3 = 0;
     if (!no_dd) {     // second tier (double-double) and third tier (quad-double, only what the second could not resolve)
       g2 = d->grid_dd; mq_launch_integrate_dd(d, seed, st);
@@ -163,7 +168,7 @@ int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint6
     const int g1 = (int)std::min<uint64_t>(mqk::MAXGRID, (m + mqk::PTS_EVAL - 1) / mqk::PTS_EVAL);
     const bool list = f_out && !no_dd;
     mq_launch_reset(d, st);
-    mq_launch_eval_points(d, g1, first_sample + done, m, seed, no_dd ? INFINITY : d->opt.cond_max, no_dd ? -1.0 : d->opt.amin_min,
+    mq_launch_eval_points(d, g1, first_sample + done, m, seed, d->prec(no_dd),
                           z_out ? z_out + done * M : nullptr, order_out ? order_out + done * M : nullptr, p_out ? p_out + done : nullptr,
                           f_out ? f_out + done : nullptr, f64_out ? f64_out + done : nullptr, cond_out ? cond_out + done : nullptr,
                           flag_out ? flag_out + done : nullptr, list, st);
@@ -227,7 +232,7 @@ int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint6
   if (cudaMemset(b->d_mem, 0, off) != cudaSuccess) { mc_batch_free(b); return MC_ECUDA; }
   char *base = (char *)b->d_mem;
   std::vector<mqk::BatchDiag> dg(nd);
-  for (size_t i = 0; i < nd; i++) { dg[i].blob = diagrams[i]->d_blob; dg[i].cond_max = diagrams[i]->opt.cond_max; dg[i].amin_min = diagrams[i]->opt.amin_min; }
+  for (size_t i = 0; i < nd; i++) { dg[i].blob = diagrams[i]->d_blob; dg[i].pr = diagrams[i]->prec(false); }
   if (cudaMemcpy(base + o_dg, dg.data(), nd * sizeof(mqk::BatchDiag), cudaMemcpyHostToDevice) != cudaSuccess) { mc_batch_free(b); return MC_ECUDA; }
   mqk::BatchView &v = b->view;
   v.dg = (const mqk::BatchDiag *)(base + o_dg); v.nd = n_diagrams; v.cap = b->cap; v.ipd = 0;

@@ -229,10 +229,85 @@ template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
   }
 };
 
+// ---- looped pairings for c >= 3 in double-double -------------------------------------------------------------------
+// Fully unrolled, the (2c-1)!! pairings of c = 3, 4 make the double-double evaluator ~1 MB of straight-line code, far
+// beyond the instruction caches (ncu: "no instruction" was its largest stall). In double-double one coefficient costs
+// ~11 FP64 instructions, so a few integer instructions per pairing are free: the outer levels of the pairing recursion
+// become real loops over "pair the first free slot with the j-th later one", each iteration gathers the beta~ it needs
+// through a static position table (positions in the member's index bytes), and only the last level (three pairings of
+// four slots) is unrolled. Same pairing order as the canonical recursion, so the coefficient layout is unchanged.
+struct PairTbl3 { uint8_t p[5][7]; };            // c = 3: iteration j pairs slot 0 with slot j+1; [0] = that beta, [1..6] = ab ac ad bc bd cd of the other four
+struct PairTbl4 { uint8_t o[7]; uint8_t p[7][5][7]; };
+constexpr PairTbl3 make_tbl3() {
+  PairTbl3 t{};
+  for (int j = 0; j < 5; j++) {
+    int rest[4] = {0, 0, 0, 0}, n = 0;
+    for (int e = 1; e < 6; e++) if (e != j + 1) rest[n++] = e;
+    t.p[j][0] = (uint8_t)pair_index<6>(0, j + 1);
+    int k = 1;
+    for (int x = 0; x < 4; x++) for (int y = x + 1; y < 4; y++) t.p[j][k++] = (uint8_t)pair_index<6>(rest[x], rest[y]);
+  }
+  return t;
+}
+constexpr PairTbl4 make_tbl4() {
+  PairTbl4 t{};
+  for (int j1 = 0; j1 < 7; j1++) {
+    int r6[6] = {0, 0, 0, 0, 0, 0}, n = 0;
+    for (int e = 1; e < 8; e++) if (e != j1 + 1) r6[n++] = e;
+    t.o[j1] = (uint8_t)pair_index<8>(0, j1 + 1);
+    for (int j2 = 0; j2 < 5; j2++) {
+      int rest[4] = {0, 0, 0, 0}, m = 0;
+      for (int e = 1; e < 6; e++) if (e != j2 + 1) rest[m++] = r6[e];
+      t.p[j1][j2][0] = (uint8_t)pair_index<8>(r6[0], r6[j2 + 1]);
+      int k = 1;
+      for (int x = 0; x < 4; x++) for (int y = x + 1; y < 4; y++) t.p[j1][j2][k++] = (uint8_t)pair_index<8>(rest[x], rest[y]);
+    }
+  }
+  return t;
+}
+__constant__ PairTbl3 c_tbl3 = make_tbl3();
+__constant__ PairTbl4 c_tbl4 = make_tbl4();
+
+// the three pairings of four slots a<b<c<d, each with prefix weight wp: g = (ab, ac, ad, bc, bd, cd)
+template <class T, int KD>
+__device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, const T *r, T &sum) {
+  sum = mq_fma(mq_mul(mq_mul(wp, g[0]), g[5]), horner<T, KD>(s_coef, r), sum);     // (ab)(cd)
+  sum = mq_fma(mq_mul(mq_mul(wp, g[1]), g[4]), horner<T, KD>(s_coef, r), sum);     // (ac)(bd)
+  sum = mq_fma(mq_mul(mq_mul(wp, g[2]), g[3]), horner<T, KD>(s_coef, r), sum);     // (ad)(bc)
+}
+
 // s_idx: shared address of the index bytes; s_coef: of the coefficients; s_S: of this thread's S[0]; sstride: bytes per S index
 template <class T, int C, int KD>
 __device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
   constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
+  if constexpr (C >= 3 && sizeof(T) == sizeof(dd)) {
+    T r[KD > 0 ? KD : 1];
+#pragma unroll
+    for (int i = 0; i < KD; i++) r[i] = lds_T<T>(s_S + lds_u8(s_idx + NB + i) * sstride);
+    T sum = T(0.0);
+    if constexpr (C == 3) {
+#pragma unroll 1
+      for (int j = 0; j < 5; j++) {
+        T g[7];
+#pragma unroll
+        for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl3.p[j][k]) * sstride);
+        pair_body4<T, KD>(g[0], g + 1, s_coef, r, sum);
+      }
+    } else {
+#pragma unroll 1
+      for (int j1 = 0; j1 < 7; j1++) {
+        const T w1 = lds_T<T>(s_S + lds_u8(s_idx + c_tbl4.o[j1]) * sstride);
+#pragma unroll 1
+        for (int j2 = 0; j2 < 5; j2++) {
+          T g[7];
+#pragma unroll
+          for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl4.p[j1][j2][k]) * sstride);
+          pair_body4<T, KD>(mq_mul(w1, g[0]), g + 1, s_coef, r, sum);
+        }
+      }
+    }
+    return sum;
+  } else {
   uint64_t iw[NW > 2 ? NW : 2];
   iw[0] = w0; iw[1] = w1;                          // the first 16 index bytes were prefetched with the header
 #pragma unroll
@@ -245,6 +320,7 @@ __device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_id
   T sum = T(0.0);
   PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum);
   return sum;
+  }
 }
 
 template <class T>
