@@ -11,6 +11,9 @@
 
 namespace mqk {
 
+template <> __device__ __forceinline__ qd mq_shfl_xor<qd>(qd v, int m) {
+  return qd(__shfl_xor_sync(0xffffffffu, v.x[0], m), __shfl_xor_sync(0xffffffffu, v.x[1], m), __shfl_xor_sync(0xffffffffu, v.x[2], m), __shfl_xor_sync(0xffffffffu, v.x[3], m));
+}
 template <> __device__ __forceinline__ qd lds_T<qd>(uint32_t a) {
   const double2 lo = lds_f64x2(a), hi = lds_f64x2(a + 16);
   return qd(lo.x, lo.y, hi.x, hi.y);
@@ -18,23 +21,23 @@ template <> __device__ __forceinline__ qd lds_T<qd>(uint32_t a) {
 
 // Few points reach this tier (per-mille of the flagged ones), so the parallelism must come from inside a point: W_QD warps
 // share one group of 32 points and split its families (mcqed_kernels.cuh "warp split").
-constexpr int W_QD = 8, PTS_QD = 32, TPB_QD = W_QD * PTS_QD;
+constexpr int W_QD = 8, PTS_QD = 32 / MQ_WL, TPB_QD = W_QD * 32;   // per CTA: one group of 32 / MQ_WL points, MQ_WL lanes per point, W_QD warps
 
 // points listed in lost_list (sample indices) by the double-double pass
 __global__ void __launch_bounds__(TPB_QD) k_integrate_qd(const uint64_t *__restrict__ blob, uint64_t seed, double *partial,
                                                          const unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<qd, W_QD, 1> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_QD, 1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  const Roles<qd, W_QD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_QD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
   const unsigned long long cnt = counters[2] < LOSTCAP ? counters[2] : LOSTCAP;
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
   for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
-    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<false>(v, lost_list[i < cnt ? i : cnt - 1], seed, z, nullptr);
     qd f, a; double amin, xmin;
-    eval_integrand<qd, W_QD, false>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<qd, W_QD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
     if (bad_point(z, v.h->M, p) || !isfinite(fd)) atomicAdd(&counters[1], 1ull);     // dropped: w = 0
@@ -47,8 +50,8 @@ __global__ void __launch_bounds__(TPB_QD) k_integrate_qd(const uint64_t *__restr
 __global__ void __launch_bounds__(TPB_QD) k_batch_qd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item; __shared__ int s_d;
-  const Roles<qd, W_QD, 1> ro(smem_raw, scal_len);
-  StreamReader rd; setup_reader<W_QD, 1>(rd, smem_raw, scal_len, sizeof(qd));
+  const Roles<qd, W_QD, MQ_WL> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<W_QD, MQ_WL>(rd, smem_raw, scal_len, sizeof(qd));
   const uint32_t total = bv.qd_start[bv.nd];
   for (;;) {
     __syncthreads();
@@ -59,12 +62,12 @@ __global__ void __launch_bounds__(TPB_QD) k_batch_qd(BatchView bv, uint64_t firs
     const int d = s_d;
     const DiagView v = make_view(bv.dg[d].blob);
     const unsigned long long cnt = bv.nlost[d] < bv.lostcap ? bv.nlost[d] : bv.lostcap;
-    const unsigned long long i = (unsigned long long)(item - bv.qd_start[d]) * PTS_QD + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    const unsigned long long i = (unsigned long long)(item - bv.qd_start[d]) * PTS_QD + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
     const uint32_t rel = bv.lost_list[(size_t)d * bv.lostcap + (i < cnt ? i : cnt - 1)];
     double z[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<false>(v, first + rel, seed, z, nullptr);
     qd f, a; double amin, xmin;
-    eval_integrand<qd, W_QD, false>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<qd, W_QD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
@@ -80,16 +83,16 @@ __global__ void __launch_bounds__(TPB_QD) k_eval_points_qd(const uint64_t *__res
                                                            const unsigned long long *lost_list, const unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<qd, W_QD, 1> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_QD, 1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  const Roles<qd, W_QD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_QD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
   const unsigned long long cnt = counters[2] < LOSTCAP ? counters[2] : LOSTCAP;
   for (unsigned long long base = (unsigned long long)blockIdx.x * ro.P; base < cnt; base += (unsigned long long)gridDim.x * ro.P) {
-    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0;
+    const unsigned long long i = base + ro.slot; const bool live = i < cnt && ro.gw == 0 && ro.sub == 0;
     double z[MQ_MAXM];
     const unsigned long long rel = lost_list[i < cnt ? i : cnt - 1];
     if (ro.gw == 0) draw_point<false>(v, first + rel, seed, z, nullptr);
     qd f, a; double amin, xmin;
-    eval_integrand<qd, W_QD, false>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<qd, W_QD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) f_out[rel] = mq_to_double(f);
   }
 }
@@ -97,15 +100,15 @@ __global__ void __launch_bounds__(TPB_QD) k_eval_z_qd(const uint64_t *__restrict
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  const Roles<qd, W_QD, 1> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_QD, 1>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
+  const Roles<qd, W_QD, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_QD, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(qd));
   for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const bool live = base + ro.slot < n && ro.gw == 0;
+    const bool live = base + ro.slot < n && ro.gw == 0 && ro.sub == 0;
     const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     qd f, a; double amin, xmin;
-    eval_integrand<qd, W_QD, false>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<qd, W_QD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) fqd_out[i] = mq_to_double(f);
   }
 }
@@ -115,7 +118,7 @@ __global__ void __launch_bounds__(TPB_QD) k_eval_z_qd(const uint64_t *__restrict
 using namespace mqk;
 
 int mq_config_qd(mc_diagram *d) {
-  d->smem_qd = smem_bytes(d->max_scal_len, TPB_QD, sizeof(qd), W_QD, 1);
+  d->smem_qd = smem_bytes(d->max_scal_len, TPB_QD, sizeof(qd), W_QD, MQ_WL);
   cudaError_t e;
   if ((e = allow_max_smem(k_integrate_qd)) != cudaSuccess) return (int)e;
   if ((e = allow_max_smem(k_eval_points_qd)) != cudaSuccess) return (int)e;
@@ -152,7 +155,7 @@ int mq_batch_config_qd(size_t smem, int *grid) {
   *grid = nsm * occ;
   return 0;
 }
-size_t mq_batch_smem_qd(int scal_len) { return smem_bytes(scal_len, TPB_QD, sizeof(qd), W_QD, 1); }
+size_t mq_batch_smem_qd(int scal_len) { return smem_bytes(scal_len, TPB_QD, sizeof(qd), W_QD, MQ_WL); }
 void mq_launch_batch_qd(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st) {
   k_batch_qd<<<grid, TPB_QD, smem, (cudaStream_t)st>>>(bv, first, seed, scal_len);
 }

@@ -276,6 +276,17 @@ __device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, c
   sum = mq_fma(mq_mul(mq_mul(wp, g[2]), g[3]), horner<T, KD>(s_coef, r), sum);     // (ad)(bc)
 }
 
+// byte i (compile-time) of an array of 64-bit index words: one PRMT
+template <int I> __device__ __forceinline__ uint32_t idx_byte(const uint64_t *iw) {
+  const uint32_t w = (I & 4) ? (uint32_t)(iw[I >> 3] >> 32) : (uint32_t)iw[I >> 3];
+  return __byte_perm(w, 0u, 0x4440u | (uint32_t)(I & 3));
+}
+template <class T, int N, int OFF, int I = 0> struct Gather {
+  static __device__ __forceinline__ void run(const uint64_t *iw, uint32_t s_S, uint32_t sstride, T *out) {
+    if constexpr (I < N) { out[I] = lds_T<T>(s_S + idx_byte<OFF + I>(iw) * sstride); Gather<T, N, OFF, I + 1>::run(iw, s_S, sstride, out); }
+  }
+};
+
 // s_idx: shared address of the index bytes; s_coef: of the coefficients; s_S: of this thread's S[0]; sstride: bytes per S index
 template <class T, int C, int KD>
 __device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
@@ -313,10 +324,8 @@ __device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_id
 #pragma unroll
   for (int k = 2; k < NW; k++) iw[k] = lds_u64(s_idx + 8 * k);
   T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
-#pragma unroll
-  for (int i = 0; i < NB; i++) b[i] = lds_T<T>(s_S + (uint32_t)((iw[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
-#pragma unroll
-  for (int i = 0; i < KD; i++) r[i] = lds_T<T>(s_S + (uint32_t)((iw[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
+  Gather<T, NB, 0>::run(iw, s_S, sstride, b);
+  Gather<T, KD, NB>::run(iw, s_S, sstride, r);
   T sum = T(0.0);
   PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum);
   return sum;
@@ -348,16 +357,10 @@ __device__ __forceinline__ void family_eval2(const uint64_t *w, uint32_t s_idxA,
 #pragma unroll
   for (int k = 2; k < NW; k++) { iwA[k] = lds_u64(s_idxA + 8 * k); iwB[k] = lds_u64(s_idxB + 8 * k); }
   double bA[NB > 0 ? NB : 1], rA[KD > 0 ? KD : 1], bB[NB > 0 ? NB : 1], rB[KD > 0 ? KD : 1];
-#pragma unroll
-  for (int i = 0; i < NB; i++) {
-    bA[i] = lds_f64(s_S + (uint32_t)((iwA[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
-    bB[i] = lds_f64(s_S + (uint32_t)((iwB[i >> 3] >> (8 * (i & 7))) & 0xff) * sstride);
-  }
-#pragma unroll
-  for (int i = 0; i < KD; i++) {
-    rA[i] = lds_f64(s_S + (uint32_t)((iwA[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
-    rB[i] = lds_f64(s_S + (uint32_t)((iwB[(NB + i) >> 3] >> (8 * ((NB + i) & 7))) & 0xff) * sstride);
-  }
+  Gather<double, NB, 0>::run(iwA, s_S, sstride, bA);
+  Gather<double, NB, 0>::run(iwB, s_S, sstride, bB);
+  Gather<double, KD, NB>::run(iwA, s_S, sstride, rA);
+  Gather<double, KD, NB>::run(iwB, s_S, sstride, rB);
   double sumA = 0.0, sumB = 0.0;
   PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA);
   PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB);
@@ -527,9 +530,10 @@ template <> __device__ __forceinline__ double mq_shfl_xor<double>(double v, int 
 template <> __device__ __forceinline__ dd mq_shfl_xor<dd>(dd v, int m) { return dd(__shfl_xor_sync(0xffffffffu, v.hi, m), __shfl_xor_sync(0xffffffffu, v.lo, m)); }
 
 template <class T, int W, bool LANES>
-__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd, const double *z, T *S, int stride, T *xT, double *xA, int gw, int sub,
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const double *z, T *S, int stride, T *xT, double *xA, int gw, int sub,
                                             T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
   constexpr bool TRACK = true;
+  StreamReader rd = rd_io;                             // work on a register copy (the caller's object lives in local memory across this call)
   const DevHeader &h = *v.h;
   T nodeval[/*worst case*/ 1024];
   double nodeabs[TRACK ? 1024 : 1];
@@ -721,6 +725,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd,
     }
   }
   f_out = f; abs_out = asum; amin_out = amin; xmin_out = xmin;
+  rd_io = rd;
 }
 
 }  // namespace mqk
