@@ -175,8 +175,8 @@ class Diagram:
     def set_flags(self, flags):
         _check(lib().mc_diagram_set_flags(self.h, flags), "mc_diagram_set_flags")
 
-    def set_dd_limit(self, dd_cond_max):
-        _check(lib().mc_diagram_set_dd_limit(self.h, dd_cond_max), "mc_diagram_set_precision")
+    def set_precision(self, cond_max=1e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=1e-10):
+        _check(lib().mc_diagram_set_precision(self.h, cond_max, amin_min, dd_cond_max, w_abs_tol), "mc_diagram_set_precision")
 
     def blob(self):
         n = lib().mc_diagram_blob(self.h, None, 0)

@@ -15,6 +15,10 @@
 
 namespace mqk {
 
+#ifndef MQ_DUAL
+#define MQ_DUAL 1     // binary64: evaluate two consecutive same-shape entries together (independent chains)
+#endif
+
 struct DiagView {
   const uint64_t *blob; const DevHeader *h; const double *Z, *invdeg;
   const DevGeom *geom; const DevTable *tab; const DevNode *node; const DevTerm *term;
@@ -583,7 +587,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         if (havenext) { hdn = lds_u64(an); if constexpr (LANES) fetch_member(an, hdn, sub, hln, n0, n1); }
         // pair this entry with the next one if it has the same shape (binary64: doubles the ILP of the warp)
         bool dual = false;
-        if constexpr (sizeof(T) == sizeof(double) && LANES) {
+        if constexpr (sizeof(T) == sizeof(double) && LANES && MQ_DUAL) {
           if (havenext && left > 1 && c <= 3 && (int)(hdn & 63) == (int)(hd & 63)) {
             const int size2 = MQ_WL * (1 + (int)(hdn >> 16 & 0xFFFF)) + (int)(uint32_t)(hdn >> 32);
             dual = npos + size2 <= MQ_CHUNK_WORDS;
@@ -595,6 +599,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         auto account = [&](T val, uint64_t ml, uint32_t sidx) {
           const int ns = (int)(ml >> 10 & 15), keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
           val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
+#pragma unroll 1
           for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(sidx + nb + i) * sstride);
           if (keyk != key) {
             if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }

@@ -59,6 +59,13 @@ def test_no_cpu_fallback(mc):
     with pytest.raises(mc.McError) as ei:      # a host-only handle never computes
         d.integrate_host(0, 10, 1)
     assert ei.value.code == mc.MC_EINVAL
+    with pytest.raises(mc.McError) as ei:      # neither does a batch built on one (no device: MC_ECUDA before the handles are looked at)
+        mc.Batch([d], 1024)
+    assert ei.value.code in (mc.MC_EINVAL, mc.MC_ECUDA)
+    with pytest.raises(mc.McError) as ei:      # precision thresholds are validated on the host
+        d.set_precision(cond_max=-1.0)
+    assert ei.value.code == mc.MC_EINVAL
+    d.set_precision(cond_max=1e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=0.0)
     if not _has_cuda():
         with pytest.raises(mc.McError) as ei:
             mc.Diagram(1, 1, [(0, 2)])
