@@ -289,7 +289,7 @@ void mq_launch_batch_f64(const BatchView &bv, int grid, size_t smem, uint64_t fi
 void mq_launch_batch_compact(const BatchView &bv, mq_stream st) { k_batch_compact<<<bv.nd, 128, 0, (cudaStream_t)st>>>(bv); }
 void mq_launch_batch_ranges(const BatchView &bv, int tier, mq_stream st) {
   if (tier == 1) k_batch_ranges<<<1, 1, 0, (cudaStream_t)st>>>(bv.nflag, ~0ull, bv.nd, (unsigned)PTS_DD, bv.dd_start, bv.queue + 1);
-  else k_batch_ranges<<<1, 1, 0, (cudaStream_t)st>>>(bv.nlost, (unsigned long long)bv.lostcap, bv.nd, (unsigned)(32 / MQ_WL), bv.qd_start, bv.queue + 2);
+  else k_batch_ranges<<<1, 1, 0, (cudaStream_t)st>>>(bv.nlost, (unsigned long long)bv.lostcap, bv.nd, 1u, bv.qd_start, bv.queue + 2);   // quad-double items are single points
 }
 void mq_launch_batch_finish(const BatchView &bv, int tiers, double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st) {
   k_batch_finish<<<(bv.nd + 127) / 128, 128, 0, (cudaStream_t)st>>>(bv, tiers, out_sum, out_sumsq, out_nflag, out_ndrop);

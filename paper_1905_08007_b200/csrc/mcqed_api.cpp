@@ -221,7 +221,7 @@ int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint6
   const size_t P = mqk::PTS_F64, nd = (size_t)n_diagrams;
   b->cap = (uint32_t)((max_samples_per_call + P - 1) / P * P);
   b->lostcap = std::max<uint32_t>(1024u, b->cap / 8);
-  const size_t ipd = b->cap / P, idd = (size_t)b->cap / mqk::PTS_DD + 1, iqd = (size_t)b->lostcap / (32 / MQ_WL) + 1;
+  const size_t ipd = b->cap / P, idd = (size_t)b->cap / mqk::PTS_DD + 1, iqd = (size_t)b->lostcap + 1;
   // carve one allocation (every array 256-byte aligned)
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };

@@ -353,11 +353,11 @@ __device__ __noinline__ T family_dispatch(int ckd, uint64_t w0, uint64_t w1, uin
 // Two consecutive families of the same shape evaluated together: their arithmetic chains are independent, which
 // doubles the instruction-level parallelism of a warp at unchanged shared-memory footprint (binary64 only).
 template <int C, int KD>
-__device__ __forceinline__ void family_eval2(const uint64_t *w, uint32_t s_idxA, uint32_t s_coefA, uint32_t s_idxB, uint32_t s_coefB,
-                                             uint32_t s_S, uint32_t sstride, double &outA, double &outB) {
+__device__ __forceinline__ double2 family_eval2(uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
+                                                uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
   constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
   uint64_t iwA[NW > 2 ? NW : 2], iwB[NW > 2 ? NW : 2];
-  iwA[0] = w[0]; iwA[1] = w[1]; iwB[0] = w[2]; iwB[1] = w[3];
+  iwA[0] = wA0; iwA[1] = wA1; iwB[0] = wB0; iwB[1] = wB1;
 #pragma unroll
   for (int k = 2; k < NW; k++) { iwA[k] = lds_u64(s_idxA + 8 * k); iwB[k] = lds_u64(s_idxB + 8 * k); }
   double bA[NB > 0 ? NB : 1], rA[KD > 0 ? KD : 1], bB[NB > 0 ? NB : 1], rB[KD > 0 ? KD : 1];
@@ -368,18 +368,20 @@ __device__ __forceinline__ void family_eval2(const uint64_t *w, uint32_t s_idxA,
   double sumA = 0.0, sumB = 0.0;
   PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA);
   PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB);
-  outA = sumA; outB = sumB;
+  return make_double2(sumA, sumB);
 }
-static __device__ __noinline__ void family_dispatch2(int ckd, const uint64_t *w, uint32_t s_idxA, uint32_t s_coefA, uint32_t s_idxB, uint32_t s_coefB,
-                                              uint32_t s_S, uint32_t sstride, double &outA, double &outB) {
+// arguments and results in registers (no stack traffic across the call)
+static __device__ __noinline__ double2 family_dispatch2(int ckd, uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
+                                                        uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
   switch (ckd) {
-#define MQ_CASE(C, K) case C * 8 + K: family_eval2<C, K>(w, s_idxA, s_coefA, s_idxB, s_coefB, s_S, sstride, outA, outB); return;
+#define MQ_CASE(C, K) case C * 8 + K: return family_eval2<C, K>(wA0, wA1, wB0, wB1, s_idxA, s_coefA, s_idxB, s_coefB, s_S, sstride);
 #define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
     MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3)
 #undef MQ_ROW
 #undef MQ_CASE
   }
   __trap();
+  return make_double2(0.0, 0.0);
 }
 
 // Loop-based family evaluation for wide types (quad-double): same arithmetic as family_eval, no unrolling.
@@ -411,6 +413,47 @@ __device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t
     if (level == c - 1) { sum = sum + wn * horner_at(s_coef); s_coef += 8 * MQ_WL * nblk; }
     else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
   }
+  return sum;
+}
+
+// Entry-parallel family evaluation (quad-double tier): member m of the stream entry at ent (GLOBAL memory), scalars from
+// S[index * stride] (shared). Same arithmetic and pairing order as family_generic; the scalar factors are applied here and
+// the accumulation key (output, pattern, grade) of the member is returned in key.
+template <class T>
+__device__ __noinline__ T family_spread(const uint64_t *ent, uint64_t hd, int m, const T *S, int stride, int &key) {
+  const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7), idxw = (int)(hd >> 16 & 0xFFFF);
+  const uint64_t ml = ent[m];
+  const uint8_t *idx = reinterpret_cast<const uint8_t *>(ent + MQ_WL + (size_t)idxw * m);
+  const double *coef = reinterpret_cast<const double *>(ent + MQ_WL * (1 + idxw)) + (kd ? 2 : 1) * m;
+  key = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
+  const int n2 = 2 * c, nb = c * (2 * c - 1), nblk = 1 << kd, ns = (int)(ml >> 10 & 15);
+  T b[28], r[4], v[8];
+  for (int i = 0; i < nb; i++) b[i] = S[(int)idx[i] * stride];
+  for (int i = 0; i < kd; i++) r[i] = S[(int)idx[nb + i] * stride];
+  auto horner_at = [&](const double *a) -> T {
+    if (kd == 0) return T(a[0]);
+    const int H = 1 << (kd - 1);
+    for (int j = 0; j < H; j++) v[j] = mq_fma_c(a[2 * MQ_WL * j + 1], r[kd - 1], a[2 * MQ_WL * j], T());
+    for (int i = kd - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
+    return v[0];
+  };
+  T sum = T(0.0);
+  if (c == 0) sum = horner_at(coef);
+  else {
+    T w[5]; unsigned used[5]; int scur[5];
+    int level = 0; used[0] = 0u; w[0] = T(1.0); scur[0] = -1;
+    while (level >= 0) {
+      const unsigned u = used[level]; const int f = __ffs(~u) - 1;
+      int s2 = scur[level] < 0 ? f + 1 : scur[level] + 1;
+      while (s2 < n2 && (u >> s2 & 1u)) s2++;
+      if (s2 >= n2) { level--; continue; }
+      scur[level] = s2;
+      const T wn = w[level] * b[f * n2 - f * (f + 1) / 2 + (s2 - f - 1)];
+      if (level == c - 1) { sum = sum + wn * horner_at(coef); coef += MQ_WL * nblk; }
+      else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
+    }
+  }
+  for (int i = 0; i < ns; i++) sum = sum * S[(int)idx[nb + kd + i] * stride];
   return sum;
 }
 
@@ -533,7 +576,7 @@ template <class T> __device__ __forceinline__ T mq_shfl_xor(T v, int m);
 template <> __device__ __forceinline__ double mq_shfl_xor<double>(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 template <> __device__ __forceinline__ dd mq_shfl_xor<dd>(dd v, int m) { return dd(__shfl_xor_sync(0xffffffffu, v.hi, m), __shfl_xor_sync(0xffffffffu, v.lo, m)); }
 
-template <class T, int W, bool LANES>
+template <class T, int W, bool LANES, bool SPREAD = false>
 __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const double *z, T *S, int stride, T *xT, double *xA, int gw, int sub,
                                             T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
   constexpr bool TRACK = true;
@@ -549,8 +592,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
     const DevGeom &g = v.geom[gi];
     T U = T(1.0), V = T(0.0), G = T(1.0);
     if constexpr (LANES) __syncwarp();                 // every lane role has finished reading S of the previous piece
-    if (gw == 0) piece_scalars<T>(g, z, S, stride, sub == 0, U, V, G, amin, xmin);
-    if constexpr (W > 1) __syncthreads();              // S of this piece is complete before any warp gathers from it
+    if constexpr (SPREAD) __syncthreads();             // (entry-parallel) nobody still reads S of the previous piece
+    if (gw == 0) piece_scalars<T>(g, z, S, stride, SPREAD ? threadIdx.x == 0 : sub == 0, U, V, G, amin, xmin);
+    if constexpr (W > 1 || SPREAD) __syncthreads();              // S of this piece is complete before any warp gathers from it
     else if constexpr (LANES) __syncwarp();
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
@@ -562,6 +606,52 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = 0.0; }
       // entries of this table from the staged stream; a run of families with the same (output, pattern, grade)
       // accumulates in registers and is flushed when the key changes
+      if constexpr (SPREAD) {
+        // entry-parallel: the whole CTA works on ONE point; every thread walks the staged stream (headers only), takes the
+        // entries with index = its thread id (mod CTA size) and evaluates them from global memory once a full round is dealt
+        const uint64_t *pend = nullptr; uint64_t pend_h = 0;
+        auto flush_round = [&]() {
+          if (pend) {
+#pragma unroll 1
+            for (int m = 0; m < MQ_WL; m++) {
+              int kk;
+              const T val = family_spread<T>(pend, pend_h, m, S, stride, kk);
+              N[kk >> 7][(kk >> 3) & 15][kk & 7] = N[kk >> 7][(kk >> 3) & 15][kk & 7] + val;
+              if constexpr (TRACK) Na[kk >> 7][(kk >> 3) & 15][kk & 7] += fabs(mq_to_double(val));
+            }
+            pend = nullptr;
+          }
+        };
+        unsigned unit = 0;
+        for (int left = tb.nfam; left > 0;) {
+          if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
+          const uint64_t hd = lds_u64(rd.addr());
+          const int idxw = (int)(hd >> 16 & 0xFFFF);
+          if ((int)(hd & 7) == MQ_PAD_MARK) { rd.pos += 1 + idxw; continue; }
+          if (unit % blockDim.x == threadIdx.x) { pend = rd.gsrc + (size_t)rd.chunk * MQ_CHUNK_WORDS + rd.pos; pend_h = hd; }
+          rd.pos += MQ_WL * (1 + idxw) + (int)(uint32_t)(hd >> 32); left--; unit++;
+          if (unit % blockDim.x == 0) flush_round();
+        }
+        flush_round();
+        // CTA-wide sum of the partial graded sums: warp butterflies, then the warp totals through xT / xA; every thread ends
+        // with the same totals
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        const int ne = tb.nout * npat * MQ_NGRADE;
+        for (int e = 0; e < ne; e++) {
+          const int o = e / (npat * MQ_NGRADE), p = (e / MQ_NGRADE) % npat, c = e % MQ_NGRADE;
+          T t = N[o][p][c]; double ta = Na[o][p][c];
+          for (int m = 1; m < 32; m <<= 1) { t = t + mq_shfl_xor<T>(t, m); ta += __shfl_xor_sync(0xffffffffu, ta, m); }
+          if (lane == 0) { xT[wid * ne + e] = t; xA[wid * ne + e] = ta; }
+        }
+        __syncthreads();
+        for (int e = 0; e < ne; e++) {
+          const int o = e / (npat * MQ_NGRADE), p = (e / MQ_NGRADE) % npat, c = e % MQ_NGRADE;
+          T t = xT[e]; double ta = xA[e];
+          for (int w = 1; w < nw; w++) { t = t + xT[w * ne + e]; ta += xA[w * ne + e]; }
+          N[o][p][c] = t; Na[o][p][c] = ta;
+        }
+        __syncthreads();
+      } else {
       int key = -1; T racc = T(0.0); double racca = 0.0;
       bool have = false; uint32_t a0 = 0; uint64_t hd = 0, hl = 0, w0 = 0, w1 = 0;   // entry header, this lane's member header + first index words
       int unit = 0;                                                                  // evaluation units are dealt round-robin to the W warps
@@ -616,13 +706,11 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             const bool have3 = npos2 < MQ_CHUNK_WORDS;
             if (have3) { hd3 = lds_u64(a2); fetch_member(a2, hd3, sub, hl3, m0, m1); }
             if (W == 1 || unit % W == gw) {
-              const uint64_t w4[4] = {w0, w1, n0, n1};
               const uint32_t sidxA = a0 + 8 * MQ_WL + 8 * idxw * sub, sidxB = an + 8 * MQ_WL + 8 * idxw2 * sub;
-              double vA, vB;
-              family_dispatch2(c * 8 + kd, w4, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub, sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub,
-                               s_S, sstride, vA, vB);
-              account(T(vA), hl, sidxA);
-              account(T(vB), hln, sidxB);
+              const double2 vAB = family_dispatch2(c * 8 + kd, w0, w1, n0, n1, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub,
+                                                   sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub, s_S, sstride);
+              account(T(vAB.x), hl, sidxA);
+              account(T(vAB.y), hln, sidxB);
             }
             unit++;
             rd.pos = npos2; left -= 2;
@@ -647,6 +735,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         have = havenext; a0 = an; hd = hdn; hl = hln; w0 = n0; w1 = n1;
       }
       if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
+      }
       if constexpr (LANES && MQ_WL > 1) {              // add the partial sums of the lane roles: afterwards every lane holds the totals
         for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
