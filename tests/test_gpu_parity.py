@@ -269,3 +269,68 @@ def test_batched_path_equals_per_diagram_path(po, mc):
     b.close()
     for d in ds:
         d.close()
+
+
+def test_bench_launch_configuration_five_loop(mc):
+    """BASELINE.json configs[4] in the launch configuration bench.py times (mc_batch_integrate, 37888 points per graph and
+    pass, 5-loop graphs of the seeded set): properties that hold at any size, and the per-diagram path on sampled graphs.
+    Per-point parity of 5-loop values against the oracle is test_five_loop_points_against_stored_oracle_values."""
+    from paper_1905_08007_b200 import workloads
+    st = torch.cuda.current_stream().cuda_stream
+    graphs = workloads.config_graphs(4)[::23]                      # 12 of the 256 graphs, spread over the classes
+    ds = [mc.Diagram(g[0], g[1], g[2]) for _, g in graphs]
+    B, seed = 37888, workloads.CONFIG_SEED[4]
+    b = mc.Batch(ds, B)
+    s1, s2, nf, nd = b.integrate_host(0, B, seed, st)
+    t1, t2, mf, md = b.integrate_host(0, B, seed, st)
+    assert np.array_equal(s1, t1) and np.array_equal(s2, t2) and np.array_equal(nf, mf)     # bit-deterministic
+    assert not nd.any() and np.all(nf <= B) and np.all(np.isfinite(s1)) and np.all(s2 > 0)
+    # additivity over disjoint sample ranges (the checkpoint / sharding story): two half passes = one pass
+    h1 = b.integrate_host(0, B // 2, seed, st)
+    h2 = b.integrate_host(B // 2, B - B // 2, seed, st)
+    assert np.array_equal(h1[2] + h2[2], nf)
+    assert np.all(np.abs(h1[0] + h2[0] - s1) <= 1e-12 * np.sqrt(B * s2))
+    # the per-diagram entry point on sampled graphs of the set
+    for k in (0, 5, 11):
+        r1, r2, rf, rd = ds[k].integrate_host(0, B, seed, st)
+        assert rf == nf[k] and rd == 0
+        assert abs(r1 - s1[k]) <= 1e-12 * math.sqrt(B * r2) and abs(r2 - s2[k]) <= 1e-12 * r2
+    # the absolute acceptance criterion changes the sums by less than its own bound (w_abs_tol per point)
+    for d in ds[:3]:
+        d.set_precision(w_abs_tol=0.0)
+    b2 = mc.Batch(ds[:3], B)
+    u1, u2, uf, ud = b2.integrate_host(0, B, seed, st)
+    assert np.all(uf >= nf[:3]) and np.all(np.abs(u1 - s1[:3]) <= 1e-10 * B)
+    b.close(); b2.close()
+    for d in ds:
+        d.close()
+
+
+def test_two_loop_full_size_against_paper_value_and_stored_oracle_run(mc):
+    """BASELINE.json configs[1] at full size: the six 2-loop graphs, 1e8 points each, seed 2. The sum must reproduce
+    A1^(4) without lepton loops = -0.344166 (north_star) within the statistical error, and every graph must agree with the
+    oracle's own 1e8-point run on the SAME points (tests/golden/oracle_two_loop_mc.txt, written by the oracle alone) far
+    inside one sigma (the oracle run keeps binary64 values at ill-conditioned points, hence not bit-equal sums)."""
+    from conftest import read_golden
+    rows = read_golden("oracle_two_loop_mc.txt")
+    st = torch.cuda.current_stream().cuda_stream
+    n = 100_000_000
+    ds, ref = [], []
+    for e, ch, k, m, nn, npts, mean, sig in rows:
+        assert int(npts) == n
+        chords = [(int(ch[2 * i]), int(ch[2 * i + 1])) for i in range(len(ch) // 2)]
+        ds.append(mc.Diagram(2, int(e), chords, deg_floor=0.5))          # the stored run used Deg floor 0.5
+        ref.append((float(mean), float(sig)))
+    b = mc.Batch(ds, 1 << 22)
+    s1, s2, nf, nd = b.integrate_host(0, n, 2, st)
+    assert not nd.any()
+    mean = s1 / n
+    err = np.sqrt(np.maximum(s2 / n - mean * mean, 0.0) / n)
+    for k, (m0, e0) in enumerate(ref):
+        assert abs(err[k] - e0) <= 0.02 * e0, (k, err[k], e0)
+        assert abs(mean[k] - m0) <= 0.05 * e0, (k, mean[k], m0, e0)       # same points: far inside one sigma
+    total, sigma = float(mean.sum()), float(np.sqrt((err ** 2).sum()))
+    assert sigma < 5e-4 and abs(total + 0.344166) <= 3.0 * sigma, (total, sigma)
+    b.close()
+    for d in ds:
+        d.close()
