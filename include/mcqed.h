@@ -54,11 +54,9 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {0.5, 1e30, 4096.0, 1e-5, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5).
- * Precision flag (O8): a point is re-evaluated in double-double when
- *   sum_terms sum_grades |contribution| > cond_max * |f|,  or  min over electron lines of every piece of
- *   A_t = 1 - x_t is below amin_min (the scalar currents lose relative accuracy like eps/A_t),  or
- *   anything is non-finite / some z_l < 2^-600.
+/* NULL => defaults {0.75, 1e30, 3e4, 1e-2, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5).
+ * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
+ *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.
  * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0).
  * flags bit 1: build no numerator tables (introspection of the combinatorics only; host handles). */
 typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; } mc_options;
@@ -98,16 +96,18 @@ int mc_diagram_sampler_tables(const mc_diagram *, double *deg, double *Z, double
 int mc_diagram_set_flags(mc_diagram *, uint32_t flags);
 
 /* Precision policy of an existing handle (O8; "interval arithmetic ... with different precisions":
- * the paper gives no thresholds). Every tier carries a = sum |contribution| next to f and inner = the smallest |A_t|, g_t and
- * pivot ratio of the point. A tier's value is ACCEPTED if
- *   (relative) a <= cond * |f| and inner >= inner_min, with (cond, inner_min) = (cond_max, amin_min) in binary64 (then
- *              |df| <= 1e-10 |f|) and (dd_cond_max, 1/dd_cond_max) in double-double, or
- *   (absolute) 64 ulp * a / min(1, inner) <= w_abs_tol * p: the round-off bound on the WEIGHT w = f/p is below
- *              w_abs_tol. The Monte Carlo sums need absolute accuracy of the weights; deep in the corners of the simplex the
- *              subtracted integrand loses all relative precision while f/p is 1e-20 and smaller.
- * Otherwise the point goes to the next tier (binary64 -> double-double -> quad-double). Defaults: cond_max, amin_min from
- * mc_options; dd_cond_max = 1e26; w_abs_tol = 1e-10 (0 switches the absolute criterion off). A batch copies the values
- * when it is created. HOST. MC_EINVAL on cond_max <= 0, dd_cond_max < 1, w_abs_tol < 0. */
+ * the paper gives no thresholds). Every tier carries next to f a running bound a on the sum of |monomial| (it sees the
+ * cancellation between terms, pieces, families, pairings and inside a coefficient block), amin = the smallest |A_t| and
+ * xmin = the smallest pivot ratio / g_t of the point. A tier's value is ACCEPTED if
+ *   (relative) a <= cond * |f| and min(amin, xmin) >= inner_min, with (cond, inner_min) = (cond_max, amin_min) in binary64
+ *              (then |df| <= 1e-10 |f|) and (dd_cond_max, 1/dd_cond_max) in double-double, or
+ *   (absolute) unit * a <= w_abs_tol * p * min(1, xmin), unit = 32 ulp of the tier's arithmetic (64 in double-double): the
+ *              round-off bound on the WEIGHT w = f/p is below w_abs_tol. The Monte Carlo sums need absolute accuracy of the
+ *              weights; deep in the corners of the simplex the subtracted integrand loses all relative precision while f/p
+ *              is 1e-20 and smaller.
+ * Otherwise the point goes to the next tier (binary64 -> double-double -> quad-double). Defaults: cond_max = 3e4, amin_min =
+ * 1e-2 (mc_options); dd_cond_max = 1e26; w_abs_tol = 1e-10 (0 switches the absolute criterion off). A batch copies the
+ * values when it is created. HOST. MC_EINVAL on cond_max <= 0, dd_cond_max < 1, w_abs_tol < 0. */
 int mc_diagram_set_precision(mc_diagram *, double cond_max, double amin_min, double dd_cond_max, double w_abs_tol);
 
 /* Host copy of the device table blob (layout: csrc/device_layout.h), for format tests. Returns the

@@ -117,7 +117,7 @@ def make_graph(loops, ext_pos, chords):
 class Diagram:
     """RAII handle around mc_diagram*"""
 
-    def __init__(self, loops, ext_pos, chords, deg_floor=0.75, deg_cap=1e30, cond_max=1e4, amin_min=1e-2, flags=0, host_only=False, forests=None):
+    def __init__(self, loops, ext_pos, chords, deg_floor=0.75, deg_cap=1e30, cond_max=3e4, amin_min=1e-2, flags=0, host_only=False, forests=None):
         self.loops, self.M = loops, 3 * loops
         g = make_graph(loops, ext_pos, chords)
         opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags)
@@ -175,7 +175,7 @@ class Diagram:
     def set_flags(self, flags):
         _check(lib().mc_diagram_set_flags(self.h, flags), "mc_diagram_set_flags")
 
-    def set_precision(self, cond_max=1e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=1e-10):
+    def set_precision(self, cond_max=3e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=1e-10):
         _check(lib().mc_diagram_set_precision(self.h, cond_max, amin_min, dd_cond_max, w_abs_tol), "mc_diagram_set_precision")
 
     def blob(self):

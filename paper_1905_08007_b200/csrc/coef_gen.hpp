@@ -32,8 +32,8 @@ struct Family {
   int c = 0, kd = 0, pattern = 0, out = 0;
   std::vector<uint8_t> paired, inner;
   std::vector<uint8_t> scal;       // kind<<4 | slot
-  std::vector<double> coef;        // stream order (see device_layout.h)
-  int64_t nonzero = 0;
+  std::vector<double> coef;        // stream order (see device_layout.h), incl. the closing (sum |c|, -) unit of every kd >= 3 block
+  int64_t nonzero = 0, n_coef = 0; // non-zero / stored numerator coefficients (closing units not counted)
 };
 struct TableBuild { int nout = 1; std::vector<Family> fams; int64_t n_stored = 0, n_nonzero = 0; };
 
@@ -263,10 +263,16 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
         for (size_t pi = 0; pi < npair; pi++) {
           const double *src = &cm[((size_t)out * npair + pi) * nsig];
           auto at = [&](size_t si) { return src[so | (si << ko)]; };   // outer bits low, inner bits high
-          if (kd == 0) f.coef.push_back(at(0));
-          else for (size_t jj = 0; jj < half; jj++) { f.coef.push_back(at(jj)); f.coef.push_back(at(jj + half)); }
+          if (kd == 0) { f.coef.push_back(at(0)); f.n_coef++; if (at(0) != 0.0) f.nonzero++; continue; }
+          if (kd <= 4) for (size_t jj = 0; jj < half; jj++) { f.coef.push_back(at(jj)); f.coef.push_back(at(jj + half)); }
+          else for (size_t top = 0; top < (ninner >> 4); top++)          // kd = 5, 6: sub-blocks of kd = 4, top bits ascending
+            for (size_t jj = 0; jj < 8; jj++) { f.coef.push_back(at(top << 4 | jj)); f.coef.push_back(at(top << 4 | (jj + 8))); }
+          double l1 = 0.0;                                             // exact: dyadic numbers of a few bits
+          for (size_t si = 0; si < ninner; si++) { l1 += std::fabs(at(si)); if (at(si) != 0.0) f.nonzero++; }
+          if (kd >= 3) { f.coef.push_back(l1); f.coef.push_back(0.0); }  // closing unit of the block: (sum |c|, -) for the round-off bound
+          f.n_coef += (int64_t)ninner;
         }
-        for (double v : f.coef) if (v != 0.0) { any = true; f.nonzero++; }
+        any = f.nonzero > 0;
         if (!any) continue;
         for (int s : ji.pairedSlots) f.paired.push_back((uint8_t)s);
         for (int b = 0; b < kd; b++) f.inner.push_back((uint8_t)ji.binSlots[ko + b]);
@@ -276,7 +282,7 @@ inline TableBuild buildTable(const Piece &p, int op, int nthreads, int maxGrade,
         famsOf[j].push_back(std::move(f));
       }
   });
-  for (auto &v : famsOf) for (auto &f : v) { tb.n_stored += (int64_t)f.coef.size(); tb.n_nonzero += f.nonzero; tb.fams.push_back(std::move(f)); }
+  for (auto &v : famsOf) for (auto &f : v) { tb.n_stored += f.n_coef; tb.n_nonzero += f.nonzero; tb.fams.push_back(std::move(f)); }
   lap("families");
   return tb;
 }

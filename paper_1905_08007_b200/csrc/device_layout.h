@@ -16,7 +16,12 @@
 #define MQ_MAXNODE 256
 #define MQ_MAXPAT 16      // 2^(max #S-children of a piece)
 // inner dense binary dimensions of a family, by number of Wick pairs c (bounds the static code and the family size)
-static inline int mq_kd_max(int c) { return c <= 3 ? 4 : 2; }   // keeps every family below one chunk;   // larger inner blocks (5, 6) were measured slower (register spills)
+// kd <= 4 blocks are evaluated by one Horner pass in registers (8 partial values); kd = 5, 6 blocks are 2 / 4 such blocks
+// combined over the top variables (two-stage Horner), so the register need does not grow. A larger kd merges the 2^(kd-4)
+// families of a slot set that differ only in the P+/P- choice of outer lines: half the stream entries, a third fewer operand
+// gathers and scalar factors at 5-loop for 3 % more stored coefficients (measured). Caps keep an entry of MQ_WL families
+// below one chunk.
+static inline int mq_kd_max(int c) { return c <= 2 ? 6 : c == 3 ? 4 : 2; }
 #define MQ_MAXSCAL 12
 #define MQ_CHUNK_WORDS 1024   // staging granule of the family stream (8 KiB): the largest entry (MQ_WL families of c = 4, kd = 2) must fit
 #define MQ_WL 2               // families per stream entry = lanes that share one sample point in the binary64 / double-double kernels
@@ -85,9 +90,12 @@ struct DevHeader {
 //   (c, kd, idx_words and the coefficient count are the same in all MQ_WL header words)
 // index bytes of member s: C(2c,2) beta~ indices of its paired slots (pair (i<j) at i*2c - i(i+1)/2 + j-i-1) | kd inner
 //   binary slot ids | nscal scalar-factor indices; all are direct indices into the per-point scalar array S
-// coefficients: for every pairing (canonical order) 2^kd values per member. kd >= 1: stored as 16-byte units
-//   (c[j], c[j+2^(kd-1)]), j < 2^(kd-1) (the first Horner level); unit j of pairing q of member s sits at unit index
-//   (q*2^(kd-1) + j)*MQ_WL + s. kd = 0: one double per pairing, at double index q*MQ_WL + s.
+// coefficients: for every pairing (canonical order) 2^kd values per member (index bit b <-> inner slot b). 1 <= kd <= 4:
+//   stored as 16-byte units (c[j], c[j+2^(kd-1)]), j < 2^(kd-1) (the first Horner level). kd = 5, 6: the 2^(kd-4) sub-blocks
+//   of kd = 4 (top index bits fixed, ascending) one after the other, each in that unit layout. Unit u of a member's
+//   Every kd >= 3 block is closed by one more unit (sum_sigma |c_sigma|, 0): the evaluator needs it for a round-off bound that
+//   sees the cancellation INSIDE a block (O8); for kd <= 2 it adds the |c| it has loaded anyway. Unit u of a member's sequence sits at unit index u*MQ_WL + s.
+//   kd = 0: one double per pairing, at double index q*MQ_WL + s.
 //   The lanes of a warp therefore read MQ_WL adjacent units with one shared-memory wavefront.
 static inline uint64_t mq_pack_family(int c, int kd, int pattern, int nscal, int out, int idx_words, uint32_t ncoef, int is_void = 0) {
   return (uint64_t)c | (uint64_t)kd << 3 | (uint64_t)pattern << 6 | (uint64_t)nscal << 10 | (uint64_t)out << 14 | (uint64_t)is_void << 15 |

@@ -63,18 +63,20 @@ __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   
   return bad;
 }
 
-// Precision decision of one tier (O8). a = sum |contribution| carried by the evaluator, inner = min over the
-// electron lines of every piece of (|A_t|, g_t, pivot / diagonal), unit = 64 ulp of the tier's arithmetic.
-//   0: accepted, relative round-off bound met (a <= cond_max |f| and inner >= inner_min): |df| <= 1e-10 |f| in tier 1
+// Precision decision of one tier (O8). a = sum of |monomial| bounds carried by the evaluator (sum|c| of every
+// coefficient block x |pairing weight| x |scalar factors|, through the whole tree), amin = min |A_t| over the electron lines
+// of every piece, xmin = min over pieces of (pivot / diagonal of the loop-matrix elimination, g_t = 1 + A_t): the quantities
+// every operand is divided by. unit = 32 (binary64) / 64 (double-double) ulp of the tier's arithmetic.
+//   0: accepted, relative round-off bound met (a <= cond_max |f| and min(amin, xmin) >= inner_min): |df| <= 1e-10 |f| in tier 1
 //   2: precision loss detected, but the absolute round-off bound on the WEIGHT w = f/p is below w_abs_tol: the
 //      Monte Carlo sums need absolute, not relative, accuracy of w (PAPER.md:91 controls the round-off error of the result)
 //   1: handed to the next tier
-#define MQ_UNIT_F64 (64.0 * 0x1p-53)
+#define MQ_UNIT_F64 (32.0 * 0x1p-53)
 #define MQ_UNIT_DD (64.0 * 0x1p-103)
-__device__ __forceinline__ int tier_decision(bool hard, double f, double a, double inner, double p, double cond_max, double inner_min, double unit, double w_abs_tol) {
+__device__ __forceinline__ int tier_decision(bool hard, double f, double a, double amin, double xmin, double p, double cond_max, double inner_min, double unit, double w_abs_tol) {
   if (hard || !isfinite(f) || !isfinite(a)) return 1;
-  if (a <= cond_max * fabs(f) && inner >= inner_min) return 0;
-  if (unit * a <= w_abs_tol * p * fmin(1.0, inner)) return 2;
+  if (a <= cond_max * fabs(f) && fmin(amin, xmin) >= inner_min) return 0;
+  if (unit * a <= w_abs_tol * p * fmin(1.0, xmin)) return 2;
   return 1;
 }
 

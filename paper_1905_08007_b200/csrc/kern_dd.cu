@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
-    const bool lost = tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;
+    const bool lost = tier_decision(false, fd, mq_to_double(a), amin, xmin, p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;
     if (bad_point(z, v.h->M, p)) atomicAdd(&counters[1], 1ull);                  // dropped: w = 0
     else if (lost) {                                          // third tier: quad-double
       const unsigned long long slot = atomicAdd(&counters[2], 1ull);
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
-      const bool lost = tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;     // same rule as k_integrate_dd
+      const bool lost = tier_decision(false, fd, mq_to_double(a), amin, xmin, p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;     // same rule as k_integrate_dd
       if (bad_point(z, v.h->M, p)) atomicAdd(&bv.ndrop[d], 1ull);
       else if (lost) {
         const unsigned long long slot = atomicAdd(&bv.nlost[d], 1ull);
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
     if (live) {
       const double fd = mq_to_double(f);
       f_out[rel] = fd;
-      if (tier_decision(false, fd, mq_to_double(a), fmin(amin, xmin), p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1) {
+      if (tier_decision(false, fd, mq_to_double(a), amin, xmin, p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1) {
         const unsigned long long slot = atomicAdd(&counters[2], 1ull);
         if (slot < LOSTCAP) lost_list[slot] = rel;
       }

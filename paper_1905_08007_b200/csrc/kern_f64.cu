@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(TPB_F64, 2) k_integrate_f64(const uint64_t *__
     double f, a, amin, xmin;
     eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
-    const bool flag = tier_decision(bad_point(z, v.h->M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+    const bool flag = tier_decision(bad_point(z, v.h->M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
     if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
     else { const double w = f / p; s1.add(w); s2.add(w * w); }
   }
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
     double f, a, amin, xmin;
     eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
-    const int dec = tier_decision(bad_point(z, M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
+    const int dec = tier_decision(bad_point(z, M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
     const bool flag = dec == 1;
     if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
     if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(TPB_F64, 2) k_batch_f64(BatchView bv, uint64_t
     const double p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
     double f, a, amin, xmin;
     eval_integrand<double, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
-    const bool flag = live && tier_decision(bad_point(z, v.h->M, p), f, a, fmin(amin, xmin), p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+    const bool flag = live && tier_decision(bad_point(z, v.h->M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
     const unsigned bal = __ballot_sync(0xffffffffu, flag);
     if (lane == 0) s_wcnt[warp] = __popc(bal);
     __syncthreads();

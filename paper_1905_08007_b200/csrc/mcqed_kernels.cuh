@@ -186,9 +186,20 @@ struct StreamReader {
 // coefficients and index bytes come from the staged stream (shared memory, broadcast reads); the per-point
 // operands r_t and beta~_tu are gathered once per family from S[index][thread] into registers
 template <class T, int KD>
-__device__ __forceinline__ T horner(uint32_t &s_coef, const T *r) {
+__device__ __forceinline__ T horner_raw(uint32_t &s_coef, const T *r) {
   if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8 * MQ_WL; return v; }   // the MQ_WL members of an entry are interleaved
-  else {
+  else if constexpr (KD > 4) {                     // two-stage: 2^(KD-4) sub-blocks of kd = 4, combined over the top variables
+    constexpr int NS = 1 << (KD - 4);
+    T s[NS];
+#pragma unroll
+    for (int q = 0; q < NS; q++) s[q] = horner_raw<T, 4>(s_coef, r);
+#pragma unroll
+    for (int i = 0; i < KD - 4; i++) {
+#pragma unroll
+      for (int j = 0; j < (NS >> (i + 1)); j++) s[j] = mq_fma(s[2 * j + 1], r[4 + i], s[2 * j]);
+    }
+    return s[0];
+  } else {
     constexpr int H = 1 << (KD - 1);
     T v[H];
 #pragma unroll
@@ -205,30 +216,53 @@ __device__ __forceinline__ T horner(uint32_t &s_coef, const T *r) {
     return v[0];
   }
 }
+// one pairing block: its value, and l1 = sum |c| from the block's closing unit (kd = 0: |c| itself) for the round-off bound
+__device__ __forceinline__ double mq_absd(double a) { return fabs(a); }
+__device__ __forceinline__ double mq_absd(dd a) { return fabs(a.hi); }
+template <class T, int KD>
+__device__ __forceinline__ T horner(uint32_t &s_coef, const T *r, double &l1) {
+  if constexpr (KD == 0) { const double c0 = lds_f64(s_coef); s_coef += 8 * MQ_WL; l1 = fabs(c0); return T(c0); }
+  else if constexpr (KD == 1) {                    // small blocks carry no closing unit: add the |c| just loaded
+    const double2 cc = lds_f64x2(s_coef); s_coef += 16 * MQ_WL;
+    l1 = fabs(cc.x) + fabs(cc.y);
+    return mq_fma_c(cc.y, r[0], cc.x, T());
+  } else if constexpr (KD == 2) {
+    const double2 c0 = lds_f64x2(s_coef), c1 = lds_f64x2(s_coef + 16 * MQ_WL); s_coef += 32 * MQ_WL;
+    l1 = (fabs(c0.x) + fabs(c0.y)) + (fabs(c1.x) + fabs(c1.y));
+    return mq_fma(mq_fma_c(c1.y, r[1], c1.x, T()), r[0], mq_fma_c(c0.y, r[1], c0.x, T()));
+  } else {
+    const T h = horner_raw<T, KD>(s_coef, r);
+    l1 = lds_f64(s_coef); s_coef += 16 * MQ_WL;
+    return h;
+  }
+}
 // index of the pair (i<j) among the C(N2,2) gathered betas
 template <int N2> __host__ __device__ constexpr int pair_index(int i, int j) { return i * N2 - i * (i + 1) / 2 + (j - i - 1); }
 constexpr int ctz_c(unsigned x) { int n = 0; while (!(x & 1u)) { x >>= 1; n++; } return n; }
 
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec;
 template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> struct PairStep {
-  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, double &asum) {
     if constexpr (S < N2) {
       if constexpr (!((USED >> S) & 1u)) {
-        if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], s_coef, r, sum);
-        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, mq_mul(w, b[pair_index<N2>(F, S)]), s_coef, r, sum);
+        if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], s_coef, r, sum, asum);
+        else PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, mq_mul(w, b[pair_index<N2>(F, S)]), s_coef, r, sum, asum);
       }
-      PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, s_coef, r, sum);
+      PairStep<T, KD, N2, USED, FIRST, F, S + 1>::run(b, w, s_coef, r, sum, asum);
     }
   }
 };
+// sum += w_pairing * block, asum += |w_pairing| * sum|c|  (the latter bounds the block by sum|c| prod max(1,|r|), applied by the caller)
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
-  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, double &asum) {
     if constexpr (USED == ((1u << N2) - 1u)) {
-      T h = horner<T, KD>(s_coef, r);
-      if constexpr (FIRST) sum = h; else sum = mq_fma(w, h, sum);   // FIRST at a leaf: no pairs, one block
+      double l1;
+      T h = horner<T, KD>(s_coef, r, l1);
+      if constexpr (FIRST) { sum = h; asum = l1; }   // FIRST at a leaf: no pairs, one block
+      else { sum = mq_fma(w, h, sum); asum = fma(mq_absd(w), l1, asum); }
     } else {
       constexpr int F = ctz_c(~USED);
-      PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, s_coef, r, sum);
+      PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, s_coef, r, sum, asum);
     }
   }
 };
@@ -274,10 +308,11 @@ __constant__ PairTbl4 c_tbl4 = make_tbl4();
 
 // the three pairings of four slots a<b<c<d, each with prefix weight wp: g = (ab, ac, ad, bc, bd, cd)
 template <class T, int KD>
-__device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, const T *r, T &sum) {
-  sum = mq_fma(mq_mul(mq_mul(wp, g[0]), g[5]), horner<T, KD>(s_coef, r), sum);     // (ab)(cd)
-  sum = mq_fma(mq_mul(mq_mul(wp, g[1]), g[4]), horner<T, KD>(s_coef, r), sum);     // (ac)(bd)
-  sum = mq_fma(mq_mul(mq_mul(wp, g[2]), g[3]), horner<T, KD>(s_coef, r), sum);     // (ad)(bc)
+__device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, const T *r, T &sum, double &asum) {
+  double l1; T w;
+  w = mq_mul(mq_mul(wp, g[0]), g[5]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ab)(cd)
+  w = mq_mul(mq_mul(wp, g[1]), g[4]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ac)(bd)
+  w = mq_mul(mq_mul(wp, g[2]), g[3]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ad)(bc)
 }
 
 // byte i (compile-time) of an array of 64-bit index words: one PRMT
@@ -291,22 +326,32 @@ template <class T, int N, int OFF, int I = 0> struct Gather {
   }
 };
 
+// value of a family and its round-off magnitude a = sum_pairings |w| sum|c| prod_inner max(1,|r|) >= sum of |monomial|
+template <class T> struct FamRes { T v; double a; };
+template <class T, int KD> __device__ __forceinline__ double rbound(const T *r) {
+  double R = 1.0;
+#pragma unroll
+  for (int i = 0; i < KD; i++) R *= fmax(1.0, mq_absd(r[i]));
+  return R;
+}
+
 // s_idx: shared address of the index bytes; s_coef: of the coefficients; s_S: of this thread's S[0]; sstride: bytes per S index
 template <class T, int C, int KD>
-__device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+__device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
   constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
+  FamRes<T> res;
   if constexpr (C >= 3 && sizeof(T) == sizeof(dd)) {
     T r[KD > 0 ? KD : 1];
 #pragma unroll
     for (int i = 0; i < KD; i++) r[i] = lds_T<T>(s_S + lds_u8(s_idx + NB + i) * sstride);
-    T sum = T(0.0);
+    T sum = T(0.0); double asum = 0.0;
     if constexpr (C == 3) {
 #pragma unroll 1
       for (int j = 0; j < 5; j++) {
         T g[7];
 #pragma unroll
         for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl3.p[j][k]) * sstride);
-        pair_body4<T, KD>(g[0], g + 1, s_coef, r, sum);
+        pair_body4<T, KD>(g[0], g + 1, s_coef, r, sum, asum);
       }
     } else {
 #pragma unroll 1
@@ -317,43 +362,46 @@ __device__ __forceinline__ T family_eval(uint64_t w0, uint64_t w1, uint32_t s_id
           T g[7];
 #pragma unroll
           for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl4.p[j1][j2][k]) * sstride);
-          pair_body4<T, KD>(mq_mul(w1, g[0]), g + 1, s_coef, r, sum);
+          pair_body4<T, KD>(mq_mul(w1, g[0]), g + 1, s_coef, r, sum, asum);
         }
       }
     }
-    return sum;
+    res.v = sum; res.a = asum * rbound<T, KD>(r);
   } else {
-  uint64_t iw[NW > 2 ? NW : 2];
-  iw[0] = w0; iw[1] = w1;                          // the first 16 index bytes were prefetched with the header
+    uint64_t iw[NW > 2 ? NW : 2];
+    iw[0] = w0; iw[1] = w1;                          // the first 16 index bytes were prefetched with the header
 #pragma unroll
-  for (int k = 2; k < NW; k++) iw[k] = lds_u64(s_idx + 8 * k);
-  T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
-  Gather<T, NB, 0>::run(iw, s_S, sstride, b);
-  Gather<T, KD, NB>::run(iw, s_S, sstride, r);
-  T sum = T(0.0);
-  PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum);
-  return sum;
+    for (int k = 2; k < NW; k++) iw[k] = lds_u64(s_idx + 8 * k);
+    T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
+    Gather<T, NB, 0>::run(iw, s_S, sstride, b);
+    Gather<T, KD, NB>::run(iw, s_S, sstride, r);
+    T sum = T(0.0); double asum = 0.0;
+    PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum, asum);
+    res.v = sum; res.a = asum * rbound<T, KD>(r);
   }
+  return res;
 }
 
 template <class T>
-__device__ __noinline__ T family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+__device__ __noinline__ FamRes<T> family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
   switch (ckd) {     // key = c*8 + kd; the inner dimension kd is capped per c by mq_kd_max (device_layout.h)
 #define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(w0, w1, s_idx, s_coef, s_S, sstride);
-#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3)
+#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2)
     MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_ROW(4)
-    MQ_CASE(0, 4) MQ_CASE(0, 5) MQ_CASE(0, 6) MQ_CASE(1, 4) MQ_CASE(1, 5) MQ_CASE(1, 6) MQ_CASE(2, 4) MQ_CASE(2, 5) MQ_CASE(3, 4)
+    MQ_CASE(0, 3) MQ_CASE(0, 4) MQ_CASE(0, 5) MQ_CASE(0, 6) MQ_CASE(1, 3) MQ_CASE(1, 4) MQ_CASE(1, 5) MQ_CASE(1, 6)
+    MQ_CASE(2, 3) MQ_CASE(2, 4) MQ_CASE(2, 5) MQ_CASE(2, 6) MQ_CASE(3, 3) MQ_CASE(3, 4)
 #undef MQ_ROW
 #undef MQ_CASE
   }
   __trap();          // a family shape the tables must never contain
-  return T(0.0);
+  return FamRes<T>{T(0.0), 0.0};
 }
 
-// Two consecutive families of the same shape evaluated together: their arithmetic chains are independent, which
+// Two consecutive entries of the same shape evaluated together: their arithmetic chains are independent, which
 // doubles the instruction-level parallelism of a warp at unchanged shared-memory footprint (binary64 only).
+// Returns (value A, value B, magnitude A, magnitude B); arguments and results in registers.
 template <int C, int KD>
-__device__ __forceinline__ double2 family_eval2(uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
+__device__ __forceinline__ double4 family_eval2(uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
                                                 uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
   constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
   uint64_t iwA[NW > 2 ? NW : 2], iwB[NW > 2 ? NW : 2];
@@ -365,80 +413,64 @@ __device__ __forceinline__ double2 family_eval2(uint64_t wA0, uint64_t wA1, uint
   Gather<double, NB, 0>::run(iwB, s_S, sstride, bB);
   Gather<double, KD, NB>::run(iwA, s_S, sstride, rA);
   Gather<double, KD, NB>::run(iwB, s_S, sstride, rB);
-  double sumA = 0.0, sumB = 0.0;
-  PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA);
-  PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB);
-  return make_double2(sumA, sumB);
+  double sumA = 0.0, sumB = 0.0, aA = 0.0, aB = 0.0;
+  PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA, aA);
+  PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB, aB);
+  return make_double4(sumA, sumB, aA * rbound<double, KD>(rA), aB * rbound<double, KD>(rB));
 }
-// arguments and results in registers (no stack traffic across the call)
-static __device__ __noinline__ double2 family_dispatch2(int ckd, uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
+static __device__ __noinline__ double4 family_dispatch2(int ckd, uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
                                                         uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
   switch (ckd) {
 #define MQ_CASE(C, K) case C * 8 + K: return family_eval2<C, K>(wA0, wA1, wB0, wB1, s_idxA, s_coefA, s_idxB, s_coefB, s_S, sstride);
 #define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
-    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3)
+    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_CASE(0, 5) MQ_CASE(1, 5) MQ_CASE(2, 5) MQ_CASE(0, 6) MQ_CASE(1, 6) MQ_CASE(2, 6)
 #undef MQ_ROW
 #undef MQ_CASE
   }
   __trap();
-  return make_double2(0.0, 0.0);
-}
-
-// Loop-based family evaluation for wide types (quad-double): same arithmetic as family_eval, no unrolling.
-// Pairings are enumerated in the canonical order (the first free element pairs with every later one).
-template <class T>
-__device__ __noinline__ T family_generic(int c, int kd, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
-  const int n2 = 2 * c, nb = c * (2 * c - 1), nblk = 1 << kd;
-  T b[28], r[4], v[8];
-  for (int i = 0; i < nb; i++) b[i] = lds_T<T>(s_S + lds_u8(s_idx + i) * sstride);
-  for (int i = 0; i < kd; i++) r[i] = lds_T<T>(s_S + lds_u8(s_idx + nb + i) * sstride);
-  auto horner_at = [&](uint32_t a) -> T {
-    if (kd == 0) return T(lds_f64(a));
-    const int H = 1 << (kd - 1);
-    for (int j = 0; j < H; j++) { const double2 cc = lds_f64x2(a + 16 * MQ_WL * j); v[j] = mq_fma_c(cc.y, r[kd - 1], cc.x, T()); }
-    for (int i = kd - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
-    return v[0];
-  };
-  if (c == 0) return horner_at(s_coef);
-  T sum = T(0.0), w[5];
-  unsigned used[5]; int scur[5];
-  int level = 0; used[0] = 0u; w[0] = T(1.0); scur[0] = -1;
-  while (level >= 0) {
-    const unsigned u = used[level]; const int f = __ffs(~u) - 1;
-    int s2 = scur[level] < 0 ? f + 1 : scur[level] + 1;
-    while (s2 < n2 && (u >> s2 & 1u)) s2++;
-    if (s2 >= n2) { level--; continue; }
-    scur[level] = s2;
-    const T wn = w[level] * b[f * n2 - f * (f + 1) / 2 + (s2 - f - 1)];
-    if (level == c - 1) { sum = sum + wn * horner_at(s_coef); s_coef += 8 * MQ_WL * nblk; }
-    else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
-  }
-  return sum;
+  return make_double4(0.0, 0.0, 0.0, 0.0);
 }
 
 // Entry-parallel family evaluation (quad-double tier): member m of the stream entry at ent (GLOBAL memory), scalars from
-// S[index * stride] (shared). Same arithmetic and pairing order as family_generic; the scalar factors are applied here and
+// S[index * stride] (shared). Loop-based (no unrolling); same arithmetic and pairing order as family_eval (the first free
+// element pairs with every later one); the scalar factors are applied here and
 // the accumulation key (output, pattern, grade) of the member is returned in key.
 template <class T>
-__device__ __noinline__ T family_spread(const uint64_t *ent, uint64_t hd, int m, const T *S, int stride, int &key) {
+__device__ __noinline__ T family_spread(const uint64_t *ent, uint64_t hd, int m, const T *S, int stride, int &key, double &amag) {
   const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7), idxw = (int)(hd >> 16 & 0xFFFF);
   const uint64_t ml = ent[m];
   const uint8_t *idx = reinterpret_cast<const uint8_t *>(ent + MQ_WL + (size_t)idxw * m);
   const double *coef = reinterpret_cast<const double *>(ent + MQ_WL * (1 + idxw)) + (kd ? 2 : 1) * m;
   key = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
   const int n2 = 2 * c, nb = c * (2 * c - 1), nblk = 1 << kd, ns = (int)(ml >> 10 & 15);
-  T b[28], r[4], v[8];
+  T b[28], r[6], v[8];
   for (int i = 0; i < nb; i++) b[i] = S[(int)idx[i] * stride];
   for (int i = 0; i < kd; i++) r[i] = S[(int)idx[nb + i] * stride];
-  auto horner_at = [&](const double *a) -> T {
-    if (kd == 0) return T(a[0]);
-    const int H = 1 << (kd - 1);
-    for (int j = 0; j < H; j++) v[j] = mq_fma_c(a[2 * MQ_WL * j + 1], r[kd - 1], a[2 * MQ_WL * j], T());
-    for (int i = kd - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
+  auto block_at = [&](const double *a, int kk) -> T {      // one block of kk <= 4 inner variables
+    if (kk == 0) return T(a[0]);
+    const int H = 1 << (kk - 1);
+    for (int j = 0; j < H; j++) v[j] = mq_fma_c(a[2 * MQ_WL * j + 1], r[kk - 1], a[2 * MQ_WL * j], T());
+    for (int i = kk - 2; i >= 0; i--) for (int j = 0; j < (1 << i); j++) v[j] = mq_fma(v[j + (1 << i)], r[i], v[j]);
     return v[0];
   };
-  T sum = T(0.0);
-  if (c == 0) sum = horner_at(coef);
+  const int blk = kd >= 3 ? MQ_WL * (nblk + 2) : MQ_WL * nblk;       // doubles per pairing block incl. the closing (sum |c|, 0) unit of kd >= 3
+  auto l1_at = [&](const double *a) -> double {
+    if (kd >= 3) return a[MQ_WL * nblk];
+    if (kd == 0) return fabs(a[0]);
+    double t = 0.0;
+    for (int j = 0; j < nblk / 2; j++) t += fabs(a[2 * MQ_WL * j]) + fabs(a[2 * MQ_WL * j + 1]);
+    return t;
+  };
+  auto horner_at = [&](const double *a) -> T {
+    if (kd <= 4) return block_at(a, kd);
+    T s[4];                                                 // kd = 5, 6: sub-blocks of kd = 4, combined over r[4], r[5]
+    const int nsub = 1 << (kd - 4);
+    for (int q = 0; q < nsub; q++) s[q] = block_at(a + 16 * MQ_WL * q, 4);
+    for (int i = 0; i < kd - 4; i++) for (int j = 0; j < (nsub >> (i + 1)); j++) s[j] = mq_fma(s[2 * j + 1], r[4 + i], s[2 * j]);
+    return s[0];
+  };
+  T sum = T(0.0); double asum = 0.0;
+  if (c == 0) { sum = horner_at(coef); asum = l1_at(coef); }
   else {
     T w[5]; unsigned used[5]; int scur[5];
     int level = 0; used[0] = 0u; w[0] = T(1.0); scur[0] = -1;
@@ -449,11 +481,13 @@ __device__ __noinline__ T family_spread(const uint64_t *ent, uint64_t hd, int m,
       if (s2 >= n2) { level--; continue; }
       scur[level] = s2;
       const T wn = w[level] * b[f * n2 - f * (f + 1) / 2 + (s2 - f - 1)];
-      if (level == c - 1) { sum = sum + wn * horner_at(coef); coef += MQ_WL * nblk; }
+      if (level == c - 1) { sum = sum + wn * horner_at(coef); asum += fabs(mq_to_double(wn)) * l1_at(coef); coef += blk; }
       else { level++; used[level] = u | 1u << f | 1u << s2; w[level] = wn; scur[level] = -1; }
     }
   }
-  for (int i = 0; i < ns; i++) sum = sum * S[(int)idx[nb + kd + i] * stride];
+  for (int i = 0; i < kd; i++) asum *= fmax(1.0, fabs(mq_to_double(r[i])));
+  for (int i = 0; i < ns; i++) { const T sc = S[(int)idx[nb + kd + i] * stride]; sum = sum * sc; asum *= fabs(mq_to_double(sc)) + 0.125; }
+  amag = asum;
   return sum;
 }
 
@@ -534,7 +568,7 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
       const double xd = mq_to_double(x);
-      amin = fmin(amin, fmin(fabs(1.0 - xd), 2.0 - xd));
+      amin = fmin(amin, fabs(1.0 - xd)); xmin = fmin(xmin, 2.0 - xd);   // |A_t| (scalar factors of insertion pieces) ; g_t divides every operand of slot t
     }
   }
   if (wr)
@@ -614,10 +648,10 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           if (pend) {
 #pragma unroll 1
             for (int m = 0; m < MQ_WL; m++) {
-              int kk;
-              const T val = family_spread<T>(pend, pend_h, m, S, stride, kk);
+              int kk; double am;
+              const T val = family_spread<T>(pend, pend_h, m, S, stride, kk, am);
               N[kk >> 7][(kk >> 3) & 15][kk & 7] = N[kk >> 7][(kk >> 3) & 15][kk & 7] + val;
-              if constexpr (TRACK) Na[kk >> 7][(kk >> 3) & 15][kk & 7] += fabs(mq_to_double(val));
+              if constexpr (TRACK) Na[kk >> 7][(kk >> 3) & 15][kk & 7] += am;
             }
             pend = nullptr;
           }
@@ -686,17 +720,17 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         const int nb = c * (2 * c - 1) + kd;
         const uint32_t ustride = kd ? 16u : 8u;                        // bytes between the members' coefficient units
         // member header ml: scalar factors and accumulation key; sidx: shared address of the member's index bytes
-        auto account = [&](T val, uint64_t ml, uint32_t sidx) {
+        auto account = [&](T val, double amag, uint64_t ml, uint32_t sidx) {
           const int ns = (int)(ml >> 10 & 15), keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
           val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
 #pragma unroll 1
-          for (int i = 0; i < ns; i++) val = val * lds_T<T>(s_S + lds_u8(sidx + nb + i) * sstride);
+          for (int i = 0; i < ns; i++) { const T sc = lds_T<T>(s_S + lds_u8(sidx + nb + i) * sstride); val = val * sc; amag *= mq_absd(sc) + 0.125; }   // + 1/8: the factor's own absolute round-off (A_t = 1 - x_t may be tiny)
           if (keyk != key) {
             if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
             key = keyk; racc = T(0.0); racca = 0.0;
           }
           racc = racc + val;
-          if constexpr (TRACK) racca += fabs(mq_to_double(val));
+          if constexpr (TRACK) racca += amag;      // sum of |monomial| bounds: sees the cancellation inside a family too
         };
         if (dual) {
           if constexpr (sizeof(T) == sizeof(double) && LANES) {
@@ -707,10 +741,10 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             if (have3) { hd3 = lds_u64(a2); fetch_member(a2, hd3, sub, hl3, m0, m1); }
             if (W == 1 || unit % W == gw) {
               const uint32_t sidxA = a0 + 8 * MQ_WL + 8 * idxw * sub, sidxB = an + 8 * MQ_WL + 8 * idxw2 * sub;
-              const double2 vAB = family_dispatch2(c * 8 + kd, w0, w1, n0, n1, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub,
+              const double4 vAB = family_dispatch2(c * 8 + kd, w0, w1, n0, n1, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub,
                                                    sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub, s_S, sstride);
-              account(T(vAB.x), hl, sidxA);
-              account(T(vAB.y), hln, sidxB);
+              account(T(vAB.x), vAB.z, hl, sidxA);
+              account(T(vAB.y), vAB.w, hln, sidxB);
             }
             unit++;
             rd.pos = npos2; left -= 2;
@@ -724,10 +758,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             const int m = LANES ? sub : q;
             if constexpr (!LANES) fetch_member(a0, hd, m, hl, w0, w1);
             const uint32_t sidx = a0 + 8 * MQ_WL + 8 * idxw * m, scoef = a0 + 8 * MQ_WL * (1 + idxw) + ustride * m;
-            T val;
-            if constexpr (sizeof(T) > sizeof(dd)) val = family_generic<T>(c, kd, sidx, scoef, s_S, sstride);
-            else val = family_dispatch<T>(c * 8 + kd, w0, w1, sidx, scoef, s_S, sstride);
-            account(val, hl, sidx);
+            static_assert(sizeof(T) <= sizeof(dd), "wider types use the entry-parallel path");
+            const FamRes<T> fr = family_dispatch<T>(c * 8 + kd, w0, w1, sidx, scoef, s_S, sstride);
+            account(fr.v, fr.a, hl, sidx);
           }
         }
         unit++;

@@ -37,6 +37,23 @@ def pairings(n2):
     return list(rec(list(range(n2))))
 
 
+def _flatten_big_blocks(coef, kd):
+    """device_layout.h: a kd = 5, 6 block is stored as 2^(kd-4) sub-blocks of kd = 4, each as units (c[j], c[j+8]); returns the
+    block in the single-level layout (c[j], c[j+2^(kd-1)]) that family_value undoes"""
+    n, half = 1 << kd, 1 << (kd - 1)
+    out = np.empty_like(coef)
+    for q in range(len(coef) // n):
+        blk = coef[q * n:(q + 1) * n]
+        nat = np.empty(n)
+        for top in range(n >> 4):
+            sub = blk[top * 16:(top + 1) * 16]
+            nat[(top << 4):(top << 4) + 8] = sub[0::2]
+            nat[(top << 4) + 8:(top << 4) + 16] = sub[1::2]
+        o = out[q * n:(q + 1) * n]
+        o[0::2], o[1::2] = nat[:half], nat[half:]
+    return out
+
+
 class Blob:
     def __init__(self, words):
         self.w = np.ascontiguousarray(words, np.uint64)
@@ -75,6 +92,12 @@ class Blob:
                 assert (hm & 63) == (hd & 63) and (hm >> 16) == (hd >> 16)
                 pat, nscal, out, void = hm >> 6 & 15, hm >> 10 & 15, hm >> 14 & 1, hm >> 15 & 1
                 coef = np.ascontiguousarray(allc[:, m, :]).reshape(-1)
+                if kd >= 3:                     # strip (and check) the closing (sum |c|, 0) unit of every block
+                    blocks = coef.reshape(-1, (1 << kd) + 2)
+                    assert np.array_equal(blocks[:, -2], np.abs(blocks[:, :-2]).sum(axis=1)) and not blocks[:, -1].any()
+                    coef = np.ascontiguousarray(blocks[:, :-2]).reshape(-1)
+                if kd > 4:                      # sub-blocks of kd = 4 (top index bits ascending) -> one (lo,hi)-interleaved block
+                    coef = _flatten_big_blocks(coef, kd)
                 if void:
                     assert not coef.any()
                     continue
