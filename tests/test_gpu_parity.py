@@ -334,3 +334,34 @@ def test_two_loop_full_size_against_paper_value_and_stored_oracle_run(mc):
     b.close()
     for d in ds:
         d.close()
+
+
+def test_precision_policy_bounds_hold_on_five_loop_sample(mc):
+    """DESIGN.md O8 on 6 graphs of configs[4] x 37888 points: every point accepted by the relative bound (flag 0) is within
+    1e-10 relative of the library's double-double value, every point accepted by the absolute bound (flag 2) within
+    |dw| <= w_abs_tol = 1e-10 of it, and re-evaluated points (flag 1) carry the double-double (or quad-double) value.
+    The double-double value itself is pinned to the oracle's binary128 value by the parity tests above."""
+    from paper_1905_08007_b200 import workloads
+    st = torch.cuda.current_stream().cuda_stream
+    n, seed = 37888, workloads.CONFIG_SEED[4]
+    mix = np.zeros(3)
+    for _, g in workloads.config_graphs(4)[5::45]:
+        d = mc.Diagram(g[0], g[1], g[2])
+        r = _gpu_points(mc, d, 0, n, seed)
+        fdd = torch.zeros(n, dtype=torch.float64, device="cuda")
+        d.eval_z(n, torch.tensor(r["z"], device="cuda"), st, None, fdd, None, None)
+        torch.cuda.synchronize()
+        fdd = fdd.cpu().numpy()
+        fl = r["flag"]
+        ok = np.isfinite(fdd)
+        rel = np.abs(r["f64"] - fdd) / np.abs(fdd)
+        assert np.all(rel[(fl == 0) & ok] <= 1e-10), rel[(fl == 0) & ok].max()
+        dw = np.abs(r["f64"] - fdd) / r["p"]
+        assert np.all(dw[(fl == 2) & ok] <= 1e-10), dw[(fl == 2) & ok].max()
+        assert np.array_equal(r["f"][fl != 1], r["f64"][fl != 1])
+        redo = (fl == 1) & ok
+        agree = np.abs(r["f"] - fdd)[redo] <= 1e-13 * np.abs(fdd)[redo]
+        assert agree.mean() > 0.99                                  # the rest went on to quad-double
+        mix += np.bincount(fl, minlength=3)
+        d.close()
+    assert mix[1] / mix.sum() < 0.5 and mix[0] > 0 and mix[2] > 0
