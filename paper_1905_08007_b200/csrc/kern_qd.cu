@@ -37,7 +37,7 @@ __device__ __forceinline__ void qd_setup_reader(StreamReader &rd, unsigned char 
   const size_t s = qd_head_bytes(scal_len);
   rd.init(reinterpret_cast<uint64_t *>(smem + s), reinterpret_cast<uint64_t *>(smem + s + 2 * MQ_CHUNK_WORDS * 8));
 }
-// the integrand of one point in quad-double, computed by the whole CTA; every thread returns the same value
+// the integrand of one point in quad-double, computed by the whole CTA; the value is valid in thread 0
 __device__ __forceinline__ double qd_point(const DiagView &v, StreamReader &rd, const QdRoles &ro, const double *z) {
   qd f, a; double amin, xmin;
   eval_integrand<qd, 1, false, true>(v, rd, z, ro.S, 1, ro.xT, ro.xA, 0, 0, f, a, amin, xmin);

@@ -620,6 +620,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   double nodeabs[TRACK ? 1024 : 1];
   T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
   double amin = 1.0, xmin = 1.0;
+  const bool owner = gw == 0 && sub == 0 && (!SPREAD || threadIdx.x == 0);   // the lane whose f_out is used
   const uint32_t s_S = smem_u32(S), sstride = (uint32_t)(stride * sizeof(T));
   rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
   for (int gi = 0; gi < h.ngeom; gi++) {
@@ -801,8 +802,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           __syncthreads();
         }
       }
-      // nodes that use this table: combine with the children's graded values (owner warp only)
-      if (gw == 0)
+      // nodes that use this table: combine with the children's graded values. Only the owner lane of a point does this
+      // (the other lane role holds the same totals: doing it twice would only double the local-memory traffic)
+      if (owner)
       for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {
         const DevNode &nd = v.node[ni];
         T Up = U, Vs = V;
@@ -834,7 +836,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   // a6: terms.  f = sum sign * sum_{c<L} (L-c-1)! N_c / (Uprod^2 Vsum^(L-c))
   const int L = h.L;
   T f = T(0.0), asum = T(0.0);
-  if (gw == 0)
+  if (owner)
   for (int t = 0; t < h.nterm; t++) {
     const DevTerm tm = v.term[t];
     const DevNode &nd = v.node[tm.root];
