@@ -182,6 +182,15 @@ def run_ours(args):
         mean = s[0, i] / n_tot
         var_sum += max(s[1, i] / n_tot - mean * mean, 0.0) / n_tot
     flagged_frac = float(c[0].sum()) / (G * n_tot)
+    # per gauge-invariant class (k,m,n) of PAPER.md:104, the columns of Table 1: sum a_j, its sigma, sum |a_j|, max |a_j|
+    classes = {}
+    for i, (_, g) in enumerate(graphs):
+        mean = s[0, i] / n_tot
+        var = max(s[1, i] / n_tot - mean * mean, 0.0) / n_tot
+        e = classes.setdefault("%d,%d,%d" % workloads.graph_class(g), {"n_diag": 0, "sum": 0.0, "var": 0.0, "sum_abs": 0.0, "max_abs": 0.0})
+        e["n_diag"] += 1; e["sum"] += mean; e["var"] += var; e["sum_abs"] += abs(mean); e["max_abs"] = max(e["max_abs"], abs(mean))
+    for e in classes.values():
+        e["sigma"] = math.sqrt(e.pop("var"))
     # ---- per-kernel times: the same steps with the higher tiers switched off (flags bit 0: binary64 kernel alone;
     #      bit 1: no quad-double pass); the double-double and quad-double kernels are timed as the differences ----
     state["flags"] = mc.FLAG_NO_DD
@@ -250,7 +259,7 @@ def run_ours(args):
                        "n_graphs": G, "batch": B, "seed": seed, "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
                        "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "precision": precision, "dropped": int(c[1].sum()),
                        "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
-                       "algorithmic_flop_per_sample_mean": sum(flop) / G},
+                       "algorithmic_flop_per_sample_mean": sum(flop) / G, "classes": classes},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         r = oracle_run(args, graphs, seed, 1, 0)
