@@ -214,10 +214,10 @@ def run_ours(args):
     dom = "k_batch_dd" if ms_dd > ms_f64 else "k_batch_f64"
     ach = ach_dd if dom == "k_batch_dd" else ach_f64
     roofline = {"bound": "alu", "kernel": dom, "achieved": ach / 1e12, "peak": peak_flops / 1e12, "unit": "TFLOP/s", "frac": ach / peak_flops,
-                "traffic": 88.68e9 if (dom == "k_batch_f64" and G == 256 and B == 37888 and args.config == 4) else None,
+                "traffic": 73.74e9 if (dom == "k_batch_f64" and G == 256 and B == 37888 and args.config == 4) else None,
                 "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of k_batch_f64 in this launch configuration, one ncu --set full capture "
-                                "(profiles/r1_summary.md: 34.6 GB read + 54.1 GB written in a 2.11 s launch = 42 GB/s, 0.6 % of HBM bandwidth); the "
-                                "algorithmic bytes are ~0 (no per-sample input or output): this is per-thread stack (node values, graded sums) going through L2",
+                                "(profiles/r1_v6_ncu_f64_fullconfig_details.txt: 35.8 GB read + 37.9 GB written in a 1.75 s launch = 42 GB/s, 0.6 % of HBM bandwidth); the "
+                                "algorithmic bytes are ~0 (no per-sample input or output): the reads are the table streams missing L2 (2.3 GB of tables), the writes per-thread stack (node values, graded sums)",
                 "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
                 "kernels": {"k_batch_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
                             "k_batch_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
