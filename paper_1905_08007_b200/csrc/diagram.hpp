@@ -10,9 +10,10 @@
 
 namespace mqk {
 constexpr int TPB_F64 = 256, TPB_DD = 128, TPB_EVAL = 128;
-// warp split (mcqed_kernels.cuh): W warps share one group of 32 points, so a CTA of T threads holds T / W points.
-// Measured on B200 (profiles/r1_summary.md): W = 2 doubles the resident warps but is slower than W = 1 (binary64 11.9 % vs
-// 13.5 % of peak on a subtraction-free graph; double-double 2.6e5 vs 4.2e5 points/s on a 12-term graph), so W = 1.
+// warp split (mcqed_kernels.cuh): W warps share one group of points. Measured on B200 before the lane split existed
+// (profiles/r1_summary.md): W = 2 doubles the resident warps but is slower than W = 1 (binary64 11.9 % vs 13.5 % of peak on a
+// subtraction-free graph; double-double 2.6e5 vs 4.2e5 points/s on a 12-term graph), so W = 1; the lane split (MQ_WL lanes of a
+// warp per point, device_layout.h) is what doubles the resident warps now.
 constexpr int W_F64 = 1, W_DD = 1;
 constexpr int PTS_F64 = TPB_F64 / (W_F64 * MQ_WL), PTS_DD = TPB_DD / (W_DD * MQ_WL), PTS_EVAL = TPB_EVAL / (W_F64 * MQ_WL);   // points per CTA (MQ_WL lanes per point)
 constexpr uint64_t CHUNK = 1ull << 22;     // samples per launch (bounds the flagged-index list)

@@ -1,4 +1,5 @@
-// kern_common.cuh — pieces shared by the two kernel translation units (binary64 and double-double).
+// kern_common.cuh — pieces shared by the kernel translation units (binary64, double-double, quad-double): thread roles,
+// reductions, the precision decision, the batched path's item lookup.
 // Product code (libmcqed.so).
 #pragma once
 #include "diagram.hpp"

@@ -1,11 +1,12 @@
 // mcqed_kernels.cuh — device code of the hot path (steps a1-a8 of DESIGN.md §2), sm_100a.
 // Product code (libmcqed.so); shares nothing with oracle/.
 //
-// Mapping: one thread = one sample point (lanes = points). All threads of a launch work on the same
-// diagram, so every table read (family headers, coefficients, Z/invDeg rows) is warp-uniform and
-// control flow never diverges inside the integrand. Per-point operands that the tables address by
-// index (r_t, A_t, A'_t/g_t, beta_tu/(g_t g_u)) live in shared memory laid out [index][thread]
-// (conflict-free); everything with static indexing lives in registers. FP64 FMA pipe is the roofline.
+// Mapping: lanes = sample points of ONE diagram (MQ_WL lanes share a point and evaluate the MQ_WL families of a
+// stream entry side by side: "lane split" below). All threads of a CTA work on the same diagram, so every table
+// read (entry headers, coefficients, Z/invDeg rows) is warp-uniform and control flow never diverges inside the
+// integrand. Per-point operands that the tables address by index (r_t, A_t, A'_t/g_t, beta_tu/(g_t g_u)) live in
+// shared memory laid out [index][point] (conflict-free); everything with static indexing lives in registers.
+// The quad-double tier works entry-parallel instead (one point per CTA). FP64 FMA pipe is the roofline.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
