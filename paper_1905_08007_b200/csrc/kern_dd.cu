@@ -44,8 +44,8 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
 __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item; __shared__ int s_d;
-  const Roles<dd, 1, MQ_WL> ro(smem_raw, scal_len);
-  StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(dd));
+  const Roles<dd, W_DD, MQ_WL> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<W_DD, MQ_WL>(rd, smem_raw, scal_len, sizeof(dd));
   const uint32_t total = bv.dd_start[bv.nd];
   for (;;) {
     __syncthreads();
@@ -57,12 +57,12 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     const DiagView v = make_view(bv.dg[d].blob);
     const MqPrec pr = bv.dg[d].pr;
     const unsigned long long cnt = bv.nflag[d];
-    const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + ro.slot; const bool live = i < cnt && ro.sub == 0;
+    const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + ro.slot; const bool live = i < cnt && ro.sub == 0 && ro.gw == 0;
     const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (i < cnt ? i : cnt - 1)];
     double z[MQ_MAXM];
     const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
@@ -160,7 +160,7 @@ int mq_batch_config_dd(size_t smem, int *grid) {
   *grid = nsm * occ;
   return 0;
 }
-size_t mq_batch_smem_dd(int scal_len) { return smem_bytes(scal_len, TPB_DD, sizeof(dd), 1, MQ_WL); }
+size_t mq_batch_smem_dd(int scal_len) { return smem_bytes(scal_len, TPB_DD, sizeof(dd), W_DD, MQ_WL); }
 void mq_launch_batch_dd(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t seed, int scal_len, mq_stream st) {
   k_batch_dd<<<grid, TPB_DD, smem, (cudaStream_t)st>>>(bv, first, seed, scal_len);
 }
