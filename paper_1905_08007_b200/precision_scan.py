@@ -1,6 +1,7 @@
 """Precision scan: how many points of a diagram lose precision in binary64, and how well the run-time
-indicators of the binary64 kernel (cond = sum|.|/|f| tracked at family granularity; inner = min(|A_t|, g_t,
+indicators of the binary64 kernel (cond = a/|f| with a the running bound on the sum of |monomial|; inner = min(|A_t|, g_t,
 pivot ratio)) predict it. Used to choose mc_options.cond_max / amin_min / deg_floor (DESIGN.md sections 6, 7).
+profiles/r1_precision_scan.md was written by an earlier version whose a was the sum of |family value|.
 
   python -m paper_1905_08007_b200.precision_scan [--points N] [--loops L --index I ...] > profiles/<name>.md
 
