@@ -130,7 +130,7 @@ int mc_integrate_host(const mc_diagram *, uint64_t first_sample, uint64_t n_samp
                       double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
 
 /* Batched form of the hot path: the same computation as mc_integrate for EVERY diagram of a set, with one
- * persistent kernel launch per precision tier for the whole set instead of three launches per diagram. The
+ * persistent kernel launch per precision tier for the whole set instead of four launches per diagram. The
  * paper's workload is a sum over thousands of graphs (Table 1 :112-124): per-diagram launches
  * leave the GPU idle in the tail of every launch (a point costs up to milliseconds in double-double), a set-wide
  * work queue has one tail per call. Work items are CTA-loads of points of one diagram; results do not depend on
@@ -157,7 +157,7 @@ void mc_batch_free(mc_batch *);
 /* Parity hook: per-point values for comparison with the oracle. DEVICE outputs, any may be NULL:
  * z_out n*M (row = point, column = line index), order_out n*M (the Hepp sector j_1..j_M),
  * p_out n (density), f_out n (value used by mc_integrate: binary64, or double-double rounded to
- * binary64 if flagged), f64_out n (plain binary64 value), cond_out n (sum|contrib|/|f|), flag_out n: 0 = accepted by the
+ * binary64 if re-evaluated), f64_out n (plain binary64 value), cond_out n (a/|f|), flag_out n: 0 = accepted by the
  * relative bound, 1 = re-evaluated in double-double (or beyond), 2 = precision loss detected but accepted by the absolute
  * bound on the weight (mc_diagram_set_precision). */
 int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
@@ -165,8 +165,8 @@ int mc_eval_points(const mc_diagram *, uint64_t first_sample, uint64_t n, uint64
                    double *cond_out, uint8_t *flag_out);
 
 /* Integrand at caller-supplied points (DEVICE z_in n*M): f64_out, fdd_out (double-double evaluation
- * rounded to binary64), cond_out (sum|contrib|/|f|), aux_out n*2 (min A_t, min x_t over the electron
- * lines of all pieces); any output may be NULL. */
+ * rounded to binary64), cond_out (a/|f|, a = the running bound on the sum of |monomial|), aux_out n*2 (amin = min |A_t|;
+ * xmin = min over pieces of pivot/diagonal ratio and g_t = 1 + A_t); any output may be NULL. */
 int mc_eval_z(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream,
               double *f64_out, double *fdd_out, double *cond_out, double *aux_out);
 
