@@ -189,7 +189,16 @@ struct StreamReader {
 template <class T, int KD>
 __device__ __forceinline__ T horner_raw(uint32_t &s_coef, const T *r) {
   if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8 * MQ_WL; return v; }   // the MQ_WL members of an entry are interleaved
-  else if constexpr (KD > 4) {                     // two-stage: 2^(KD-4) sub-blocks of kd = 4, combined over the top variables
+  else if constexpr (KD == 6 && sizeof(T) == sizeof(dd)) {   // double-double: the two halves in a real loop (half the code; integer overhead is free here)
+    T acc = T(0.0);
+#pragma unroll 1
+    for (int hh = 0; hh < 2; hh++) {
+      const T lo = horner_raw<T, 4>(s_coef, r), hi = horner_raw<T, 4>(s_coef, r);
+      const T t = mq_fma(hi, r[4], lo);
+      acc = hh ? mq_fma(t, r[5], acc) : t;
+    }
+    return acc;
+  } else if constexpr (KD > 4) {                     // two-stage: 2^(KD-4) sub-blocks of kd = 4, combined over the top variables
     constexpr int NS = 1 << (KD - 4);
     T s[NS];
 #pragma unroll
