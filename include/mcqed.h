@@ -33,6 +33,7 @@ extern "C" {
 #define MC_ENOMEM (-2)
 #define MC_ECUDA (-3)   /* CUDA runtime error or no device */
 #define MC_ELIMIT (-4)  /* graph exceeds a compiled-in limit */
+#define MC_ETOOBIG (-5) /* n_samples exceeds the capacity of the static scratch of mc_integrate_static */
 
 typedef struct mc_diagram mc_diagram; /* opaque; owns its host and device tables */
 
@@ -128,6 +129,26 @@ int mc_integrate(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, 
  * and synchronises the stream. For end-to-end use without touching device memory. */
 int mc_integrate_host(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
                       double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
+
+/* The binary64 tier of mc_integrate (steps a1-a7) for callers that cannot allocate: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc. Same kernels and launch configuration as mc_integrate on
+ * a handle with flags bit 0 set (no double-double pass: only points with a non-finite value or an underflowed coordinate are
+ * flagged; they contribute 0 and are counted in out_n_flagged), so the results are the same numbers. The per-call scratch
+ * (per-block partial sums, the flagged-index list, counters) lives in a file-scope `static __device__` array of the library
+ * instead of device memory owned by the handle: every GPU that loads the library holds MC_STATIC_SCRATCH_BYTES (0.65 MiB)
+ * until the process exits. The call makes no cudaMalloc / cudaFree / allocating library call. The first call on a device
+ * resolves the array's device address (cudaGetSymbolAddress, once per device, with that device current): make it outside
+ * stream capture. n_samples must not exceed MC_STATIC_MAX_SAMPLES (the flagged list holds one entry per sample in the worst
+ * case): MC_ETOOBIG otherwise, nothing launched; split longer ranges into several calls (results are additive).
+ * Every call on a device shares the one array, which keeps the last call's contents (the counters are cleared on the stream
+ * at the start of each call): calls whose kernels can overlap on the GPU (different streams, threads or processes sharing the
+ * context) race on it and give wrong sums without an error; calls on one stream are ordered and safe.
+ * out_* are DEVICE pointers, one element each, accumulated into (+=), any may be NULL. Asynchronous on cuda_stream.
+ * Errors: MC_EINVAL (NULL or host-only handle), MC_ETOOBIG, MC_ECUDA. */
+#define MC_STATIC_MAX_SAMPLES 65536
+#define MC_STATIC_SCRATCH_BYTES (256 + 32 * 148 * 32 + 8 * MC_STATIC_MAX_SAMPLES)
+int mc_integrate_static(const mc_diagram *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                        double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped);
 
 /* Batched form of the hot path: the same computation as mc_integrate for EVERY diagram of a set, with one
  * persistent kernel launch per precision tier for the whole set instead of four launches per diagram. The

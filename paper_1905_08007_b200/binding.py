@@ -10,14 +10,15 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ELIMIT = 0, -1, -2, -3, -4
+MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ELIMIT, MC_ETOOBIG = 0, -1, -2, -3, -4, -5
+STATIC_MAX_SAMPLES = 65536            # MC_STATIC_MAX_SAMPLES of include/mcqed.h
 FLAG_NO_DD, FLAG_NO_TABLES = 1, 2    # mc_options.flags
 FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
     "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags", "mc_diagram_set_precision",
-    "mc_integrate", "mc_integrate_host", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
+    "mc_integrate", "mc_integrate_host", "mc_integrate_static", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
 
@@ -72,6 +73,7 @@ def lib():
         L.mc_diagram_set_flags.argtypes = [vp, C.c_uint32]
         L.mc_diagram_set_precision.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_double]
         L.mc_integrate.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
+        L.mc_integrate_static.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp]
         L.mc_integrate_host.argtypes = [vp, u64, u64, u64, vp, dp, dp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.mc_batch_create.argtypes = [C.POINTER(vp), C.c_int32, u64, C.POINTER(vp)]
         L.mc_batch_integrate.argtypes = [vp, u64, u64, u64, C.c_uint32, vp, vp, vp, vp, vp]
@@ -189,6 +191,11 @@ class Diagram:
         """mc_integrate: out_* are device tensors/pointers (accumulated into); asynchronous on `stream` (int handle)"""
         _check(lib().mc_integrate(self.h, first_sample, n_samples, seed, _ptr(stream), _ptr(out_sum), _ptr(out_sumsq),
                                   _ptr(out_n_flagged), _ptr(out_n_dropped)), "mc_integrate")
+
+    def integrate_static(self, first_sample, n_samples, seed, stream, out_sum, out_sumsq, out_n_flagged, out_n_dropped):
+        """mc_integrate_static: binary64 tier, scratch in the library's static device array (no allocation); n_samples <= STATIC_MAX_SAMPLES"""
+        _check(lib().mc_integrate_static(self.h, first_sample, n_samples, seed, _ptr(stream), _ptr(out_sum), _ptr(out_sumsq),
+                                         _ptr(out_n_flagged), _ptr(out_n_dropped)), "mc_integrate_static")
 
     def integrate_host(self, first_sample, n_samples, seed, stream=None):
         s, s2, nf, nd = C.c_double(), C.c_double(), C.c_ulonglong(), C.c_ulonglong()

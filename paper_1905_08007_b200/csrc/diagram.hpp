@@ -108,6 +108,9 @@ void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed
 void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st);
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st);
 int mq_fp64_peak(int iters, mq_stream st, double *flops, double *ms);
+// binary64 tier with the scratch in a file-scope device array (kern_f64.cu); allocates nothing
+int mq_static_integrate_f64(const mc_diagram *d, uint64_t first, uint64_t n, uint64_t seed, mqk::MqPrec pr,
+                            double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);
 // batched path (kern_f64.cu / kern_dd.cu / kern_qd.cu)
 size_t mq_batch_smem_f64(int scal_len); size_t mq_batch_smem_dd(int scal_len); size_t mq_batch_smem_qd(int scal_len);
 int mq_batch_config_f64(size_t smem, int *grid); int mq_batch_config_dd(size_t smem, int *grid); int mq_batch_config_qd(size_t smem, int *grid);

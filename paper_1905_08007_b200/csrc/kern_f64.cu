@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "kern_common.cuh"
 
@@ -268,6 +269,49 @@ int mq_fp64_peak(int iters, mq_stream stream, double *flops, double *ms) {
   if (flops) *flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)blocks * tpb / (t * 1e-3);
   cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
   return (int)e;
+}
+
+// ---- mc_integrate_static: the binary64 tier with its scratch in a file-scope device array (no allocation at call time) ----
+// Layout of g_static_scratch: [ counters: 4 x u64 | partial: MAXGRID x 4 doubles | flag_list: MC_STATIC_MAX_SAMPLES x u64 ].
+// Every GPU that loads the library holds the array until the process exits; every call shares it (calls that overlap on
+// one GPU race). In host code the array's NAME is only a host-side stand-in: the device address comes from
+// cudaGetSymbolAddress, resolved once per device with that device current.
+namespace {
+constexpr size_t STATIC_OFF_PARTIAL = 256;                                                      // after the counters
+constexpr size_t STATIC_OFF_FLAGS = STATIC_OFF_PARTIAL + sizeof(double) * 4 * (size_t)mqk::MAXGRID;
+constexpr size_t STATIC_BYTES = STATIC_OFF_FLAGS + sizeof(unsigned long long) * (size_t)MC_STATIC_MAX_SAMPLES;
+static_assert(STATIC_OFF_FLAGS % 256 == 0, "flag list stays 256-byte aligned");
+constexpr int STATIC_MAXDEV = 64;
+void *g_static_ptr[STATIC_MAXDEV];                  // device address of g_static_scratch per device ordinal, nullptr = not resolved yet
+std::mutex g_static_mu;
+}  // namespace
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_BYTES];
+
+int mq_static_integrate_f64(const mc_diagram *d, uint64_t first, uint64_t n, uint64_t seed, mqk::MqPrec pr,
+                            double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream stream) {
+  int dev = -1;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= STATIC_MAXDEV) return (int)cudaErrorInvalidDevice;
+  unsigned char *base;
+  {
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+      void *p = nullptr;
+      if ((e = cudaGetSymbolAddress(&p, g_static_scratch)) != cudaSuccess) return (int)e;
+      g_static_ptr[dev] = p;
+    }
+    base = static_cast<unsigned char *>(g_static_ptr[dev]);
+  }
+  unsigned long long *counters = reinterpret_cast<unsigned long long *>(base);
+  double *partial = reinterpret_cast<double *>(base + STATIC_OFF_PARTIAL);
+  unsigned long long *flag_list = reinterpret_cast<unsigned long long *>(base + STATIC_OFF_FLAGS);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int grid = (int)std::min<uint64_t>((uint64_t)d->grid_f64, (n + PTS_F64 - 1) / PTS_F64);
+  k_reset_counters<<<1, 1, 0, st>>>(counters);      // the array keeps the last call's contents: the counters must start at zero
+  k_integrate_f64<<<grid, TPB_F64, d->smem_f64, st>>>(d->d_blob, first, n, seed, pr, partial, flag_list, counters);
+  k_finish<<<1, 32, 0, st>>>(partial, grid, 0, 0, counters, out_sum, out_sumsq, out_nflag, out_ndrop);
+  return (int)cudaGetLastError();
 }
 
 // ---- batched path launchers ----

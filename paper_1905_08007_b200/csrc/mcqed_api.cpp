@@ -157,6 +157,16 @@ int mc_integrate_host(const mc_diagram *d, uint64_t first_sample, uint64_t n_sam
   return MC_OK;
 }
 
+int mc_integrate_static(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
+                        double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
+  if (!d || !d->on_device) return MC_EINVAL;
+  if (n_samples > (uint64_t)MC_STATIC_MAX_SAMPLES) return MC_ETOOBIG;       // the static flagged list has one slot per sample
+  if (n_samples == 0) return MC_OK;
+  if (mq_static_integrate_f64(d, first_sample, n_samples, seed, d->prec(true), out_sum, out_sumsq, out_n_flagged, out_n_dropped, (mq_stream)cuda_stream) != 0) return MC_ECUDA;
+  g_launches += 3;
+  return MC_OK;
+}
+
 int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
                    double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out, uint8_t *flag_out) {
   if (!d || !d->on_device) return MC_EINVAL;
@@ -320,6 +330,7 @@ const char *mc_strerror(int code) {
     case MC_ENOMEM: return "out of memory";
     case MC_ECUDA: return "CUDA error or no CUDA device (this library has no CPU fallback)";
     case MC_ELIMIT: return "graph exceeds a compiled-in limit";
+    case MC_ETOOBIG: return "n_samples exceeds MC_STATIC_MAX_SAMPLES, the capacity of the static scratch of mc_integrate_static (split the range)";
   }
   return "unknown error";
 }
