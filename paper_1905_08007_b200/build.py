@@ -15,8 +15,9 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmcqed.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-NVCC_FLAGS = ARCH + ["-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "-Xptxas", "-v"] + os.environ.get("MCQED_NVCC_EXTRA", "").split()   # e.g. MCQED_NVCC_EXTRA=-DMQ_DUAL=0 for a tuning build
-GXX_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-ffp-contract=off", "-pthread", "-I/usr/local/cuda/include"]
+DEFS = os.environ.get("MCQED_DEFS", "").split()    # tuning builds: -D macros seen by BOTH compilers, e.g. MCQED_DEFS="-DMQ_WL=2 -DMQ_TPB_F64=128" (diagram.hpp, device_layout.h)
+NVCC_FLAGS = ARCH + ["-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "-Xptxas", "-v"] + DEFS + os.environ.get("MCQED_NVCC_EXTRA", "").split()   # e.g. MCQED_NVCC_EXTRA=-DMQ_DUAL=0 for a tuning build
+GXX_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-ffp-contract=off", "-pthread", "-I/usr/local/cuda/include"] + DEFS
 COMMON = ["device_layout.h", "host_model.hpp", "diagram.hpp", os.path.join("..", "..", "include", "mcqed.h")]
 KERN = COMMON + ["mcqed_kernels.cuh", "dd_arith.cuh", "kern_common.cuh"]
 UNITS = {  # object -> (compiler, source, dependencies)

@@ -13,7 +13,8 @@
 #define MQ_MAXCHILD 5
 #define MQ_NGRADE 6
 #define MQ_MAXGEOM 96
-#define MQ_MAXNODE 256
+#define MQ_MAXNODE 96          // nodes of the term trees of one diagram (max over all 6354 five-loop graphs: 95)
+#define MQ_MAXNODEVAL 544      // graded node values of one diagram (max over all five-loop graphs: 528)
 #define MQ_MAXPAT 16      // 2^(max #S-children of a piece)
 // inner dense binary dimensions of a family, by number of Wick pairs c (bounds the static code and the family size)
 // kd <= 4 blocks are evaluated by one Horner pass in registers (8 partial values); kd = 5, 6 blocks are 2 / 4 such blocks
@@ -21,10 +22,17 @@
 // families of a slot set that differ only in the P+/P- choice of outer lines: half the stream entries, a third fewer operand
 // gathers and scalar factors at 5-loop for 3 % more stored coefficients (measured). Caps keep an entry of MQ_WL families
 // below one chunk.
-static inline int mq_kd_max(int c) { return c <= 2 ? 6 : c == 3 ? 4 : 2; }
+#ifndef MQ_KD4
+#define MQ_KD4 2              // inner dimension cap of c = 4 families (1 lets an entry of 4 families fit a 1024-word chunk)
+#endif
+static inline int mq_kd_max(int c) { return c <= 2 ? 6 : c == 3 ? 4 : MQ_KD4; }
 #define MQ_MAXSCAL 12
-#define MQ_CHUNK_WORDS 1024   // staging granule of the family stream (8 KiB): the largest entry (MQ_WL families of c = 4, kd = 2) must fit
-#define MQ_WL 2               // families per stream entry = lanes that share one sample point in the binary64 / double-double kernels
+#ifndef MQ_WL
+#define MQ_WL 4               // families per stream entry = lanes that share one point group (MQ_NP points in binary64, 1 in double-double)
+#endif
+#ifndef MQ_CHUNK_WORDS
+#define MQ_CHUNK_WORDS (MQ_WL > 2 ? 2048 : 1024)   // staging granule of the family stream (8 / 16 KiB): the largest entry (MQ_WL families of c = 4, kd = 2) must fit
+#endif
 #define MQ_PAD_MARK 7        // header field c of a PAD entry
 
 enum { MQ_OP_A = 0, MQ_OP_U = 1, MQ_OP_L = 2, MQ_OP_LMU = 3 };
@@ -71,7 +79,7 @@ struct DevTerm { int32_t root, sign; };
 
 struct DevHeader {
   int32_t L, M, diag_id, ngeom, ntable, nnode, nterm, nodeval_len;
-  int32_t max_scal_len, pad0;
+  int32_t max_scal_len, wl;               // wl = MQ_WL the streams were laid out for
   double C, cond_max;
   int64_t off_Z, off_invdeg, off_geom, off_table, off_node, off_term, total_words;
   int64_t off_stream, stream_chunks;      // the family streams: stream_chunks chunks of MQ_CHUNK_WORDS words
@@ -86,7 +94,8 @@ struct DevHeader {
 //   bits  6..9  pattern (compressed)           bits 10..13 nscal (#extra scalar factors)
 //   bits 14     out (0/1: which output of an S-type piece)                  bit 15  VOID member
 //   bits 16..31 idx_words: 8-byte words of index bytes PER MEMBER
-//   bits 32..63 number of coefficient doubles of the WHOLE entry (MQ_WL x per family)
+//   bits 32..47 number of coefficient doubles of the WHOLE entry (MQ_WL x per family)
+//   bits 48..63 run length: entries from this one to the end of its run of equal shape (c, kd) within the table (>= 1)
 //   (c, kd, idx_words and the coefficient count are the same in all MQ_WL header words)
 // index bytes of member s: C(2c,2) beta~ indices of its paired slots (pair (i<j) at i*2c - i(i+1)/2 + j-i-1) | kd inner
 //   binary slot ids | nscal scalar-factor indices; all are direct indices into the per-point scalar array S

@@ -9,13 +9,27 @@
 #include "host_model.hpp"
 
 namespace mqk {
-constexpr int TPB_F64 = 256, TPB_DD = 128, TPB_EVAL = 128;
+// binary64 tier: a lane carries NP_F64 sample points (pt2_arith.cuh: every loaded table coefficient feeds NP_F64 FMAs)
+#ifndef MQ_NP
+#define MQ_NP 4
+#endif
+#ifndef MQ_TPB_F64
+#define MQ_TPB_F64 128
+#endif
+#ifndef MQ_MINB_F64
+#define MQ_MINB_F64 2
+#endif
+#ifndef MQ_TPB_DD
+#define MQ_TPB_DD 128
+#endif
+constexpr int NP_F64 = MQ_NP;    // 1, 2 or 4
+constexpr int TPB_F64 = MQ_TPB_F64, TPB_DD = MQ_TPB_DD, TPB_EVAL = 128;
 // warp split (mcqed_kernels.cuh): W warps share one group of points. Measured on B200 before the lane split existed
 // (profiles/r1_summary.md): W = 2 doubles the resident warps but is slower than W = 1 (binary64 11.9 % vs 13.5 % of peak on a
 // subtraction-free graph; double-double 2.6e5 vs 4.2e5 points/s on a 12-term graph), so W = 1; the lane split (MQ_WL lanes of a
 // warp per point, device_layout.h) is what doubles the resident warps now.
 constexpr int W_F64 = 1, W_DD = 1;
-constexpr int PTS_F64 = TPB_F64 / (W_F64 * MQ_WL), PTS_DD = TPB_DD / (W_DD * MQ_WL), PTS_EVAL = TPB_EVAL / (W_F64 * MQ_WL);   // points per CTA (MQ_WL lanes per point)
+constexpr int PTS_F64 = TPB_F64 / (W_F64 * MQ_WL) * NP_F64, PTS_DD = TPB_DD / (W_DD * MQ_WL), PTS_EVAL = TPB_EVAL / (W_F64 * MQ_WL) * NP_F64;   // points per CTA (MQ_WL lanes share NP points)
 constexpr uint64_t CHUNK = 1ull << 22;     // samples per launch (bounds the flagged-index list)
 constexpr int MAXGRID = 148 * 32;
 // precision policy of one diagram as the kernels see it (O8; include/mcqed.h mc_diagram_set_precision)

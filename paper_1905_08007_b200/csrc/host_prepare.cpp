@@ -140,7 +140,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     N.val_off = d->nodeval_len; d->nodeval_len += N.nout * N.ngr;
     d->nodes[ni] = N;
   }
-  if (d->nodeval_len > 1024) return MC_ELIMIT;
+  if (d->nodeval_len > MQ_MAXNODEVAL) return MC_ELIMIT;
   for (size_t ti = 0; ti < d->tables.size(); ti++) {
     DevGeom &G = d->geoms[d->tables[ti].geom];
     if (G.ntable == 0) G.first_table = (int)ti;
@@ -163,7 +163,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   auto words = [](size_t bytes) { return (int64_t)((bytes + 7) / 8); };
   DevHeader H; std::memset(&H, 0, sizeof H);
   H.L = d->g.L; H.M = d->g.M; H.diag_id = d->id; H.ngeom = ngeom0; H.ntable = (int)d->tables.size(); H.nnode = nnode0; H.nterm = (int)d->terms.size();
-  H.nodeval_len = d->nodeval_len; H.max_scal_len = d->max_scal_len; H.C = d->st.C; H.cond_max = d->opt.cond_max;
+  H.nodeval_len = d->nodeval_len; H.max_scal_len = d->max_scal_len; H.wl = MQ_WL; H.C = d->st.C; H.cond_max = d->opt.cond_max;
   int64_t off = words(sizeof(DevHeader));
   const int64_t nZ = (int64_t)1 << d->g.M;
   H.off_Z = off; off += nZ; H.off_invdeg = off; off += nZ;
@@ -209,6 +209,8 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
       return true;
     };
     int nentries = 0;
+    std::vector<size_t> entry_at;                                              // stream position of every entry header of this table
+    std::vector<int> entry_shape;
     for (size_t at0 = 0; at0 < order.size();) {
       const mq::Family &f0 = *order[at0];
       int nm = 1;                                                              // members of this entry (same shape), the rest is VOID
@@ -229,9 +231,10 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
         streams.push_back(mq_pack_family(7, 0, 0, 0, 0, (int)(rest - 1), 0u));
         streams.resize(streams.size() + (size_t)(rest - 1), 0ull);
       }
+      entry_at.push_back(streams.size()); entry_shape.push_back(f0.c * 8 + f0.kd);
       for (int m = 0; m < MQ_WL; m++) {
         const mq::Family &f = m < nm ? *order[at0 + m] : f0;
-        if (f.coef.size() != ncf) return MC_ELIMIT;
+        if (f.coef.size() != ncf || MQ_WL * ncf > 0xFFFF) return MC_ELIMIT;
         streams.push_back(mq_pack_family(f.c, f.kd, f.pattern, m < nm ? (int)f.scal.size() : 0, f.out, idxw, (uint32_t)(MQ_WL * ncf), m < nm ? 0 : 1));
       }
       for (int m = 0; m < MQ_WL; m++) {
@@ -246,6 +249,13 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
         for (size_t u = 0; u < nunit; u++) std::memcpy(streams.data() + at + (u * MQ_WL + m) * unit, src + u * unit, sizeof(double) * unit);
       }
       at0 += nm; nentries++;
+    }
+    // run lengths: bits 48..63 of every header word = entries from this one to the end of its run of equal shape (c, kd);
+    // the kernels take the shape switch once per run (mcqed_kernels.cuh run_loop)
+    for (size_t i = entry_at.size(); i-- > 0;) {
+      const uint64_t run = (i + 1 < entry_at.size() && entry_shape[i + 1] == entry_shape[i]) ? (streams[entry_at[i + 1]] >> 48) + 1 : 1;
+      if (run > 0xFFFF) return MC_ELIMIT;
+      for (int m = 0; m < MQ_WL; m++) streams[entry_at[i] + m] |= run << 48;
     }
     T.nfam = nentries;
     T.stream_words = stream_base + (int64_t)streams.size() - T.stream_off;

@@ -63,6 +63,29 @@ __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   
   for (int i = 0; i < M; i++) bad |= !(z[i] >= 0x1p-600);
   return bad;
 }
+template <int N> __device__ __forceinline__ bool bad_point(const ptn<N> *z, int k, int M, double p) {   // the same for point k of a lane that carries N
+  bool bad = !(p > 0.0) || !isfinite(p);
+  for (int i = 0; i < M; i++) bad |= !(mq_comp(z[i], k) >= 0x1p-600);
+  return bad;
+}
+__device__ __forceinline__ bool bad_point(const double *z, int, int M, double p) { return bad_point(z, M, p); }
+
+// draws the PtsOf<T>::n sample points of this lane: indices first + min(i0 + k, n - 1), k = 0, 1 (surplus slots redo the last
+// point and are discarded by the caller); z[line] holds the coordinates of both, p[k] the densities
+template <class T, bool WANT_ORDER>
+__device__ __forceinline__ void draw_points(const DiagView &v, uint64_t first, uint64_t i0, uint64_t n, uint64_t seed, typename MagOf<T>::type *z, double *p, int32_t *order_out) {
+  constexpr int NP = PtsOf<T>::n;
+  if constexpr (NP == 1) p[0] = draw_point<WANT_ORDER>(v, first + (i0 < n ? i0 : n - 1), seed, z, order_out);
+  else {
+    const int M = v.h->M;
+#pragma unroll 1
+    for (int k = 0; k < NP; k++) {
+      double zz[MQ_MAXM];
+      p[k] = draw_point<WANT_ORDER>(v, first + (i0 + k < n ? i0 + k : n - 1), seed, zz, WANT_ORDER ? order_out + k * MQ_MAXM : nullptr);
+      for (int j = 0; j < M; j++) mq_setc(z[j], k, zz[j]);
+    }
+  }
+}
 
 // Precision decision of one tier (O8). a = sum of |monomial| bounds carried by the evaluator (sum|c| of every
 // coefficient block x |pairing weight| x |scalar factors|, through the whole tree), amin = min |A_t| over the electron lines
@@ -97,14 +120,14 @@ __host__ __device__ inline size_t smem_bytes(int scal_len, int threads, size_t e
 }
 template <class T, int W, int WLX> struct Roles {
   int gw, sub, slot, P;     // role of this warp in its group, role of this lane for its point, point slot of this lane in the CTA, points per CTA
-  T *S, *xT; double *xA;
+  unsigned char *S; T *xT; typename MagOf<T>::type *xA;   // S: this lane's slot base of the scalar scratch (SAcc<T>, mcqed_kernels.cuh)
   __device__ __forceinline__ Roles(unsigned char *smem, int scal_len) {
     constexpr int PPW = 32 / WLX;
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
     gw = w % W; sub = l / PPW; P = blockDim.x / (W * WLX); slot = (w / W) * PPW + l % PPW;
-    S = reinterpret_cast<T *>(smem) + slot;
+    S = smem + (size_t)slot * SAcc<T>::slot_bytes;
     xT = reinterpret_cast<T *>(smem) + (size_t)scal_len * P + slot;
-    xA = reinterpret_cast<double *>(smem + ((size_t)scal_len * P + (size_t)(W - 1) * MQ_NGRADE * P) * sizeof(T)) + slot;
+    xA = reinterpret_cast<typename MagOf<T>::type *>(smem + ((size_t)scal_len * P + (size_t)(W - 1) * MQ_NGRADE * P) * sizeof(T)) + slot;
   }
 };
 template <int W, int WLX> __device__ __forceinline__ void setup_reader(StreamReader &rd, unsigned char *smem, int scal_len, size_t elem) {

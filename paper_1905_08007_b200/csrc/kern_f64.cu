@@ -4,33 +4,45 @@
 
 #include <algorithm>
 #include <mutex>
+#include <type_traits>
 
 #include "kern_common.cuh"
 
 namespace mqk {
 
+// value type of the binary64 tier: pt2 = two sample points per lane (pt2_arith.cuh), double = one
+using FT = std::conditional<NP_F64 == 4, pt4, std::conditional<NP_F64 == 2, pt2, double>::type>::type;
+using FM = MagOf<FT>::type;
+constexpr int NP = PtsOf<FT>::n;
+
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
-__global__ void __launch_bounds__(TPB_F64, 2) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
+__global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
                                                            MqPrec pr, double *partial,
                                                            unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
+  const Roles<FT, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(FT));
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
   // the evaluator is CTA-collective (it stages the table stream through shared memory and splits the families of a
   // point group over W warps): every thread of the CTA runs the same number of iterations; slots past the end
   // re-evaluate the last point and discard it; only the owner warp (gw = 0) of a group draws and accumulates
-  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0 && ro.sub == 0;
-    double z[MQ_MAXM]; double p = 1.0;
-    if (ro.gw == 0) p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
-    double f, a, amin, xmin;
-    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if (!live) continue;
-    const bool flag = tier_decision(bad_point(z, v.h->M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
-    if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i; }
-    else { const double w = f / p; s1.add(w); s2.add(w * w); }
+  const uint64_t per = (uint64_t)ro.P * NP;
+  for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
+    const uint64_t i0 = base + (uint64_t)ro.slot * NP;
+    FM z[MQ_MAXM]; double p[NP];
+    if (ro.gw == 0) draw_points<FT, false>(v, first, i0, n, seed, z, p, nullptr);
+    FT f, a; FM amin, xmin;
+    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    if (ro.gw != 0 || ro.sub != 0) continue;
+#pragma unroll
+    for (int k = 0; k < NP; k++) {
+      if (i0 + k >= n) continue;
+      const double fk = mq_comp(f, k);
+      const bool flag = tier_decision(bad_point(z, k, v.h->M, p[k]), fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+      if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i0 + k; }
+      else { const double w = fk / p[k]; s1.add(w); s2.add(w * w); }
+    }
   }
   block_reduce_store(s1, s2, partial);
 }
@@ -60,26 +72,32 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
                                                           double *cond_out, uint8_t *flag_out, unsigned long long *flag_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  const Roles<FT, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
   const int M = v.h->M;
-  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
-  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const uint64_t i = base + ro.slot; const bool live = i < n && ro.gw == 0 && ro.sub == 0;
-    double z[MQ_MAXM]; int32_t ord[MQ_MAXM]; double p = 1.0;
-    if (ro.gw == 0) p = draw_point<true>(v, first + (i < n ? i : n - 1), seed, z, ord);
-    double f, a, amin, xmin;
-    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if (!live) continue;
-    const int dec = tier_decision(bad_point(z, M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
-    const bool flag = dec == 1;
-    if (z_out) for (int k = 0; k < M; k++) z_out[i * M + k] = z[k];
-    if (order_out) for (int k = 0; k < M; k++) order_out[i * M + k] = ord[k];
-    if (p_out) p_out[i] = p;
-    if (f_out) f_out[i] = f;
-    if (f64_out) f64_out[i] = f;
-    if (cond_out) cond_out[i] = a / fabs(f);
-    if (flag_out) flag_out[i] = (uint8_t)dec;      // 0 accepted (relative), 1 re-evaluated in double-double, 2 accepted by the absolute bound on w
-    if (flag && flag_list) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = i; }
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(FT));
+  const uint64_t per = (uint64_t)ro.P * NP;
+  for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
+    const uint64_t i0 = base + (uint64_t)ro.slot * NP;
+    FM z[MQ_MAXM]; int32_t ord[NP * MQ_MAXM]; double p[NP];
+    if (ro.gw == 0) draw_points<FT, true>(v, first, i0, n, seed, z, p, ord);
+    FT f, a; FM amin, xmin;
+    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    if (ro.gw != 0 || ro.sub != 0) continue;
+    for (int k = 0; k < NP; k++) {
+      const uint64_t i = i0 + k;
+      if (i >= n) continue;
+      const double fk = mq_comp(f, k);
+      const int dec = tier_decision(bad_point(z, k, M, p[k]), fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
+      const bool flag = dec == 1;
+      if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = mq_comp(z[j], k);
+      if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[k * MQ_MAXM + j];
+      if (p_out) p_out[i] = p[k];
+      if (f_out) f_out[i] = fk;
+      if (f64_out) f64_out[i] = fk;
+      if (cond_out) cond_out[i] = mq_comp(a, k) / fabs(fk);
+      if (flag_out) flag_out[i] = (uint8_t)dec;      // 0 accepted (relative), 1 re-evaluated in double-double, 2 accepted by the absolute bound on w
+      if (flag && flag_list) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = i; }
+    }
   }
 }
 
@@ -88,30 +106,37 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
-  const Roles<double, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
-  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(double));
-  for (uint64_t base = (uint64_t)blockIdx.x * ro.P; base < n; base += (uint64_t)gridDim.x * ro.P) {
-    const bool live = base + ro.slot < n && ro.gw == 0 && ro.sub == 0;
-    const uint64_t i = base + ro.slot < n ? base + ro.slot : n - 1;           // surplus slots redo the last point
-    double z[MQ_MAXM];
-    for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
-    double f, a, amin, xmin;
-    eval_integrand<double, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if (!live) continue;
-    if (f64_out) f64_out[i] = f;
-    if (cond_out) cond_out[i] = a / fabs(f);
-    if (aux_out) { aux_out[2 * i] = amin; aux_out[2 * i + 1] = xmin; }
+  const Roles<FT, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
+  StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(FT));
+  const uint64_t per = (uint64_t)ro.P * NP;
+  for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
+    const uint64_t i0 = base + (uint64_t)ro.slot * NP;
+    FM z[MQ_MAXM];
+    for (int k = 0; k < NP; k++) {
+      const uint64_t i = i0 + k < n ? i0 + k : n - 1;                         // surplus slots redo the last point
+      for (int j = 0; j < MQ_MAXM; j++) mq_setc(z[j], k, j < M ? z_in[i * M + j] : 0.0);
+    }
+    FT f, a; FM amin, xmin;
+    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    if (ro.gw != 0 || ro.sub != 0) continue;
+    for (int k = 0; k < NP; k++) {
+      const uint64_t i = i0 + k;
+      if (i >= n) continue;
+      if (f64_out) f64_out[i] = mq_comp(f, k);
+      if (cond_out) cond_out[i] = mq_comp(a, k) / fabs(mq_comp(f, k));
+      if (aux_out) { aux_out[2 * i] = mq_comp(amin, k); aux_out[2 * i + 1] = mq_comp(xmin, k); }
+    }
   }
 }
 
 // ------------------------------------------------------------------ batched path, binary64 tier (a1-a7 for every diagram of a batch)
 // Persistent CTAs; item = PTS_F64 consecutive sample indices of one diagram, taken from queue[0].
 // Flagged points are compacted inside the item in thread order (ballot + prefix): deterministic lists.
-__global__ void __launch_bounds__(TPB_F64, 2) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
+__global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item, s_wcnt[TPB_F64 / 32];
-  const Roles<double, 1, MQ_WL> ro(smem_raw, scal_len);
-  StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(double));
+  const Roles<FT, 1, MQ_WL> ro(smem_raw, scal_len);
+  StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(FT));
   const uint32_t total = (uint32_t)bv.nd * bv.ipd;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (;;) {
@@ -124,22 +149,33 @@ __global__ void __launch_bounds__(TPB_F64, 2) k_batch_f64(BatchView bv, uint64_t
     const DiagView v = make_view(bv.dg[d].blob);
     MqPrec pr = bv.dg[d].pr;
     if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
-    const uint64_t i = (uint64_t)b * PTS_F64 + ro.slot; const bool live = i < n && ro.sub == 0;
-    double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + (i < n ? i : n - 1), seed, z, nullptr);
-    double f, a, amin, xmin;
-    eval_integrand<double, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
-    const bool flag = live && tier_decision(bad_point(z, v.h->M, p), f, a, amin, xmin, p, pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
-    const unsigned bal = __ballot_sync(0xffffffffu, flag);
-    if (lane == 0) s_wcnt[warp] = __popc(bal);
+    const uint64_t i0 = (uint64_t)b * PTS_F64 + (uint64_t)ro.slot * NP;
+    FM z[MQ_MAXM]; double p[NP];
+    draw_points<FT, false>(v, first, i0, n, seed, z, p, nullptr);
+    FT f, a; FM amin, xmin;
+    eval_integrand<FT, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
+    // flagged points of the item, compacted in (lane, point) order = ascending sample index
+    bool flag[NP]; unsigned bal[NP]; unsigned mine = 0, wsum = 0;
+#pragma unroll
+    for (int k = 0; k < NP; k++) {
+      const bool live = i0 + k < n && ro.sub == 0;
+      flag[k] = live && tier_decision(bad_point(z, k, v.h->M, p[k]), mq_comp(f, k), mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+      bal[k] = __ballot_sync(0xffffffffu, flag[k]);
+      mine += __popc(bal[k] & ((1u << lane) - 1u)); wsum += __popc(bal[k]);
+    }
+    if (lane == 0) s_wcnt[warp] = wsum;
     __syncthreads();
     unsigned before = 0, all = 0;
 #pragma unroll
     for (int w = 0; w < TPB_F64 / 32; w++) { if (w < warp) before += s_wcnt[w]; all += s_wcnt[w]; }
-    if (flag) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + before + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)i;
-    if (threadIdx.x == 0) bv.item_cnt[(size_t)d * (bv.cap / PTS_F64) + b] = all;
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-    if (live && !flag) { const double w = f / p; s1.add(w); s2.add(w * w); }
+    unsigned pos = before + mine;
+#pragma unroll
+    for (int k = 0; k < NP; k++) {
+      if (flag[k]) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + pos++] = (uint32_t)(i0 + k);
+      else if (i0 + k < n && ro.sub == 0) { const double w = mq_comp(f, k) / p[k]; s1.add(w); s2.add(w * w); }
+    }
+    if (threadIdx.x == 0) bv.item_cnt[(size_t)d * (bv.cap / PTS_F64) + b] = all;
     block_reduce_to(s1, s2, bv.part_f64 + (size_t)item * 4);
   }
 }
@@ -221,8 +257,8 @@ __global__ void k_fp64_peak(int iters, double *sink) {
 using namespace mqk;
 
 int mq_config_f64(mc_diagram *d) {
-  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(double), W_F64, MQ_WL);
-  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(double), W_F64, MQ_WL);
+  d->smem_f64 = smem_bytes(d->max_scal_len, TPB_F64, sizeof(FT), W_F64, MQ_WL);
+  d->smem_eval = smem_bytes(d->max_scal_len, TPB_EVAL, sizeof(FT), W_F64, MQ_WL);
   cudaError_t e;
   if ((e = allow_max_smem(k_integrate_f64)) != cudaSuccess) return (int)e;
   if ((e = allow_max_smem(k_eval_points)) != cudaSuccess) return (int)e;
@@ -326,7 +362,7 @@ int mq_batch_config_f64(size_t smem, int *grid) {
   *grid = nsm * occ;
   return 0;
 }
-size_t mq_batch_smem_f64(int scal_len) { return smem_bytes(scal_len, TPB_F64, sizeof(double), 1, MQ_WL); }
+size_t mq_batch_smem_f64(int scal_len) { return smem_bytes(scal_len, TPB_F64, sizeof(FT), 1, MQ_WL); }
 void mq_launch_batch_f64(const BatchView &bv, int grid, size_t smem, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd, mq_stream st) {
   k_batch_f64<<<grid, TPB_F64, smem, (cudaStream_t)st>>>(bv, first, n, seed, scal_len, no_dd);
 }

@@ -11,11 +11,17 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "dd_arith.cuh"
+#include "pt2_arith.cuh"
 #include "device_layout.h"
 
 namespace mqk {
 
+// value types whose family code keeps the outer pairing levels (c >= 3) and the halves of a kd = 6 block in real loops:
+// everything but plain binary64 (double-double: code size; N points per lane: registers)
+#define MQ_LOOPED(T) (!std::is_same<T, double>::value)
 #ifndef MQ_DUAL
 #define MQ_DUAL 1     // binary64: evaluate two consecutive same-shape entries together (independent chains)
 #endif
@@ -132,6 +138,35 @@ __device__ __forceinline__ double lds_f64(uint32_t a) { double v; asm volatile("
 template <class T> __device__ __forceinline__ T lds_T(uint32_t a);
 template <> __device__ __forceinline__ double lds_T<double>(uint32_t a) { return lds_f64(a); }
 template <> __device__ __forceinline__ dd lds_T<dd>(uint32_t a) { double2 v = lds_f64x2(a); return dd(v.x, v.y); }
+// Access to the per-point scalar scratch S[index][slot] of a CTA (stride = slots per CTA; S = this lane's slot base).
+// Scalar types: one element of sizeof(T) per (index, slot). ptn<N>: N/2 planes of 16-byte point pairs per index,
+// [index][plane][slot], so that the lanes of a warp read consecutive 16-byte units (no bank conflicts for any N).
+// lds(a, sstride): a = shared address of (index, this slot), sstride = bytes per index = stride * sizeof(T).
+template <class T> struct SAcc {
+  static constexpr int slot_bytes = sizeof(T);
+  static __device__ __forceinline__ T lds(uint32_t a, uint32_t) { return lds_T<T>(a); }
+  static __device__ __forceinline__ T ld(const unsigned char *S, int i, int stride) { return reinterpret_cast<const T *>(S)[(size_t)i * stride]; }
+  static __device__ __forceinline__ void st(unsigned char *S, int i, int stride, T v) { reinterpret_cast<T *>(S)[(size_t)i * stride] = v; }
+};
+template <int N> struct SAcc<ptn<N>> {
+  static constexpr int slot_bytes = 16, NPL = N / 2;
+  static __device__ __forceinline__ ptn<N> lds(uint32_t a, uint32_t sstride) {
+    ptn<N> r;
+#pragma unroll
+    for (int h = 0; h < NPL; h++) { const double2 v = lds_f64x2(a + h * (sstride / NPL)); r.v[2 * h] = v.x; r.v[2 * h + 1] = v.y; }
+    return r;
+  }
+  static __device__ __forceinline__ ptn<N> ld(const unsigned char *S, int i, int stride) {
+    ptn<N> r;
+#pragma unroll
+    for (int h = 0; h < NPL; h++) { const double2 v = reinterpret_cast<const double2 *>(S)[(size_t)(i * NPL + h) * stride]; r.v[2 * h] = v.x; r.v[2 * h + 1] = v.y; }
+    return r;
+  }
+  static __device__ __forceinline__ void st(unsigned char *S, int i, int stride, ptn<N> x) {
+#pragma unroll
+    for (int h = 0; h < NPL; h++) reinterpret_cast<double2 *>(S)[(size_t)(i * NPL + h) * stride] = make_double2(x.v[2 * h], x.v[2 * h + 1]);
+  }
+};
 
 // The family stream of a diagram is staged through shared memory in chunks of MQ_CHUNK_WORDS words by bulk
 // asynchronous copies (cp.async.bulk + mbarrier, the TMA engine; SASS UBLKCP), two chunks in flight, so that
@@ -189,7 +224,7 @@ struct StreamReader {
 template <class T, int KD>
 __device__ __forceinline__ T horner_raw(uint32_t &s_coef, const T *r) {
   if constexpr (KD == 0) { T v = T(lds_f64(s_coef)); s_coef += 8 * MQ_WL; return v; }   // the MQ_WL members of an entry are interleaved
-  else if constexpr (KD == 6 && sizeof(T) == sizeof(dd)) {   // double-double: the two halves in a real loop (half the code; integer overhead is free here)
+  else if constexpr (KD == 6 && MQ_LOOPED(T)) {   // double-double: the two halves in a real loop (half the code; integer overhead is free here)
     T acc = T(0.0);
 #pragma unroll 1
     for (int hh = 0; hh < 2; hh++) {
@@ -227,8 +262,6 @@ __device__ __forceinline__ T horner_raw(uint32_t &s_coef, const T *r) {
   }
 }
 // one pairing block: its value, and l1 = sum |c| from the block's closing unit (kd = 0: |c| itself) for the round-off bound
-__device__ __forceinline__ double mq_absd(double a) { return fabs(a); }
-__device__ __forceinline__ double mq_absd(dd a) { return fabs(a.hi); }
 template <class T, int KD>
 __device__ __forceinline__ T horner(uint32_t &s_coef, const T *r, double &l1) {
   if constexpr (KD == 0) { const double c0 = lds_f64(s_coef); s_coef += 8 * MQ_WL; l1 = fabs(c0); return T(c0); }
@@ -252,7 +285,7 @@ constexpr int ctz_c(unsigned x) { int n = 0; while (!(x & 1u)) { x >>= 1; n++; }
 
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec;
 template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> struct PairStep {
-  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, double &asum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, typename MagOf<T>::type &asum) {
     if constexpr (S < N2) {
       if constexpr (!((USED >> S) & 1u)) {
         if constexpr (FIRST) PairRec<T, KD, N2, (USED | (1u << F) | (1u << S)), false>::run(b, b[pair_index<N2>(F, S)], s_coef, r, sum, asum);
@@ -264,12 +297,12 @@ template <class T, int KD, int N2, unsigned USED, bool FIRST, int F, int S> stru
 };
 // sum += w_pairing * block, asum += |w_pairing| * sum|c|  (the latter bounds the block by sum|c| prod max(1,|r|), applied by the caller)
 template <class T, int KD, int N2, unsigned USED, bool FIRST> struct PairRec {
-  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, double &asum) {
+  static __device__ __forceinline__ void run(const T *b, T w, uint32_t &s_coef, const T *r, T &sum, typename MagOf<T>::type &asum) {
     if constexpr (USED == ((1u << N2) - 1u)) {
       double l1;
       T h = horner<T, KD>(s_coef, r, l1);
-      if constexpr (FIRST) { sum = h; asum = l1; }   // FIRST at a leaf: no pairs, one block
-      else { sum = mq_fma(w, h, sum); asum = fma(mq_absd(w), l1, asum); }
+      if constexpr (FIRST) { sum = h; asum = typename MagOf<T>::type(l1); }   // FIRST at a leaf: no pairs, one block
+      else { sum = mq_fma(w, h, sum); asum = mq_mfma(mq_absd(w), l1, asum); }
     } else {
       constexpr int F = ctz_c(~USED);
       PairStep<T, KD, N2, USED, FIRST, F, F + 1>::run(b, w, s_coef, r, sum, asum);
@@ -318,11 +351,11 @@ __constant__ PairTbl4 c_tbl4 = make_tbl4();
 
 // the three pairings of four slots a<b<c<d, each with prefix weight wp: g = (ab, ac, ad, bc, bd, cd)
 template <class T, int KD>
-__device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, const T *r, T &sum, double &asum) {
+__device__ __forceinline__ void pair_body4(T wp, const T *g, uint32_t &s_coef, const T *r, T &sum, typename MagOf<T>::type &asum) {
   double l1; T w;
-  w = mq_mul(mq_mul(wp, g[0]), g[5]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ab)(cd)
-  w = mq_mul(mq_mul(wp, g[1]), g[4]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ac)(bd)
-  w = mq_mul(mq_mul(wp, g[2]), g[3]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = fma(mq_absd(w), l1, asum);     // (ad)(bc)
+  w = mq_mul(mq_mul(wp, g[0]), g[5]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = mq_mfma(mq_absd(w), l1, asum);     // (ab)(cd)
+  w = mq_mul(mq_mul(wp, g[1]), g[4]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = mq_mfma(mq_absd(w), l1, asum);     // (ac)(bd)
+  w = mq_mul(mq_mul(wp, g[2]), g[3]); sum = mq_fma(w, horner<T, KD>(s_coef, r, l1), sum); asum = mq_mfma(mq_absd(w), l1, asum);     // (ad)(bc)
 }
 
 // byte i (compile-time) of an array of 64-bit index words: one PRMT
@@ -332,16 +365,16 @@ template <int I> __device__ __forceinline__ uint32_t idx_byte(const uint64_t *iw
 }
 template <class T, int N, int OFF, int I = 0> struct Gather {
   static __device__ __forceinline__ void run(const uint64_t *iw, uint32_t s_S, uint32_t sstride, T *out) {
-    if constexpr (I < N) { out[I] = lds_T<T>(s_S + idx_byte<OFF + I>(iw) * sstride); Gather<T, N, OFF, I + 1>::run(iw, s_S, sstride, out); }
+    if constexpr (I < N) { out[I] = SAcc<T>::lds(s_S + idx_byte<OFF + I>(iw) * sstride, sstride); Gather<T, N, OFF, I + 1>::run(iw, s_S, sstride, out); }
   }
 };
 
 // value of a family and its round-off magnitude a = sum_pairings |w| sum|c| prod_inner max(1,|r|) >= sum of |monomial|
-template <class T> struct FamRes { T v; double a; };
-template <class T, int KD> __device__ __forceinline__ double rbound(const T *r) {
-  double R = 1.0;
+template <class T> struct FamRes { T v; typename MagOf<T>::type a; };
+template <class T, int KD> __device__ __forceinline__ typename MagOf<T>::type rbound(const T *r) {
+  typename MagOf<T>::type R(1.0);
 #pragma unroll
-  for (int i = 0; i < KD; i++) R *= fmax(1.0, mq_absd(r[i]));
+  for (int i = 0; i < KD; i++) R = R * mq_mmax1(mq_absd(r[i]));
   return R;
 }
 
@@ -350,28 +383,28 @@ template <class T, int C, int KD>
 __device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
   constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
   FamRes<T> res;
-  if constexpr (C >= 3 && sizeof(T) == sizeof(dd)) {
+  if constexpr (C >= 3 && MQ_LOOPED(T)) {
     T r[KD > 0 ? KD : 1];
 #pragma unroll
-    for (int i = 0; i < KD; i++) r[i] = lds_T<T>(s_S + lds_u8(s_idx + NB + i) * sstride);
-    T sum = T(0.0); double asum = 0.0;
+    for (int i = 0; i < KD; i++) r[i] = SAcc<T>::lds(s_S + lds_u8(s_idx + NB + i) * sstride, sstride);
+    T sum = T(0.0); typename MagOf<T>::type asum(0.0);
     if constexpr (C == 3) {
 #pragma unroll 1
       for (int j = 0; j < 5; j++) {
         T g[7];
 #pragma unroll
-        for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl3.p[j][k]) * sstride);
+        for (int k = 0; k < 7; k++) g[k] = SAcc<T>::lds(s_S + lds_u8(s_idx + c_tbl3.p[j][k]) * sstride, sstride);
         pair_body4<T, KD>(g[0], g + 1, s_coef, r, sum, asum);
       }
     } else {
 #pragma unroll 1
       for (int j1 = 0; j1 < 7; j1++) {
-        const T w1 = lds_T<T>(s_S + lds_u8(s_idx + c_tbl4.o[j1]) * sstride);
+        const T w1 = SAcc<T>::lds(s_S + lds_u8(s_idx + c_tbl4.o[j1]) * sstride, sstride);
 #pragma unroll 1
         for (int j2 = 0; j2 < 5; j2++) {
           T g[7];
 #pragma unroll
-          for (int k = 0; k < 7; k++) g[k] = lds_T<T>(s_S + lds_u8(s_idx + c_tbl4.p[j1][j2][k]) * sstride);
+          for (int k = 0; k < 7; k++) g[k] = SAcc<T>::lds(s_S + lds_u8(s_idx + c_tbl4.p[j1][j2][k]) * sstride, sstride);
           pair_body4<T, KD>(mq_mul(w1, g[0]), g + 1, s_coef, r, sum, asum);
         }
       }
@@ -385,15 +418,23 @@ __device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint3
     T b[NB > 0 ? NB : 1], r[KD > 0 ? KD : 1];
     Gather<T, NB, 0>::run(iw, s_S, sstride, b);
     Gather<T, KD, NB>::run(iw, s_S, sstride, r);
-    T sum = T(0.0); double asum = 0.0;
+    T sum = T(0.0); typename MagOf<T>::type asum(0.0);
     PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum, asum);
     res.v = sum; res.a = asum * rbound<T, KD>(r);
   }
   return res;
 }
 
+#ifndef MQ_INLINE_DISPATCH
+#define MQ_INLINE_DISPATCH 1   // 1: the shape switch is inlined into the entry loop (no call ABI: the caller-saved registers of a call went through local memory, 18 loads + 17 stores per entry with 4 points per lane)
+#endif
+#if MQ_INLINE_DISPATCH
+#define MQ_DISPATCH_ATTR __forceinline__
+#else
+#define MQ_DISPATCH_ATTR __noinline__
+#endif
 template <class T>
-__device__ __noinline__ FamRes<T> family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
+__device__ MQ_DISPATCH_ATTR FamRes<T> family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
   switch (ckd) {     // key = c*8 + kd; the inner dimension kd is capped per c by mq_kd_max (device_layout.h)
 #define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(w0, w1, s_idx, s_coef, s_S, sstride);
 #define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2)
@@ -501,10 +542,79 @@ __device__ __noinline__ T family_spread(const uint64_t *ent, uint64_t hd, int m,
   return sum;
 }
 
+// ------------------------------------------------------------------ a5: the entries of one table, run by run
+// The entries of a table come in runs of equal shape (c, kd): host_prepare.cpp sorts shape-major and stores in every header
+// the number of entries left in its run. The shape switch is taken once per RUN and each shape has its own loop over the
+// run's entries, which carries a handful of values (stream position, count, accumulation key, run accumulator) next to the
+// family body's registers. (Round 1 took the switch per entry through a call: its loop state lived in local memory and every
+// entry paid a chain of local-memory round trips, ~1800 cycles per entry whatever the arithmetic inside.)
+// A run of families with the same (output, pattern, grade) accumulates in registers; the accumulator is (re)loaded from N
+// when the key changes, BEFORE the family is evaluated, so that the local-memory load has the whole evaluation to complete.
+#ifndef MQ_RUNS
+#define MQ_RUNS 1
+#endif
+template <class T> struct RunAcc { int key; T racc; typename MagOf<T>::type racca; };
+
+template <class T, int C, int KD>
+__device__ __forceinline__ void run_loop(StreamReader &rd, int count, int sub, uint32_t s_S, uint32_t sstride,
+                                         T (*N)[MQ_MAXPAT][MQ_NGRADE], typename MagOf<T>::type (*Na)[MQ_MAXPAT][MQ_NGRADE], RunAcc<T> &ra) {
+  using M = typename MagOf<T>::type;
+  constexpr int NI = C * (2 * C - 1) + KD;
+  int pos = rd.pos;
+  uint32_t base = rd.addr() - 8u * (uint32_t)pos;              // shared address of word 0 of the current chunk
+  int key = ra.key; T racc = ra.racc; M racca = ra.racca;
+#pragma unroll 1
+  for (int i = 0; i < count;) {
+    if (pos == MQ_CHUNK_WORDS) { rd.pos = pos; rd.advance(); pos = 0; base = rd.addr(); }
+    const uint32_t a0 = base + 8u * (uint32_t)pos;
+    const uint64_t hd = lds_u64(a0);
+    const uint32_t idxw = (uint32_t)(hd >> 16 & 0xFFFF);
+    if ((int)(hd & 7) == MQ_PAD_MARK) { pos += 1 + (int)idxw; continue; }
+    const uint64_t hl = lds_u64(a0 + 8u * (uint32_t)sub);
+    const uint32_t sidx = a0 + 8u * MQ_WL + 8u * idxw * (uint32_t)sub;
+    const uint64_t w0 = lds_u64(sidx), w1 = lds_u64(sidx + 8);
+    const uint32_t scoef = a0 + 8u * MQ_WL * (1u + idxw) + (KD ? 16u : 8u) * (uint32_t)sub;
+    const int keyk = (int)((hl & 7) | ((hl >> 6 & 15) << 3) | ((hl >> 14 & 1) << 7));
+    if (keyk != key) {
+      if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
+      key = keyk; racc = N[key >> 7][(key >> 3) & 15][key & 7]; racca = Na[key >> 7][(key >> 3) & 15][key & 7];
+    }
+    const FamRes<T> fr = family_eval<T, C, KD>(w0, w1, sidx, scoef, s_S, sstride);
+    T val = mq_norm(fr.v); M amag = fr.a;             // the family code works on unnormalised pairs (dd_arith.cuh)
+    const int ns = (int)(hl >> 10 & 15);
+#pragma unroll 1
+    for (int j = 0; j < ns; j++) {                    // scalar factors; + 1/8: the factor's own absolute round-off (A_t = 1 - x_t may be tiny)
+      const T sc = SAcc<T>::lds(s_S + lds_u8(sidx + NI + j) * sstride, sstride);
+      val = val * sc; amag = amag * (mq_absd(sc) + M(0.125));
+    }
+    racc = racc + val; racca += amag;                 // racca: sum of |monomial| bounds, sees the cancellation inside a family too
+    pos += MQ_WL * (1 + (int)idxw) + (int)(hd >> 32 & 0xFFFF);
+    i++;
+  }
+  rd.pos = pos;
+  ra.key = key; ra.racc = racc; ra.racca = racca;
+}
+template <class T>
+__device__ __forceinline__ void run_dispatch(int ckd, StreamReader &rd, int count, int sub, uint32_t s_S, uint32_t sstride,
+                                             T (*N)[MQ_MAXPAT][MQ_NGRADE], typename MagOf<T>::type (*Na)[MQ_MAXPAT][MQ_NGRADE], RunAcc<T> &ra) {
+  switch (ckd) {     // key = c*8 + kd; the inner dimension kd is capped per c by mq_kd_max (device_layout.h)
+#define MQ_CASE(C, K) case C * 8 + K: run_loop<T, C, K>(rd, count, sub, s_S, sstride, N, Na, ra); return;
+#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2)
+    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_ROW(4)
+    MQ_CASE(0, 3) MQ_CASE(0, 4) MQ_CASE(0, 5) MQ_CASE(0, 6) MQ_CASE(1, 3) MQ_CASE(1, 4) MQ_CASE(1, 5) MQ_CASE(1, 6)
+    MQ_CASE(2, 3) MQ_CASE(2, 4) MQ_CASE(2, 5) MQ_CASE(2, 6) MQ_CASE(3, 3) MQ_CASE(3, 4)
+#undef MQ_ROW
+#undef MQ_CASE
+  }
+  __trap();          // a family shape the tables must never contain
+}
+
 // ------------------------------------------------------------------ a4: scalars of one piece
 // writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
 template <class T>
-__device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z, T *S, int stride, bool wr, T &U, T &V, T &G, double &amin, double &xmin) {
+__device__ __forceinline__ void piece_scalars(const DevGeom &g, const typename MagOf<T>::type *z, unsigned char *S, int stride, bool wr, T &U, T &V, T &G,
+                                              typename MagOf<T>::type &amin, typename MagOf<T>::type &xmin) {
+  using M = typename MagOf<T>::type;
   const int n = g.nch, ns = g.nslot;
   T A[MQ_MAXL][MQ_MAXL], Inv[MQ_MAXL][MQ_MAXL];
 #pragma unroll
@@ -523,15 +633,15 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
   for (int i = 0; i < MQ_MAXL; i++) if (i < n) A[i][i] = A[i][i] + T(z[g.chord_zline[i]]);
   // Gauss-Jordan without pivoting (A is symmetric positive definite); determinant = product of pivots.
   // pivot/original diagonal measures the relative accuracy lost in the Schur complements (O8).
-  double d0[MQ_MAXL];
+  M d0[MQ_MAXL];
 #pragma unroll
-  for (int i = 0; i < MQ_MAXL; i++) d0[i] = mq_to_double(A[i][i]);
+  for (int i = 0; i < MQ_MAXL; i++) d0[i] = mq_mag(A[i][i]);
   U = T(1.0);
 #pragma unroll
   for (int c = 0; c < MQ_MAXL; c++) {
     if (c < n) {
       const T p = A[c][c]; U = U * p;
-      xmin = fmin(xmin, mq_to_double(p) / d0[c]);
+      xmin = mq_mmin(xmin, mq_mag(p) / d0[c]);
       const T ip = T(1.0) / p;
 #pragma unroll
       for (int k = 0; k < MQ_MAXL; k++) { A[c][k] = A[c][k] * ip; Inv[c][k] = Inv[c][k] * ip; }
@@ -565,27 +675,27 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const double *z,
         const T zb = bsu * T(z[g.slot[u].zline]);
         x = x + zb; if (g.slot[u].sgn < 0) q = q - zb; else q = q + zb;
       }
-      if (u > s && wr) S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride] = bsu;   // raw beta, scaled below
+      if (u > s && wr) SAcc<T>::st(S, off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1), stride, bsu);   // raw beta, scaled below
     }
     const bool line = g.slot[s].kind == MQ_SLOT_LINE;
     const T gs = T(2.0) - x;
     const T igs = line ? T(1.0) / gs : T(1.0);
     ig[s] = igs;
-    if (wr) S[s * stride] = x * igs;                                  // r_t = x_t / g_t   (lines)
-    if (off_at >= 0 && wr) S[(off_at + s) * stride] = T(1.0) - x;   // A_t
+    if (wr) SAcc<T>::st(S, s, stride, x * igs);                                  // r_t = x_t / g_t   (lines)
+    if (off_at >= 0 && wr) SAcc<T>::st(S, off_at + s, stride, T(1.0) - x);   // A_t
     const T sg = T((double)g.slot[s].sgn);
-    if (off_aq >= 0 && wr) S[(off_aq + s) * stride] = (sg - q) * igs * T(0.5);   // A'_t / g_t
+    if (off_aq >= 0 && wr) SAcc<T>::st(S, off_aq + s, stride, (sg - q) * igs * T(0.5));   // A'_t / g_t
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
-      const double xd = mq_to_double(x);
-      amin = fmin(amin, fabs(1.0 - xd)); xmin = fmin(xmin, 2.0 - xd);   // |A_t| (scalar factors of insertion pieces) ; g_t divides every operand of slot t
+      const M xd = mq_mag(x);
+      amin = mq_mmin(amin, mq_absd(M(1.0) - xd)); xmin = mq_mmin(xmin, M(2.0) - xd);   // |A_t| (scalar factors of insertion pieces) ; g_t divides every operand of slot t
     }
   }
   if (wr)
   for (int s = 0; s < ns; s++)
     for (int u = s + 1; u < ns; u++) {
-      T *p = &S[(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1)) * stride];
-      *p = *p * ig[s] * ig[u];
+      const int at = off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1);
+      SAcc<T>::st(S, at, stride, SAcc<T>::ld(S, at, stride) * ig[s] * ig[u]);
     }
 }
 
@@ -618,18 +728,26 @@ template <class T> __device__ __forceinline__ void graded_mul(T *acc, const T *b
 // CTA-collective: contains __syncthreads; every thread of the CTA must call it.
 template <class T> __device__ __forceinline__ T mq_shfl_xor(T v, int m);
 template <> __device__ __forceinline__ double mq_shfl_xor<double>(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+template <> __device__ __forceinline__ pt2 mq_shfl_xor<pt2>(pt2 v, int m) { pt2 r; r.v[0] = __shfl_xor_sync(0xffffffffu, v.v[0], m); r.v[1] = __shfl_xor_sync(0xffffffffu, v.v[1], m); return r; }
+template <> __device__ __forceinline__ pt4 mq_shfl_xor<pt4>(pt4 v, int m) {
+  pt4 r;
+#pragma unroll
+  for (int i = 0; i < 4; i++) r.v[i] = __shfl_xor_sync(0xffffffffu, v.v[i], m);
+  return r;
+}
 template <> __device__ __forceinline__ dd mq_shfl_xor<dd>(dd v, int m) { return dd(__shfl_xor_sync(0xffffffffu, v.hi, m), __shfl_xor_sync(0xffffffffu, v.lo, m)); }
 
 template <class T, int W, bool LANES, bool SPREAD = false>
-__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const double *z, T *S, int stride, T *xT, double *xA, int gw, int sub,
-                                            T &f_out, T &abs_out, double &amin_out, double &xmin_out) {
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const typename MagOf<T>::type *z, unsigned char *S, int stride, T *xT, typename MagOf<T>::type *xA, int gw, int sub,
+                                            T &f_out, T &abs_out, typename MagOf<T>::type &amin_out, typename MagOf<T>::type &xmin_out) {
   constexpr bool TRACK = true;
+  using M = typename MagOf<T>::type;                   // magnitudes (round-off bounds, pivot ratios): one per sample point of the lane
   StreamReader rd = rd_io;                             // work on a register copy (the caller's object lives in local memory across this call)
   const DevHeader &h = *v.h;
-  T nodeval[/*worst case*/ 1024];
-  double nodeabs[TRACK ? 1024 : 1];
+  T nodeval[MQ_MAXNODEVAL];
+  M nodeabs[TRACK ? MQ_MAXNODEVAL : 1];
   T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
-  double amin = 1.0, xmin = 1.0;
+  M amin(1.0), xmin(1.0);
   const bool owner = gw == 0 && sub == 0 && (!SPREAD || threadIdx.x == 0);   // the lane whose f_out is used
   const uint32_t s_S = smem_u32(S), sstride = (uint32_t)(stride * sizeof(T));
   rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
@@ -645,10 +763,10 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
       const DevTable &tb = v.tab[ti];
       T N[2][MQ_MAXPAT][MQ_NGRADE];
-      double Na[TRACK ? 2 : 1][TRACK ? MQ_MAXPAT : 1][MQ_NGRADE];
+      M Na[TRACK ? 2 : 1][TRACK ? MQ_MAXPAT : 1][MQ_NGRADE];
       for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = 0.0; }
+          for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = T(0.0); if constexpr (TRACK) Na[o][p][c] = M(0.0); }
       // entries of this table from the staged stream; a run of families with the same (output, pattern, grade)
       // accumulates in registers and is flushed when the key changes
       if constexpr (SPREAD) {
@@ -660,9 +778,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
 #pragma unroll 1
             for (int m = 0; m < MQ_WL; m++) {
               int kk; double am;
-              const T val = family_spread<T>(pend, pend_h, m, S, stride, kk, am);
+              const T val = family_spread<T>(pend, pend_h, m, reinterpret_cast<const T *>(S), stride, kk, am);
               N[kk >> 7][(kk >> 3) & 15][kk & 7] = N[kk >> 7][(kk >> 3) & 15][kk & 7] + val;
-              if constexpr (TRACK) Na[kk >> 7][(kk >> 3) & 15][kk & 7] += am;
+              if constexpr (TRACK) Na[kk >> 7][(kk >> 3) & 15][kk & 7] += M(am);
             }
             pend = nullptr;
           }
@@ -674,7 +792,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           const int idxw = (int)(hd >> 16 & 0xFFFF);
           if ((int)(hd & 7) == MQ_PAD_MARK) { rd.pos += 1 + idxw; continue; }
           if (unit % blockDim.x == threadIdx.x) { pend = rd.gsrc + (size_t)rd.chunk * MQ_CHUNK_WORDS + rd.pos; pend_h = hd; }
-          rd.pos += MQ_WL * (1 + idxw) + (int)(uint32_t)(hd >> 32); left--; unit++;
+          rd.pos += MQ_WL * (1 + idxw) + (int)(hd >> 32 & 0xFFFF); left--; unit++;
           if (unit % blockDim.x == 0) flush_round();
         }
         flush_round();
@@ -684,20 +802,31 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         const int ne = tb.nout * npat * MQ_NGRADE;
         for (int e = 0; e < ne; e++) {
           const int o = e / (npat * MQ_NGRADE), p = (e / MQ_NGRADE) % npat, c = e % MQ_NGRADE;
-          T t = N[o][p][c]; double ta = Na[o][p][c];
-          for (int m = 1; m < 32; m <<= 1) { t = t + mq_shfl_xor<T>(t, m); ta += __shfl_xor_sync(0xffffffffu, ta, m); }
+          T t = N[o][p][c]; M ta = Na[o][p][c];
+          for (int m = 1; m < 32; m <<= 1) { t = t + mq_shfl_xor<T>(t, m); ta += mq_shfl_xor<M>(ta, m); }
           if (lane == 0) { xT[wid * ne + e] = t; xA[wid * ne + e] = ta; }
         }
         __syncthreads();
         for (int e = 0; e < ne; e++) {
           const int o = e / (npat * MQ_NGRADE), p = (e / MQ_NGRADE) % npat, c = e % MQ_NGRADE;
-          T t = xT[e]; double ta = xA[e];
+          T t = xT[e]; M ta = xA[e];
           for (int w = 1; w < nw; w++) { t = t + xT[w * ne + e]; ta += xA[w * ne + e]; }
           N[o][p][c] = t; Na[o][p][c] = ta;
         }
         __syncthreads();
+      } else if constexpr (LANES && W == 1 && MQ_RUNS) {
+        RunAcc<T> ra; ra.key = -1; ra.racc = T(0.0); ra.racca = M(0.0);
+        for (int left = tb.nfam; left > 0;) {
+          if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
+          const uint64_t hd = lds_u64(rd.addr());
+          if ((int)(hd & 7) == MQ_PAD_MARK) { rd.pos += 1 + (int)(hd >> 16 & 0xFFFF); continue; }
+          const int run = (int)(hd >> 48);
+          run_dispatch<T>((int)(hd & 7) * 8 + (int)(hd >> 3 & 7), rd, run, sub, s_S, sstride, N, Na, ra);
+          left -= run;
+        }
+        if (ra.key >= 0) { N[ra.key >> 7][(ra.key >> 3) & 15][ra.key & 7] = ra.racc; Na[ra.key >> 7][(ra.key >> 3) & 15][ra.key & 7] = ra.racca; }
       } else {
-      int key = -1; T racc = T(0.0); double racca = 0.0;
+      int key = -1; T racc = T(0.0); M racca(0.0);
       bool have = false; uint32_t a0 = 0; uint64_t hd = 0, hl = 0, w0 = 0, w1 = 0;   // entry header, this lane's member header + first index words
       int unit = 0;                                                                  // evaluation units are dealt round-robin to the W warps
       // this lane's member of the entry at address a with (uniform) header hu: its header word and first two index words
@@ -715,37 +844,43 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         const int idxw = (int)(hd >> 16 & 0xFFFF);
         const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7);
         if (c == MQ_PAD_MARK) { rd.pos += 1 + idxw; have = false; continue; }
-        const int size = MQ_WL * (1 + idxw) + (int)(uint32_t)(hd >> 32), npos = rd.pos + size;
+        const int size = MQ_WL * (1 + idxw) + (int)(hd >> 32 & 0xFFFF), npos = rd.pos + size;
         // software pipeline: fetch the next entry's header and index words before this entry's arithmetic
         uint32_t an = a0 + 8 * size; uint64_t hdn = 0, hln = 0, n0 = 0, n1 = 0;
         const bool havenext = npos < MQ_CHUNK_WORDS;
         if (havenext) { hdn = lds_u64(an); if constexpr (LANES) fetch_member(an, hdn, sub, hln, n0, n1); }
         // pair this entry with the next one if it has the same shape (binary64: doubles the ILP of the warp)
         bool dual = false;
-        if constexpr (sizeof(T) == sizeof(double) && LANES && MQ_DUAL) {
+        if constexpr (std::is_same<T, double>::value && LANES && MQ_DUAL) {
           if (havenext && left > 1 && c <= 3 && (int)(hdn & 63) == (int)(hd & 63)) {
-            const int size2 = MQ_WL * (1 + (int)(hdn >> 16 & 0xFFFF)) + (int)(uint32_t)(hdn >> 32);
+            const int size2 = MQ_WL * (1 + (int)(hdn >> 16 & 0xFFFF)) + (int)(hdn >> 32 & 0xFFFF);
             dual = npos + size2 <= MQ_CHUNK_WORDS;
           }
         }
         const int nb = c * (2 * c - 1) + kd;
         const uint32_t ustride = kd ? 16u : 8u;                        // bytes between the members' coefficient units
         // member header ml: scalar factors and accumulation key; sidx: shared address of the member's index bytes
-        auto account = [&](T val, double amag, uint64_t ml, uint32_t sidx) {
-          const int ns = (int)(ml >> 10 & 15), keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
+        // accumulation key (output, pattern, grade) of a member. The run accumulator is (re)loaded from N when the key changes,
+        // BEFORE the family is evaluated: the local-memory load then has the whole evaluation to complete.
+        auto open_key = [&](uint64_t ml) {
+          const int keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
+          if (keyk != key) {
+            if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
+            key = keyk; racc = N[key >> 7][(key >> 3) & 15][key & 7]; if constexpr (TRACK) racca = Na[key >> 7][(key >> 3) & 15][key & 7];
+          }
+        };
+        // member header ml: scalar factors; sidx: shared address of the member's index bytes
+        auto account = [&](T val, M amag, uint64_t ml, uint32_t sidx) {
+          const int ns = (int)(ml >> 10 & 15);
           val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
 #pragma unroll 1
-          for (int i = 0; i < ns; i++) { const T sc = lds_T<T>(s_S + lds_u8(sidx + nb + i) * sstride); val = val * sc; amag *= mq_absd(sc) + 0.125; }   // + 1/8: the factor's own absolute round-off (A_t = 1 - x_t may be tiny)
-          if (keyk != key) {
-            if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
-            key = keyk; racc = T(0.0); racca = 0.0;
-          }
+          for (int i = 0; i < ns; i++) { const T sc = SAcc<T>::lds(s_S + lds_u8(sidx + nb + i) * sstride, sstride); val = val * sc; amag = amag * (mq_absd(sc) + M(0.125)); }   // + 1/8: the factor's own absolute round-off (A_t = 1 - x_t may be tiny)
           racc = racc + val;
           if constexpr (TRACK) racca += amag;      // sum of |monomial| bounds: sees the cancellation inside a family too
         };
         if (dual) {
-          if constexpr (sizeof(T) == sizeof(double) && LANES) {
-            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = MQ_WL * (1 + idxw2) + (int)(uint32_t)(hdn >> 32), npos2 = npos + size2;
+          if constexpr (std::is_same<T, double>::value && LANES) {
+            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = MQ_WL * (1 + idxw2) + (int)(hdn >> 32 & 0xFFFF), npos2 = npos + size2;
             const uint32_t a2 = an + 8 * size2;
             uint64_t hd3 = 0, hl3 = 0, m0 = 0, m1 = 0;
             const bool have3 = npos2 < MQ_CHUNK_WORDS;
@@ -754,8 +889,8 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
               const uint32_t sidxA = a0 + 8 * MQ_WL + 8 * idxw * sub, sidxB = an + 8 * MQ_WL + 8 * idxw2 * sub;
               const double4 vAB = family_dispatch2(c * 8 + kd, w0, w1, n0, n1, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub,
                                                    sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub, s_S, sstride);
-              account(T(vAB.x), vAB.z, hl, sidxA);
-              account(T(vAB.y), vAB.w, hln, sidxB);
+              open_key(hl); account(T(vAB.x), vAB.z, hl, sidxA);
+              open_key(hln); account(T(vAB.y), vAB.w, hln, sidxB);
             }
             unit++;
             rd.pos = npos2; left -= 2;
@@ -769,8 +904,13 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             const int m = LANES ? sub : q;
             if constexpr (!LANES) fetch_member(a0, hd, m, hl, w0, w1);
             const uint32_t sidx = a0 + 8 * MQ_WL + 8 * idxw * m, scoef = a0 + 8 * MQ_WL * (1 + idxw) + ustride * m;
-            static_assert(sizeof(T) <= sizeof(dd), "wider types use the entry-parallel path");
+            static_assert(sizeof(T) <= 32, "wider types use the entry-parallel path");
+            open_key(hl);
+#if defined(MQ_EXP_NOFAM)
+            FamRes<T> fr; fr.v = T(1.0); fr.a = M(1.0);          // experiment: everything but the family evaluation
+#else
             const FamRes<T> fr = family_dispatch<T>(c * 8 + kd, w0, w1, sidx, scoef, s_S, sstride);
+#endif
             account(fr.v, fr.a, hl, sidx);
           }
         }
@@ -778,7 +918,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         rd.pos = npos; left--;
         have = havenext; a0 = an; hd = hdn; hl = hln; w0 = n0; w1 = n1;
       }
-      if (key >= 0) { T &n = N[key >> 7][(key >> 3) & 15][key & 7]; n = n + racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] += racca; }
+      if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
       }
       if constexpr (LANES && MQ_WL > 1) {              // add the partial sums of the lane roles: afterwards every lane holds the totals
         for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
@@ -787,7 +927,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
 #pragma unroll
             for (int m = 32 / MQ_WL; m < 32; m <<= 1) {
               N[o][p][c] = N[o][p][c] + mq_shfl_xor<T>(N[o][p][c], m);
-              if constexpr (TRACK) Na[o][p][c] += __shfl_xor_sync(0xffffffffu, Na[o][p][c], m);
+              if constexpr (TRACK) Na[o][p][c] += mq_shfl_xor<M>(Na[o][p][c], m);
             }
           }
       }
@@ -795,7 +935,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         const T i12 = T(1.0) / T(12.0);
         for (int p = 0; p < npat; p++)
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] *= (1.0 / 12.0); }
+          for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] = Na[0][p][c] * M(1.0 / 12.0); }
       }
       if constexpr (W > 1) {                           // add the partial sums of the other warps of the group into warp 0
         for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++) {
@@ -821,19 +961,19 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
         for (int k = 0; k < nd.nchild; k++) { Up = Up * nodeU[nd.child[k]]; Vs = Vs + nodeV[nd.child[k]]; }
         nodeU[ni] = Up; nodeV[ni] = Vs;
         for (int o = 0; o < nd.nout; o++) {
-          T tot[MQ_NGRADE]; double tota[MQ_NGRADE];
+          T tot[MQ_NGRADE]; M tota[MQ_NGRADE];
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = T(0.0); tota[c] = 0.0; }
+          for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = T(0.0); tota[c] = M(0.0); }
           for (int p = 0; p < npat; p++) {
-            T acc[MQ_NGRADE]; double acca[MQ_NGRADE];
+            T acc[MQ_NGRADE]; M acca[MQ_NGRADE];
 #pragma unroll
-            for (int c = 0; c < MQ_NGRADE; c++) { acc[c] = N[o][p][c] * G; if constexpr (TRACK) acca[c] = Na[o][p][c] * mq_to_double(G); }
+            for (int c = 0; c < MQ_NGRADE; c++) { acc[c] = N[o][p][c] * G; if constexpr (TRACK) acca[c] = Na[o][p][c] * mq_mag(G); }
             for (int k = 0; k < nd.nchild; k++) {
               const DevNode &ch = v.node[nd.child[k]];
               const int pb = g.child_patbit[k];
               const int which = (pb >= 0 && (p >> pb & 1)) ? 1 : 0;      // S-child: a (0) or b (1); V-child: its single value
               graded_mul<T>(acc, &nodeval[ch.val_off + which * ch.ngr], ch.ngr);
-              if constexpr (TRACK) graded_mul<double>(acca, &nodeabs[ch.val_off + which * ch.ngr], ch.ngr);
+              if constexpr (TRACK) graded_mul<M>(acca, &nodeabs[ch.val_off + which * ch.ngr], ch.ngr);
             }
 #pragma unroll
             for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = tot[c] + acc[c]; if constexpr (TRACK) tota[c] += acca[c]; }
@@ -859,7 +999,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
       const T scale = T(fact * (double)tm.sign) / (U2 * Vp);
       const T contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : T(0.0)) * scale;
       f = f + contrib;
-      if constexpr (TRACK) asum = asum + T(c < nd.ngr ? nodeabs[nd.val_off + c] * fabs(mq_to_double(scale)) : 0.0);
+      if constexpr (TRACK) asum = asum + T(c < nd.ngr ? nodeabs[nd.val_off + c] * mq_absd(mq_mag(scale)) : M(0.0));
       else asum = asum + mq_abs(contrib);
     }
   }

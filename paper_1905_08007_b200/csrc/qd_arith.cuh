@@ -88,5 +88,7 @@ __device__ __forceinline__ qd mq_fma_c(double coef, qd x, double c0, qd) { retur
 __device__ __forceinline__ qd mq_mul(qd a, qd b) { return a * b; }
 __device__ __forceinline__ qd mq_norm(qd a) { return a; }
 __device__ __forceinline__ double mq_to_double(qd a) { return __dadd_rn(__dadd_rn(a.x[0], a.x[1]), __dadd_rn(a.x[2], a.x[3])); }
+__device__ __forceinline__ double mq_mag(qd a) { return mq_to_double(a); }
+__device__ __forceinline__ double mq_absd(qd a) { return fabs(a.x[0]); }
 __device__ __forceinline__ qd mq_abs(qd a) { return a.x[0] < 0 ? -a : a; }
 __device__ __forceinline__ bool mq_lt0(qd a) { return a.x[0] < 0; }

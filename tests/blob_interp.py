@@ -9,7 +9,7 @@ import numpy as np
 
 MAXL, MAXSLOT, MAXCHILD, NGRADE = 5, 14, 5, 6
 HDR = np.dtype([("L", "<i4"), ("M", "<i4"), ("diag_id", "<i4"), ("ngeom", "<i4"), ("ntable", "<i4"), ("nnode", "<i4"), ("nterm", "<i4"),
-                ("nodeval_len", "<i4"), ("max_scal_len", "<i4"), ("pad0", "<i4"), ("C", "<f8"), ("cond_max", "<f8"),
+                ("nodeval_len", "<i4"), ("max_scal_len", "<i4"), ("wl", "<i4"), ("C", "<f8"), ("cond_max", "<f8"),
                 ("off_Z", "<i8"), ("off_invdeg", "<i8"), ("off_geom", "<i8"), ("off_table", "<i8"), ("off_node", "<i8"), ("off_term", "<i8"), ("total_words", "<i8"),
                 ("off_stream", "<i8"), ("stream_chunks", "<i8")])
 SLOT = np.dtype([("kind", "i1"), ("zline", "i1"), ("sgn", "i1"), ("child", "i1"), ("eps", "<u4")])
@@ -70,7 +70,7 @@ class Blob:
 
     def families(self, ti):
         """yields the families of table ti; a stream entry holds WL same-shape families side by side (device_layout.h)"""
-        WL = 2
+        WL = int(self.h["wl"])
         t = self.table[ti]
         pos = int(t["stream_off"])
         raw = self.w.view(np.uint8)
@@ -78,7 +78,7 @@ class Blob:
         while nleft:
             hd = int(self.w[pos])
             c, kd = hd & 7, hd >> 3 & 7
-            idxw, ncoef = hd >> 16 & 0xFFFF, hd >> 32
+            idxw, ncoef = hd >> 16 & 0xFFFF, hd >> 32 & 0xFFFF
             if c == 7:                      # PAD entry up to the chunk boundary
                 pos += 1 + idxw
                 continue
