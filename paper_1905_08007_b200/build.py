@@ -19,7 +19,7 @@ DEFS = os.environ.get("MCQED_DEFS", "").split()    # tuning builds: -D macros se
 NVCC_FLAGS = ARCH + ["-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "-Xptxas", "-v"] + DEFS + os.environ.get("MCQED_NVCC_EXTRA", "").split()   # e.g. MCQED_NVCC_EXTRA=-DMQ_DUAL=0 for a tuning build
 GXX_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-ffp-contract=off", "-pthread", "-I/usr/local/cuda/include"] + DEFS
 COMMON = ["device_layout.h", "host_model.hpp", "diagram.hpp", os.path.join("..", "..", "include", "mcqed.h")]
-KERN = COMMON + ["mcqed_kernels.cuh", "dd_arith.cuh", "kern_common.cuh"]
+KERN = COMMON + ["mcqed_kernels.cuh", "dd_arith.cuh", "pt2_arith.cuh", "kern_common.cuh"]
 UNITS = {  # object -> (compiler, source, dependencies)
     "host_prepare.o": ("g++", "host_prepare.cpp", COMMON + ["coef_gen.hpp"]),
     "mcqed_api.o": ("g++", "mcqed_api.cpp", COMMON),

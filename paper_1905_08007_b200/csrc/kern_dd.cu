@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
     double z[MQ_MAXM]; double p = 1.0;
     if (ro.gw == 0) p = draw_point<false>(v, flag_list[i < cnt ? i : cnt - 1], seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, nullptr, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (!live) continue;
     const double fd = mq_to_double(f);
     const bool lost = tier_decision(false, fd, mq_to_double(a), amin, xmin, p, pr.dd_cond_max, 1.0 / pr.dd_cond_max, MQ_UNIT_DD, pr.w_abs_tol) == 1;
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     double z[MQ_MAXM];
     const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, nullptr, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     if (live) {
       const double fd = mq_to_double(f);
@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
     const unsigned long long rel = flag_list[i < cnt ? i : cnt - 1];
     if (ro.gw == 0) p = draw_point<false>(v, first + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, nullptr, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) {
       const double fd = mq_to_double(f);
       f_out[rel] = fd;
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict
     double z[MQ_MAXM];
     for (int k = 0; k < MQ_MAXM; k++) z[k] = k < M ? z_in[i * M + k] : 0.0;
     dd f, a; double amin, xmin;
-    eval_integrand<dd, W_DD, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<dd, W_DD, true>(v, rd, z, nullptr, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (live) fdd_out[i] = mq_to_double(f);
   }
 }

@@ -14,6 +14,29 @@ namespace mqk {
 using FT = std::conditional<NP_F64 == 4, pt4, std::conditional<NP_F64 == 2, pt2, double>::type>::type;
 using FM = MagOf<FT>::type;
 constexpr int NP = PtsOf<FT>::n;
+// DISTK: the MQ_WL lanes of a point group carry NP = MQ_WL points; lane role k draws point k and computes its scalars in plain
+// binary64 (no redundant work across the lane roles); role 0 (the owner) gathers densities and flags with shuffles
+constexpr bool DISTK = NP > 1 && NP == MQ_WL;
+constexpr int PPW = 32 / MQ_WL;                        // point groups per warp; role k of a group sits PPW * k lanes after role 0
+
+// this lane's part of the draw and the owner's view of it: p[k], bad[k] of the NP points of the group
+struct GroupDraw { double p[NP]; bool bad[NP]; };
+template <bool WANT_ORDER>
+__device__ __forceinline__ void draw_group(const DiagView &v, uint64_t first, uint64_t i0, uint64_t n, uint64_t seed, int sub, FM *z, double *zl, int32_t *ord, GroupDraw &gd) {
+  const int M = v.h->M;
+  if constexpr (DISTK) {
+    const uint64_t im = i0 + (uint64_t)sub;
+    const double pl = draw_point<WANT_ORDER>(v, first + (im < n ? im : n - 1), seed, zl, ord);
+    const bool badl = bad_point(zl, M, pl);
+    const int l0 = (threadIdx.x & 31) % PPW;
+#pragma unroll
+    for (int k = 0; k < NP; k++) { gd.p[k] = __shfl_sync(0xffffffffu, pl, l0 + k * PPW); gd.bad[k] = __shfl_sync(0xffffffffu, (int)badl, l0 + k * PPW) != 0; }
+  } else {
+    draw_points<FT, WANT_ORDER>(v, first, i0, n, seed, z, gd.p, ord);
+#pragma unroll
+    for (int k = 0; k < NP; k++) gd.bad[k] = bad_point(z, k, M, gd.p[k]);
+  }
+}
 
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
 __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_integrate_f64(const uint64_t *__restrict__ blob, uint64_t first, uint64_t n, uint64_t seed,
@@ -30,18 +53,18 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_integrate_f64(const ui
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[MQ_MAXM]; double p[NP];
-    if (ro.gw == 0) draw_points<FT, false>(v, first, i0, n, seed, z, p, nullptr);
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; GroupDraw gd;
+    draw_group<false>(v, first, i0, n, seed, ro.sub, z, zl, nullptr, gd);
     FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (ro.gw != 0 || ro.sub != 0) continue;
 #pragma unroll
     for (int k = 0; k < NP; k++) {
       if (i0 + k >= n) continue;
       const double fk = mq_comp(f, k);
-      const bool flag = tier_decision(bad_point(z, k, v.h->M, p[k]), fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+      const bool flag = tier_decision(gd.bad[k], fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), gd.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
       if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i0 + k; }
-      else { const double w = fk / p[k]; s1.add(w); s2.add(w * w); }
+      else { const double w = fk / gd.p[k]; s1.add(w); s2.add(w * w); }
     }
   }
   block_reduce_store(s1, s2, partial);
@@ -78,19 +101,29 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[MQ_MAXM]; int32_t ord[NP * MQ_MAXM]; double p[NP];
-    if (ro.gw == 0) draw_points<FT, true>(v, first, i0, n, seed, z, p, ord);
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; int32_t ord[(DISTK ? 1 : NP) * MQ_MAXM]; GroupDraw gd;
+    draw_group<true>(v, first, i0, n, seed, ro.sub, z, zl, ord, gd);
     FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    if constexpr (DISTK) {                           // every lane role writes the coordinates of the point it drew
+      const uint64_t i = i0 + (uint64_t)ro.sub;
+      if (i < n) {
+        if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = zl[j];
+        if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[j];
+      }
+    }
     if (ro.gw != 0 || ro.sub != 0) continue;
     for (int k = 0; k < NP; k++) {
       const uint64_t i = i0 + k;
       if (i >= n) continue;
       const double fk = mq_comp(f, k);
-      const int dec = tier_decision(bad_point(z, k, M, p[k]), fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
+      const double *p = gd.p;
+      const int dec = tier_decision(gd.bad[k], fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
       const bool flag = dec == 1;
-      if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = mq_comp(z[j], k);
-      if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[k * MQ_MAXM + j];
+      if constexpr (!DISTK) {
+        if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = mq_comp(z[j], k);
+        if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[k * MQ_MAXM + j];
+      }
       if (p_out) p_out[i] = p[k];
       if (f_out) f_out[i] = fk;
       if (f64_out) f64_out[i] = fk;
@@ -111,13 +144,18 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[MQ_MAXM];
-    for (int k = 0; k < NP; k++) {
-      const uint64_t i = i0 + k < n ? i0 + k : n - 1;                         // surplus slots redo the last point
-      for (int j = 0; j < MQ_MAXM; j++) mq_setc(z[j], k, j < M ? z_in[i * M + j] : 0.0);
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1];
+    if constexpr (DISTK) {
+      const uint64_t i = i0 + ro.sub < n ? i0 + ro.sub : n - 1;               // surplus slots redo the last point
+      for (int j = 0; j < MQ_MAXM; j++) zl[j] = j < M ? z_in[i * M + j] : 0.0;
+    } else {
+      for (int k = 0; k < NP; k++) {
+        const uint64_t i = i0 + k < n ? i0 + k : n - 1;
+        for (int j = 0; j < MQ_MAXM; j++) mq_setc(z[j], k, j < M ? z_in[i * M + j] : 0.0);
+      }
     }
     FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     if (ro.gw != 0 || ro.sub != 0) continue;
     for (int k = 0; k < NP; k++) {
       const uint64_t i = i0 + k;
@@ -150,16 +188,17 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     MqPrec pr = bv.dg[d].pr;
     if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
     const uint64_t i0 = (uint64_t)b * PTS_F64 + (uint64_t)ro.slot * NP;
-    FM z[MQ_MAXM]; double p[NP];
-    draw_points<FT, false>(v, first, i0, n, seed, z, p, nullptr);
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; GroupDraw gd;
+    draw_group<false>(v, first, i0, n, seed, ro.sub, z, zl, nullptr, gd);
+    const double *p = gd.p;
     FT f, a; FM amin, xmin;
-    eval_integrand<FT, 1, true>(v, rd, z, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
+    eval_integrand<FT, 1, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
     // flagged points of the item, compacted in (lane, point) order = ascending sample index
     bool flag[NP]; unsigned bal[NP]; unsigned mine = 0, wsum = 0;
 #pragma unroll
     for (int k = 0; k < NP; k++) {
       const bool live = i0 + k < n && ro.sub == 0;
-      flag[k] = live && tier_decision(bad_point(z, k, v.h->M, p[k]), mq_comp(f, k), mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+      flag[k] = live && tier_decision(gd.bad[k], mq_comp(f, k), mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
       bal[k] = __ballot_sync(0xffffffffu, flag[k]);
       mine += __popc(bal[k] & ((1u << lane) - 1u)); wsum += __popc(bal[k]);
     }

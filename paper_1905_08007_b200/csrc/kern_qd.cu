@@ -40,7 +40,7 @@ __device__ __forceinline__ void qd_setup_reader(StreamReader &rd, unsigned char 
 // the integrand of one point in quad-double, computed by the whole CTA; the value is valid in thread 0
 __device__ __forceinline__ double qd_point(const DiagView &v, StreamReader &rd, const QdRoles &ro, const double *z) {
   qd f, a; double amin, xmin;
-  eval_integrand<qd, 1, false, true>(v, rd, z, reinterpret_cast<unsigned char *>(ro.S), 1, ro.xT, ro.xA, 0, 0, f, a, amin, xmin);
+  eval_integrand<qd, 1, false, true>(v, rd, z, nullptr, reinterpret_cast<unsigned char *>(ro.S), 1, ro.xT, ro.xA, 0, 0, f, a, amin, xmin);
   return mq_to_double(f);
 }
 

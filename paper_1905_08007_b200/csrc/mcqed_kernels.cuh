@@ -369,15 +369,9 @@ template <class T, int N, int OFF, int I = 0> struct Gather {
   }
 };
 
-// value of a family and its round-off magnitude a = sum_pairings |w| sum|c| prod_inner max(1,|r|) >= sum of |monomial|
+// value of a family and its round-off magnitude a = sum_pairings |w| sum|c|; times Rp = prod over the lines of the piece of
+// max(1,|r_t|) (applied once per table) it bounds the sum of |monomial|
 template <class T> struct FamRes { T v; typename MagOf<T>::type a; };
-template <class T, int KD> __device__ __forceinline__ typename MagOf<T>::type rbound(const T *r) {
-  typename MagOf<T>::type R(1.0);
-#pragma unroll
-  for (int i = 0; i < KD; i++) R = R * mq_mmax1(mq_absd(r[i]));
-  return R;
-}
-
 // s_idx: shared address of the index bytes; s_coef: of the coefficients; s_S: of this thread's S[0]; sstride: bytes per S index
 template <class T, int C, int KD>
 __device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
@@ -409,7 +403,7 @@ __device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint3
         }
       }
     }
-    res.v = sum; res.a = asum * rbound<T, KD>(r);
+    res.v = sum; res.a = asum;                       // the factor prod max(1,|r_inner|) is applied per piece (piece_scalars: Rp)
   } else {
     uint64_t iw[NW > 2 ? NW : 2];
     iw[0] = w0; iw[1] = w1;                          // the first 16 index bytes were prefetched with the header
@@ -420,66 +414,9 @@ __device__ __forceinline__ FamRes<T> family_eval(uint64_t w0, uint64_t w1, uint3
     Gather<T, KD, NB>::run(iw, s_S, sstride, r);
     T sum = T(0.0); typename MagOf<T>::type asum(0.0);
     PairRec<T, KD, N2, 0u, true>::run(b, T(1.0), s_coef, r, sum, asum);
-    res.v = sum; res.a = asum * rbound<T, KD>(r);
+    res.v = sum; res.a = asum;                       // the factor prod max(1,|r_inner|) is applied per piece (piece_scalars: Rp)
   }
   return res;
-}
-
-#ifndef MQ_INLINE_DISPATCH
-#define MQ_INLINE_DISPATCH 1   // 1: the shape switch is inlined into the entry loop (no call ABI: the caller-saved registers of a call went through local memory, 18 loads + 17 stores per entry with 4 points per lane)
-#endif
-#if MQ_INLINE_DISPATCH
-#define MQ_DISPATCH_ATTR __forceinline__
-#else
-#define MQ_DISPATCH_ATTR __noinline__
-#endif
-template <class T>
-__device__ MQ_DISPATCH_ATTR FamRes<T> family_dispatch(int ckd, uint64_t w0, uint64_t w1, uint32_t s_idx, uint32_t s_coef, uint32_t s_S, uint32_t sstride) {
-  switch (ckd) {     // key = c*8 + kd; the inner dimension kd is capped per c by mq_kd_max (device_layout.h)
-#define MQ_CASE(C, K) case C * 8 + K: return family_eval<T, C, K>(w0, w1, s_idx, s_coef, s_S, sstride);
-#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2)
-    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_ROW(4)
-    MQ_CASE(0, 3) MQ_CASE(0, 4) MQ_CASE(0, 5) MQ_CASE(0, 6) MQ_CASE(1, 3) MQ_CASE(1, 4) MQ_CASE(1, 5) MQ_CASE(1, 6)
-    MQ_CASE(2, 3) MQ_CASE(2, 4) MQ_CASE(2, 5) MQ_CASE(2, 6) MQ_CASE(3, 3) MQ_CASE(3, 4)
-#undef MQ_ROW
-#undef MQ_CASE
-  }
-  __trap();          // a family shape the tables must never contain
-  return FamRes<T>{T(0.0), 0.0};
-}
-
-// Two consecutive entries of the same shape evaluated together: their arithmetic chains are independent, which
-// doubles the instruction-level parallelism of a warp at unchanged shared-memory footprint (binary64 only).
-// Returns (value A, value B, magnitude A, magnitude B); arguments and results in registers.
-template <int C, int KD>
-__device__ __forceinline__ double4 family_eval2(uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
-                                                uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
-  constexpr int N2 = 2 * C, NB = C * (2 * C - 1), NI = NB + KD, NW = (NI + 7) / 8;
-  uint64_t iwA[NW > 2 ? NW : 2], iwB[NW > 2 ? NW : 2];
-  iwA[0] = wA0; iwA[1] = wA1; iwB[0] = wB0; iwB[1] = wB1;
-#pragma unroll
-  for (int k = 2; k < NW; k++) { iwA[k] = lds_u64(s_idxA + 8 * k); iwB[k] = lds_u64(s_idxB + 8 * k); }
-  double bA[NB > 0 ? NB : 1], rA[KD > 0 ? KD : 1], bB[NB > 0 ? NB : 1], rB[KD > 0 ? KD : 1];
-  Gather<double, NB, 0>::run(iwA, s_S, sstride, bA);
-  Gather<double, NB, 0>::run(iwB, s_S, sstride, bB);
-  Gather<double, KD, NB>::run(iwA, s_S, sstride, rA);
-  Gather<double, KD, NB>::run(iwB, s_S, sstride, rB);
-  double sumA = 0.0, sumB = 0.0, aA = 0.0, aB = 0.0;
-  PairRec<double, KD, N2, 0u, true>::run(bA, 1.0, s_coefA, rA, sumA, aA);
-  PairRec<double, KD, N2, 0u, true>::run(bB, 1.0, s_coefB, rB, sumB, aB);
-  return make_double4(sumA, sumB, aA * rbound<double, KD>(rA), aB * rbound<double, KD>(rB));
-}
-static __device__ __noinline__ double4 family_dispatch2(int ckd, uint64_t wA0, uint64_t wA1, uint64_t wB0, uint64_t wB1, uint32_t s_idxA, uint32_t s_coefA,
-                                                        uint32_t s_idxB, uint32_t s_coefB, uint32_t s_S, uint32_t sstride) {
-  switch (ckd) {
-#define MQ_CASE(C, K) case C * 8 + K: return family_eval2<C, K>(wA0, wA1, wB0, wB1, s_idxA, s_coefA, s_idxB, s_coefB, s_S, sstride);
-#define MQ_ROW(C) MQ_CASE(C, 0) MQ_CASE(C, 1) MQ_CASE(C, 2) MQ_CASE(C, 3) MQ_CASE(C, 4)
-    MQ_ROW(0) MQ_ROW(1) MQ_ROW(2) MQ_ROW(3) MQ_CASE(0, 5) MQ_CASE(1, 5) MQ_CASE(2, 5) MQ_CASE(0, 6) MQ_CASE(1, 6) MQ_CASE(2, 6)
-#undef MQ_ROW
-#undef MQ_CASE
-  }
-  __trap();
-  return make_double4(0.0, 0.0, 0.0, 0.0);
 }
 
 // Entry-parallel family evaluation (quad-double tier): member m of the stream entry at ent (GLOBAL memory), scalars from
@@ -610,10 +547,23 @@ __device__ __forceinline__ void run_dispatch(int ckd, StreamReader &rd, int coun
 }
 
 // ------------------------------------------------------------------ a4: scalars of one piece
-// writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t
-template <class T>
-__device__ __forceinline__ void piece_scalars(const DevGeom &g, const typename MagOf<T>::type *z, unsigned char *S, int stride, bool wr, T &U, T &V, T &G,
-                                              typename MagOf<T>::type &amin, typename MagOf<T>::type &xmin) {
+// accessors to the piece's scalar array S[index] of one point group: the whole element of type T, or (SComp) one binary64
+// component of ptn<N> elements: the lane computes the scalars of ONE of the group's points in plain binary64
+template <class T> struct SWhole {
+  unsigned char *S; int stride;
+  __device__ __forceinline__ void st(int i, T v) const { SAcc<T>::st(S, i, stride, v); }
+  __device__ __forceinline__ T ld(int i) const { return SAcc<T>::ld(S, i, stride); }
+};
+template <int N> struct SComp {
+  double *base; size_t istride;            // element i, point k of the group: plane k/2 of index i, half k&1 of the 16-byte unit
+  __device__ __forceinline__ SComp(unsigned char *S, int stride, int k) : base(reinterpret_cast<double *>(S) + (size_t)(k >> 1) * stride * 2 + (k & 1)), istride((size_t)N * stride) {}
+  __device__ __forceinline__ void st(int i, double v) const { base[(size_t)i * istride] = v; }
+  __device__ __forceinline__ double ld(int i) const { return base[(size_t)i * istride]; }
+};
+// writes S = [ r_t | A_t | A'_t/g_t | beta_tu/(g_t g_u) (t<u) ] and returns U, V, G = prod_lines g_t, Rp = prod_lines max(1,|r_t|)
+template <class T, class ACC>
+__device__ __forceinline__ void piece_scalars(const DevGeom &g, const typename MagOf<T>::type *z, const ACC acc, bool wr, T &U, T &V, T &G,
+                                              typename MagOf<T>::type &Rp, typename MagOf<T>::type &amin, typename MagOf<T>::type &xmin) {
   using M = typename MagOf<T>::type;
   const int n = g.nch, ns = g.nslot;
   T A[MQ_MAXL][MQ_MAXL], Inv[MQ_MAXL][MQ_MAXL];
@@ -655,7 +605,7 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const typename M
   }
   // beta_su = eps_s^T Inv eps_u ; x_s = sum_lines z_u beta_su ; A'_s = (sgn_s - sum_lines z_u beta_su sgn_u)/2
   T ig[MQ_MAXSLOT];
-  V = T(0.0); G = T(1.0);
+  V = T(0.0); G = T(1.0); Rp = M(1.0);
   const int off_at = g.off_at, off_aq = g.off_aq, off_bt = g.off_bt;
   for (int s = 0; s < ns; s++) {
     const uint32_t es = g.slot[s].eps;
@@ -675,27 +625,29 @@ __device__ __forceinline__ void piece_scalars(const DevGeom &g, const typename M
         const T zb = bsu * T(z[g.slot[u].zline]);
         x = x + zb; if (g.slot[u].sgn < 0) q = q - zb; else q = q + zb;
       }
-      if (u > s && wr) SAcc<T>::st(S, off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1), stride, bsu);   // raw beta, scaled below
+      if (u > s && wr) acc.st(off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1), bsu);   // raw beta, scaled below
     }
     const bool line = g.slot[s].kind == MQ_SLOT_LINE;
     const T gs = T(2.0) - x;
     const T igs = line ? T(1.0) / gs : T(1.0);
     ig[s] = igs;
-    if (wr) SAcc<T>::st(S, s, stride, x * igs);                                  // r_t = x_t / g_t   (lines)
-    if (off_at >= 0 && wr) SAcc<T>::st(S, off_at + s, stride, T(1.0) - x);   // A_t
+    const T rs = x * igs;
+    if (wr) acc.st(s, rs);                                              // r_t = x_t / g_t   (lines)
+    if (off_at >= 0 && wr) acc.st(off_at + s, T(1.0) - x);              // A_t
     const T sg = T((double)g.slot[s].sgn);
-    if (off_aq >= 0 && wr) SAcc<T>::st(S, off_aq + s, stride, (sg - q) * igs * T(0.5));   // A'_t / g_t
+    if (off_aq >= 0 && wr) acc.st(off_aq + s, (sg - q) * igs * T(0.5));   // A'_t / g_t
     if (line) {
       V = V + x * T(z[g.slot[s].zline]); G = G * gs;
       const M xd = mq_mag(x);
       amin = mq_mmin(amin, mq_absd(M(1.0) - xd)); xmin = mq_mmin(xmin, M(2.0) - xd);   // |A_t| (scalar factors of insertion pieces) ; g_t divides every operand of slot t
+      Rp = Rp * mq_mmax1(mq_absd(rs));                                  // bounds prod |r_t|^sigma over any subset of the lines
     }
   }
   if (wr)
   for (int s = 0; s < ns; s++)
     for (int u = s + 1; u < ns; u++) {
       const int at = off_bt + s * ns - s * (s + 1) / 2 + (u - s - 1);
-      SAcc<T>::st(S, at, stride, SAcc<T>::ld(S, at, stride) * ig[s] * ig[u]);
+      acc.st(at, acc.ld(at) * ig[s] * ig[u]);
     }
 }
 
@@ -738,26 +690,43 @@ template <> __device__ __forceinline__ pt4 mq_shfl_xor<pt4>(pt4 v, int m) {
 template <> __device__ __forceinline__ dd mq_shfl_xor<dd>(dd v, int m) { return dd(__shfl_xor_sync(0xffffffffu, v.hi, m), __shfl_xor_sync(0xffffffffu, v.lo, m)); }
 
 template <class T, int W, bool LANES, bool SPREAD = false>
-__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const typename MagOf<T>::type *z, unsigned char *S, int stride, T *xT, typename MagOf<T>::type *xA, int gw, int sub,
+__device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_io, const typename MagOf<T>::type *z, const double *zl, unsigned char *S, int stride, T *xT, typename MagOf<T>::type *xA, int gw, int sub,
                                             T &f_out, T &abs_out, typename MagOf<T>::type &amin_out, typename MagOf<T>::type &xmin_out) {
+  static_assert(W == 1, "the warp split (W warps per point group) was measured slower and is gone");
   constexpr bool TRACK = true;
   using M = typename MagOf<T>::type;                   // magnitudes (round-off bounds, pivot ratios): one per sample point of the lane
+  // DIST: the MQ_WL lanes of a point group carry MQ_WL points; lane role `sub` computes the scalars of point `sub` in plain
+  // binary64 from zl (its coordinates) and writes that component of S; U, V, G, Rp are gathered with shuffles. Otherwise all
+  // lanes compute all points of the group from z (role 0 writes).
+  constexpr int NPT = PtsOf<T>::n;
+  constexpr bool DIST = LANES && !SPREAD && NPT > 1 && NPT == MQ_WL;
   StreamReader rd = rd_io;                             // work on a register copy (the caller's object lives in local memory across this call)
   const DevHeader &h = *v.h;
   T nodeval[MQ_MAXNODEVAL];
   M nodeabs[TRACK ? MQ_MAXNODEVAL : 1];
   T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
   M amin(1.0), xmin(1.0);
+  double amin_l = 1.0, xmin_l = 1.0;                   // DIST: of this lane's point
   const bool owner = gw == 0 && sub == 0 && (!SPREAD || threadIdx.x == 0);   // the lane whose f_out is used
   const uint32_t s_S = smem_u32(S), sstride = (uint32_t)(stride * sizeof(T));
   rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
-    T U = T(1.0), V = T(0.0), G = T(1.0);
+    T U = T(1.0), V = T(0.0), G = T(1.0); M Rp(1.0);
     if constexpr (LANES) __syncwarp();                 // every lane role has finished reading S of the previous piece
     if constexpr (SPREAD) __syncthreads();             // (entry-parallel) nobody still reads S of the previous piece
-    if (gw == 0) piece_scalars<T>(g, z, S, stride, SPREAD ? threadIdx.x == 0 : sub == 0, U, V, G, amin, xmin);
-    if constexpr (W > 1 || SPREAD) __syncthreads();              // S of this piece is complete before any warp gathers from it
+    if constexpr (DIST) {
+      double Ul, Vl, Gl, Rl;
+      piece_scalars<double>(g, zl, SComp<NPT>(S, stride, sub), true, Ul, Vl, Gl, Rl, amin_l, xmin_l);
+      const int l0 = (threadIdx.x & 31) % (32 / MQ_WL);          // lane of role 0 of this point group; role k sits at l0 + k * (32 / MQ_WL)
+#pragma unroll
+      for (int k = 0; k < NPT; k++) {
+        const int src = l0 + k * (32 / MQ_WL);
+        mq_setc(U, k, __shfl_sync(0xffffffffu, Ul, src)); mq_setc(V, k, __shfl_sync(0xffffffffu, Vl, src));
+        mq_setc(G, k, __shfl_sync(0xffffffffu, Gl, src)); mq_setc(Rp, k, __shfl_sync(0xffffffffu, Rl, src));
+      }
+    } else piece_scalars<T>(g, z, SWhole<T>{S, stride}, SPREAD ? threadIdx.x == 0 : sub == 0, U, V, G, Rp, amin, xmin);
+    if constexpr (SPREAD) __syncthreads();              // S of this piece is complete before any warp gathers from it
     else if constexpr (LANES) __syncwarp();
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
@@ -814,7 +783,8 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           N[o][p][c] = t; Na[o][p][c] = ta;
         }
         __syncthreads();
-      } else if constexpr (LANES && W == 1 && MQ_RUNS) {
+      } else {
+        static_assert(SPREAD || LANES, "one lane per point without the lane split is not supported any more");
         RunAcc<T> ra; ra.key = -1; ra.racc = T(0.0); ra.racca = M(0.0);
         for (int left = tb.nfam; left > 0;) {
           if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
@@ -825,100 +795,6 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
           left -= run;
         }
         if (ra.key >= 0) { N[ra.key >> 7][(ra.key >> 3) & 15][ra.key & 7] = ra.racc; Na[ra.key >> 7][(ra.key >> 3) & 15][ra.key & 7] = ra.racca; }
-      } else {
-      int key = -1; T racc = T(0.0); M racca(0.0);
-      bool have = false; uint32_t a0 = 0; uint64_t hd = 0, hl = 0, w0 = 0, w1 = 0;   // entry header, this lane's member header + first index words
-      int unit = 0;                                                                  // evaluation units are dealt round-robin to the W warps
-      // this lane's member of the entry at address a with (uniform) header hu: its header word and first two index words
-      auto fetch_member = [&](uint32_t a, uint64_t hu, int m, uint64_t &ml, uint64_t &m0, uint64_t &m1) {
-        const uint32_t iw = (hu & 7) == MQ_PAD_MARK ? 0u : (uint32_t)(hu >> 16 & 0xFFFF);
-        const uint32_t ma = a + 8 * MQ_WL + 8 * iw * (uint32_t)m;
-        ml = lds_u64(a + 8 * (uint32_t)m); m0 = lds_u64(ma); m1 = lds_u64(ma + 8);
-      };
-      for (int left = tb.nfam; left > 0;) {
-        if (!have) {
-          if (rd.pos == MQ_CHUNK_WORDS) rd.advance();
-          a0 = rd.addr(); hd = lds_u64(a0);
-          if constexpr (LANES) fetch_member(a0, hd, sub, hl, w0, w1);
-        }
-        const int idxw = (int)(hd >> 16 & 0xFFFF);
-        const int c = (int)(hd & 7), kd = (int)(hd >> 3 & 7);
-        if (c == MQ_PAD_MARK) { rd.pos += 1 + idxw; have = false; continue; }
-        const int size = MQ_WL * (1 + idxw) + (int)(hd >> 32 & 0xFFFF), npos = rd.pos + size;
-        // software pipeline: fetch the next entry's header and index words before this entry's arithmetic
-        uint32_t an = a0 + 8 * size; uint64_t hdn = 0, hln = 0, n0 = 0, n1 = 0;
-        const bool havenext = npos < MQ_CHUNK_WORDS;
-        if (havenext) { hdn = lds_u64(an); if constexpr (LANES) fetch_member(an, hdn, sub, hln, n0, n1); }
-        // pair this entry with the next one if it has the same shape (binary64: doubles the ILP of the warp)
-        bool dual = false;
-        if constexpr (std::is_same<T, double>::value && LANES && MQ_DUAL) {
-          if (havenext && left > 1 && c <= 3 && (int)(hdn & 63) == (int)(hd & 63)) {
-            const int size2 = MQ_WL * (1 + (int)(hdn >> 16 & 0xFFFF)) + (int)(hdn >> 32 & 0xFFFF);
-            dual = npos + size2 <= MQ_CHUNK_WORDS;
-          }
-        }
-        const int nb = c * (2 * c - 1) + kd;
-        const uint32_t ustride = kd ? 16u : 8u;                        // bytes between the members' coefficient units
-        // member header ml: scalar factors and accumulation key; sidx: shared address of the member's index bytes
-        // accumulation key (output, pattern, grade) of a member. The run accumulator is (re)loaded from N when the key changes,
-        // BEFORE the family is evaluated: the local-memory load then has the whole evaluation to complete.
-        auto open_key = [&](uint64_t ml) {
-          const int keyk = (int)((ml & 7) | ((ml >> 6 & 15) << 3) | ((ml >> 14 & 1) << 7));
-          if (keyk != key) {
-            if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
-            key = keyk; racc = N[key >> 7][(key >> 3) & 15][key & 7]; if constexpr (TRACK) racca = Na[key >> 7][(key >> 3) & 15][key & 7];
-          }
-        };
-        // member header ml: scalar factors; sidx: shared address of the member's index bytes
-        auto account = [&](T val, M amag, uint64_t ml, uint32_t sidx) {
-          const int ns = (int)(ml >> 10 & 15);
-          val = mq_norm(val);                      // the family code works on unnormalised pairs (dd_arith.cuh)
-#pragma unroll 1
-          for (int i = 0; i < ns; i++) { const T sc = SAcc<T>::lds(s_S + lds_u8(sidx + nb + i) * sstride, sstride); val = val * sc; amag = amag * (mq_absd(sc) + M(0.125)); }   // + 1/8: the factor's own absolute round-off (A_t = 1 - x_t may be tiny)
-          racc = racc + val;
-          if constexpr (TRACK) racca += amag;      // sum of |monomial| bounds: sees the cancellation inside a family too
-        };
-        if (dual) {
-          if constexpr (std::is_same<T, double>::value && LANES) {
-            const int idxw2 = (int)(hdn >> 16 & 0xFFFF), size2 = MQ_WL * (1 + idxw2) + (int)(hdn >> 32 & 0xFFFF), npos2 = npos + size2;
-            const uint32_t a2 = an + 8 * size2;
-            uint64_t hd3 = 0, hl3 = 0, m0 = 0, m1 = 0;
-            const bool have3 = npos2 < MQ_CHUNK_WORDS;
-            if (have3) { hd3 = lds_u64(a2); fetch_member(a2, hd3, sub, hl3, m0, m1); }
-            if (W == 1 || unit % W == gw) {
-              const uint32_t sidxA = a0 + 8 * MQ_WL + 8 * idxw * sub, sidxB = an + 8 * MQ_WL + 8 * idxw2 * sub;
-              const double4 vAB = family_dispatch2(c * 8 + kd, w0, w1, n0, n1, sidxA, a0 + 8 * MQ_WL * (1 + idxw) + ustride * sub,
-                                                   sidxB, an + 8 * MQ_WL * (1 + idxw2) + ustride * sub, s_S, sstride);
-              open_key(hl); account(T(vAB.x), vAB.z, hl, sidxA);
-              open_key(hln); account(T(vAB.y), vAB.w, hln, sidxB);
-            }
-            unit++;
-            rd.pos = npos2; left -= 2;
-            have = have3; a0 = a2; hd = hd3; hl = hl3; w0 = m0; w1 = m1;
-            continue;
-          }
-        }
-        if (W == 1 || unit % W == gw) {
-#pragma unroll 1
-          for (int q = 0; q < (LANES ? 1 : MQ_WL); q++) {
-            const int m = LANES ? sub : q;
-            if constexpr (!LANES) fetch_member(a0, hd, m, hl, w0, w1);
-            const uint32_t sidx = a0 + 8 * MQ_WL + 8 * idxw * m, scoef = a0 + 8 * MQ_WL * (1 + idxw) + ustride * m;
-            static_assert(sizeof(T) <= 32, "wider types use the entry-parallel path");
-            open_key(hl);
-#if defined(MQ_EXP_NOFAM)
-            FamRes<T> fr; fr.v = T(1.0); fr.a = M(1.0);          // experiment: everything but the family evaluation
-#else
-            const FamRes<T> fr = family_dispatch<T>(c * 8 + kd, w0, w1, sidx, scoef, s_S, sstride);
-#endif
-            account(fr.v, fr.a, hl, sidx);
-          }
-        }
-        unit++;
-        rd.pos = npos; left--;
-        have = havenext; a0 = an; hd = hdn; hl = hln; w0 = n0; w1 = n1;
-      }
-      if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; if constexpr (TRACK) Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
       }
       if constexpr (LANES && MQ_WL > 1) {              // add the partial sums of the lane roles: afterwards every lane holds the totals
         for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
@@ -931,26 +807,16 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             }
           }
       }
+      if constexpr (!SPREAD) {                         // the families' magnitudes leave out prod max(1,|r_inner|) <= Rp
+        for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
+#pragma unroll
+          for (int c = 0; c < MQ_NGRADE; c++) Na[o][p][c] = Na[o][p][c] * Rp;
+      }
       if (tb.nout == 1 && (tb.op == MQ_OP_U || tb.op == MQ_OP_LMU)) {   // these tables hold 12*coefficient (coef_gen.hpp)
         const T i12 = T(1.0) / T(12.0);
         for (int p = 0; p < npat; p++)
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] = Na[0][p][c] * M(1.0 / 12.0); }
-      }
-      if constexpr (W > 1) {                           // add the partial sums of the other warps of the group into warp 0
-        for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++) {
-          if (gw > 0) {
-#pragma unroll
-            for (int c = 0; c < MQ_NGRADE; c++) { xT[((gw - 1) * MQ_NGRADE + c) * stride] = N[o][p][c]; xA[((gw - 1) * MQ_NGRADE + c) * stride] = Na[o][p][c]; }
-          }
-          __syncthreads();
-          if (gw == 0) {
-            for (int w = 0; w < W - 1; w++)
-#pragma unroll
-              for (int c = 0; c < MQ_NGRADE; c++) { N[o][p][c] = N[o][p][c] + xT[(w * MQ_NGRADE + c) * stride]; Na[o][p][c] += xA[(w * MQ_NGRADE + c) * stride]; }
-          }
-          __syncthreads();
-        }
       }
       // nodes that use this table: combine with the children's graded values. Only the owner lane of a point does this
       // (the other lane role holds the same totals: doing it twice would only double the local-memory traffic)
@@ -1001,6 +867,13 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
       f = f + contrib;
       if constexpr (TRACK) asum = asum + T(c < nd.ngr ? nodeabs[nd.val_off + c] * mq_absd(mq_mag(scale)) : M(0.0));
       else asum = asum + mq_abs(contrib);
+    }
+  }
+  if constexpr (DIST) {
+    const int l0 = (threadIdx.x & 31) % (32 / MQ_WL);
+#pragma unroll
+    for (int k = 0; k < NPT; k++) {
+      mq_setc(amin, k, __shfl_sync(0xffffffffu, amin_l, l0 + k * (32 / MQ_WL))); mq_setc(xmin, k, __shfl_sync(0xffffffffu, xmin_l, l0 + k * (32 / MQ_WL)));
     }
   }
   f_out = f; abs_out = asum; amin_out = amin; xmin_out = xmin;
