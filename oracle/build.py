@@ -8,24 +8,33 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liboracle.so")
-SRC = ["qed_oracle.c"]
-DEPS = SRC + ["qed_combi.h", "qed_piece.h", "qed_sampler.h", "qed_tables.h", "qed_eval_impl.h"]
+LIB_A = os.path.join(HERE, "liboracle_a.so")
+# two independent libraries: the table-driven oracle ("Oracle-B") and the per-point definition ("Oracle-A", qed_oracle_a.c),
+# which includes none of Oracle-B's headers
+TARGETS = {LIB: (["qed_oracle.c"], ["qed_combi.h", "qed_piece.h", "qed_sampler.h", "qed_tables.h", "qed_eval_impl.h"]),
+           LIB_A: (["qed_oracle_a.c"], [])}
 
 
-def build(force=False):
+def _build_one(lib, src, deps, force):
     import hashlib
     h = hashlib.sha256()
-    for f in DEPS:
+    for f in src + deps:
         with open(os.path.join(HERE, f), "rb") as fh:
             h.update(fh.read())
-    digest, stamp = h.hexdigest(), LIB + ".stamp"
-    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == digest:
-        return LIB      # content hash, not mtime: snapshots lose mtimes
+    digest, stamp = h.hexdigest(), lib + ".stamp"
+    if not force and os.path.exists(lib) and os.path.exists(stamp) and open(stamp).read().strip() == digest:
+        return lib      # content hash, not mtime: snapshots lose mtimes
     cmd = ["gcc", "-O2", "-std=gnu11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
-           "-Wall", "-Wno-unused-function", "-o", LIB] + [os.path.join(HERE, f) for f in SRC] + ["-lm"]
+           "-Wall", "-Wno-unused-function", "-o", lib] + [os.path.join(HERE, f) for f in src] + ["-lm"]
     subprocess.check_call(cmd)
     with open(stamp, "w") as fh:
         fh.write(digest)
+    return lib
+
+
+def build(force=False):
+    for lib, (src, deps) in TARGETS.items():
+        _build_one(lib, src, deps, force)
     return LIB
 
 

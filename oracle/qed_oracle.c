@@ -10,10 +10,15 @@
  *   (iii) the Monte Carlo sums of w=f/p and w^2.
  * Pins: see tests/test_oracle_*.py (A1^(2)=1/2 pointwise and integrated, the 2-loop value
  * -0.344166, diagram counts 3213 and Table 1 N_diag, Dirichlet closed forms, Philox known
- * answers, projector identities, an independent per-point numpy evaluator).
- * Parity status: L=1,2 pinned by the paper's values; L=3 pinned by the independent evaluator
- * and structural identities; L=4,5 values are "parity unpinned" by the paper (no per-graph
- * numbers are printed) — only structural pins apply.
+ * answers, projector identities) and tests/test_oracle_a.py: every term of every 1-, 2- and 3-loop
+ * graph (and of some 4-loop graphs) against Oracle-A (qed_oracle_a.c: the definition evaluated per
+ * point with explicit matrices, pairings and traces, its own forests and operator assignment), the
+ * infrared pin that tells the operator L from U, hand-written term lists, the oracle-only 3-loop sum.
+ * Parity status: L=1,2 pinned by the paper's values; L=3 pinned by Oracle-A, the infrared/UV scaling
+ * pins and (softly) the literature value; the branches that first appear at L>=3 (L on intermediate
+ * elements of I[G], nested forests, several S-children) are covered by those pins: swapping OP_L for
+ * OP_U in op_of() fails four CPU tests. L=4,5 VALUES are "parity unpinned" by the paper (no per-graph
+ * numbers are printed) — structural pins and Oracle-A at 4 loops apply.
  */
 #include "qed_combi.h"
 #include "qed_piece.h"

@@ -1,6 +1,6 @@
 """tests/golden/make_oracle_golden.py — writes the stored oracle results under tests/golden/.
 
-Calls ONLY oracle/ (never the CUDA path).  Usage:  python tests/golden/make_oracle_golden.py two_loop [n_per_graph]
+Calls ONLY oracle/ (never the CUDA path).  Usage:  python tests/golden/make_oracle_golden.py two_loop|three_loop [n_per_graph]
 """
 import os
 import sys
@@ -10,20 +10,33 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 from oracle import pyoracle as po  # noqa: E402
 
 
-def two_loop(n):
-    lines = ["# Oracle Monte Carlo of the six 2-loop graphs (BASELINE.json configs[1]), binary64 integrand values,",
-             "# seed 2, first_sample 0, %d points per graph, Deg floor 0.5, no cap.  Written by make_oracle_golden.py (oracle only)." % n,
-             "# The sum is pinned by north_star: -0.344166.",
-             "# e chords k m n n_points mean sigma"]
-    for g in po.all_graphs(2):
-        d = po.Diagram(g, deg_floor=0.5)
-        s1, s2, _ = d.integrate(0, n, 2, 0)
+def _mc_all(L, n, seed, deg_floor, path, head):
+    """Monte Carlo of ALL graphs of loop order L with the oracle alone, mode 2 (binary64 value unless the truth flag
+    |f64 - fwide| > 1e-10 |fwide| is set, then the binary128 value: DESIGN.md O8), sums kept exactly (hex)"""
+    lines = head + ["# e chords k m n n_points mean sigma S1(hex) S2(hex) n_truth_flagged"]
+    for g in po.all_graphs(L):
+        d = po.Diagram(g, deg_floor=deg_floor)
+        s1, s2, nf = d.integrate(0, n, seed, 2)
         m, e = po.estimate(s1, s2, n)
         k = po.graph_class(g)
-        lines.append("%d %s %d %d %d %d %.9f %.9f" % (g.ext_pos, "".join("%d%d" % c for c in g.chords()), k[0], k[1], k[2], n, m, e))
+        lines.append("%d %s %d %d %d %d %.9f %.9f %s %s %d" % (g.ext_pos, "".join("%d%d" % c for c in g.chords()), k[0], k[1], k[2], n, m, e, float(s1).hex(), float(s2).hex(), nf))
         print(lines[-1], flush=True)
-    with open(os.path.join(HERE, "oracle_two_loop_mc.txt"), "w") as fh:
-        fh.write("\n".join(lines) + "\n")
+        with open(path, "w") as fh:           # rewritten after every graph: a long run can be watched and resumed by hand
+            fh.write("\n".join(lines) + "\n")
+
+
+def two_loop(n):
+    _mc_all(2, n, 2, 0.5, os.path.join(HERE, "oracle_two_loop_mc.txt"),
+            ["# Oracle Monte Carlo of the six 2-loop graphs (BASELINE.json configs[1]), seed 2, first_sample 0, %d points per graph," % n,
+             "# Deg floor 0.5, no cap, oracle mode 2 (binary128 value where binary64 loses more than 1e-10).  Written by make_oracle_golden.py (oracle only).",
+             "# The sum of the six means is pinned by north_star: -0.344166."])
+
+
+def three_loop(n):
+    _mc_all(3, n, 3, 0.75, os.path.join(HERE, "oracle_three_loop_mc.txt"),
+            ["# Oracle Monte Carlo of all 50 3-loop graphs (BASELINE.json configs[2]), seed 3, first_sample 0, %d points per graph," % n,
+             "# default Deg (floor 0.75, no cap), oracle mode 2.  Written by make_oracle_golden.py (oracle only).",
+             "# Soft pin: the literature value of the 3-loop contribution of graphs without lepton loops, 0.904979 (SURVEY.md P9; not in PAPER.md)."])
 
 
 def high_loop(L, indices, n, seed, first):
@@ -48,3 +61,5 @@ if __name__ == "__main__":
         high_loop(int(sys.argv[2]), [int(x) for x in sys.argv[3].split(",")], int(sys.argv[4]), 5, 1000)
     if sys.argv[1] == "two_loop":
         two_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 20000000)
+    if sys.argv[1] == "three_loop":
+        three_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 1000000)
