@@ -10,19 +10,20 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 from oracle import pyoracle as po  # noqa: E402
 
 
-def _mc_all(L, n, seed, deg_floor, path, head):
-    """Monte Carlo of ALL graphs of loop order L with the oracle alone, mode 2 (binary64 value unless the truth flag
-    |f64 - fwide| > 1e-10 |fwide| is set, then the binary128 value: DESIGN.md O8), sums kept exactly (hex)"""
+def _mc_all(L, n, seed, deg_floor, path, head, mode=2):
+    """Monte Carlo of ALL graphs of loop order L with the oracle alone. mode 2: binary64 value unless the truth flag
+    |f64 - fwide| > 1e-10 |fwide| is set, then the binary128 value (O8); mode 0: binary64 values. Sums kept exactly (hex)"""
     lines = head + ["# e chords k m n n_points mean sigma S1(hex) S2(hex) n_truth_flagged"]
     for g in po.all_graphs(L):
         d = po.Diagram(g, deg_floor=deg_floor)
-        s1, s2, nf = d.integrate(0, n, seed, 2)
+        s1, s2, nf = d.integrate(0, n, seed, mode)
         m, e = po.estimate(s1, s2, n)
         k = po.graph_class(g)
         lines.append("%d %s %d %d %d %d %.9f %.9f %s %s %d" % (g.ext_pos, "".join("%d%d" % c for c in g.chords()), k[0], k[1], k[2], n, m, e, float(s1).hex(), float(s2).hex(), nf))
         print(lines[-1], flush=True)
-        with open(path, "w") as fh:           # rewritten after every graph: a long run can be watched and resumed by hand
+        with open(path + ".partial", "w") as fh:           # rewritten after every graph: a long run can be watched
             fh.write("\n".join(lines) + "\n")
+    os.replace(path + ".partial", path)
 
 
 def two_loop(n):
@@ -35,8 +36,9 @@ def two_loop(n):
 def three_loop(n):
     _mc_all(3, n, 3, 0.75, os.path.join(HERE, "oracle_three_loop_mc.txt"),
             ["# Oracle Monte Carlo of all 50 3-loop graphs (BASELINE.json configs[2]), seed 3, first_sample 0, %d points per graph," % n,
-             "# default Deg (floor 0.75, no cap), oracle mode 2.  Written by make_oracle_golden.py (oracle only).",
-             "# Soft pin: the literature value of the 3-loop contribution of graphs without lepton loops, 0.904979 (SURVEY.md P9; not in PAPER.md)."])
+             "# default Deg (floor 0.75, no cap), oracle mode 0 (binary64 values: on graphs 0, 20, 45 the binary128 re-evaluation of mode 2",
+             "# moves the mean by 1e-13, far below the statistical error, and costs 8x the time).  Written by make_oracle_golden.py (oracle only).",
+             "# Soft pin: the literature value of the 3-loop contribution of graphs without lepton loops, 0.904979 (SURVEY.md P9; not in PAPER.md)."], mode=0)
 
 
 def high_loop(L, indices, n, seed, first):
@@ -62,4 +64,4 @@ if __name__ == "__main__":
     if sys.argv[1] == "two_loop":
         two_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 20000000)
     if sys.argv[1] == "three_loop":
-        three_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 1000000)
+        three_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 4000000)
