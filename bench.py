@@ -33,7 +33,9 @@ def parse():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (4 = the metric's workload)")
     ap.add_argument("--graphs", type=int, default=0, help="use only the first G graphs of the config (0 = all; for debugging)")
     ap.add_argument("--batch", type=int, default=37888, help="sample points per diagram per step")
-    ap.add_argument("--ref-points", type=int, default=768, help="oracle sample points per step (reference arm / cpu_baseline)")
+    ap.add_argument("--ref-points", type=int, default=384, help="oracle sample points per graph and step (reference arm / cpu_baseline)")
+    ap.add_argument("--ref-graphs", type=int, default=3, help="graphs of the workload the oracle is timed on, spread over the set")
+    ap.add_argument("--no-second-policy", action="store_true", help="skip the timed step under the purely relative precision policy (w_abs_tol = 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -69,28 +71,40 @@ class ClockSampler(threading.Thread):
 
 
 def oracle_run(args, graphs, seed, steps, warmup):
-    """times the CPU oracle as it stands on a bounded sample of the workload: the first graph(s) of the set"""
+    """times the CPU oracle as it stands on a bounded sample of the workload: --ref-graphs graphs spread evenly over the set
+    (the set is sorted by canonical index = by external-vertex position, so the sample spans the gauge classes), --ref-points
+    points per graph and step, after one untimed warm-up pass per graph"""
     from oracle import pyoracle as po
-    idx, g = graphs[0]
-    og = po.OracleGraph.make(g[0], g[1], g[2])
-    t0 = time.perf_counter()
-    d = po.Diagram(og)
-    prep = time.perf_counter() - t0
+    from paper_1905_08007_b200 import workloads
+    G = len(graphs)
+    pick = sorted(set(int(round(k * (G - 1) / max(1, args.ref_graphs - 1))) for k in range(args.ref_graphs))) if args.ref_graphs > 1 else [0]
     n = args.ref_points
-    for w in range(warmup):
-        d.integrate(w * n, n, seed, 2)
-    t0 = time.perf_counter()
-    s1 = s2 = 0.0
-    for k in range(steps):
-        a, b, _ = d.integrate((warmup + k) * n, n, seed, 2)
-        s1 += a
-        s2 += b
-    dt = time.perf_counter() - t0
-    tot = n * steps
-    mean, err = po.estimate(s1, s2, tot)
+    prep = dt = 0.0
+    var = 0.0
+    classes = []
+    for gi in pick:
+        idx, g = graphs[gi]
+        t0 = time.perf_counter()
+        d = po.Diagram(po.OracleGraph.make(g[0], g[1], g[2]))
+        prep += time.perf_counter() - t0
+        for w in range(max(1, warmup)):
+            d.integrate(w * n, n, seed, 2)
+        t0 = time.perf_counter()
+        s1 = s2 = 0.0
+        for k in range(steps):
+            a, b, _ = d.integrate((max(1, warmup) + k) * n, n, seed, 2)
+            s1 += a
+            s2 += b
+        dt += time.perf_counter() - t0
+        mean, err = po.estimate(s1, s2, n * steps)
+        var += err * err
+        classes.append("%d,%d,%d" % workloads.graph_class(g))
+        del d
+    tot = n * steps * len(pick)
     return {"value": tot / dt, "seconds": dt, "cores": po.num_threads(), "prepare_s": prep, "points": tot,
-            "sample": "graph #%d of the workload (canonical index %d), %d points per step, binary64 + __float128 re-evaluation" % (0, idx, n),
-            "mean": mean, "err": err, "sigma2_time": err * err * dt}
+            "sample": "graphs #%s of the workload (classes %s), %d points per graph and step, %d step(s) after a warm-up pass, binary64 + __float128 re-evaluation" % (
+                ",".join(str(x) for x in pick), " ".join(classes), n, steps),
+            "sigma2_time": var * dt}
 
 
 def run_reference(args):
@@ -212,18 +226,56 @@ def run_ours(args):
     ach_f64 = flops_f64 / (ms_f64 * 1e-3) if ms_f64 > 0 else 0.0
     ach_dd = flops_dd / (ms_dd * 1e-3) if ms_dd > 0 else 0.0
     dom = "k_batch_dd" if ms_dd > ms_f64 else "k_batch_f64"
+    # DRAM traffic of the dominant kernel: not measurable without a profiler, so it is read from the ncu capture of this launch
+    # configuration that profiles/r2_traffic.json records (written by hand from `ncu --set full`, command in profiles/r2_summary.md);
+    # null when the run is another configuration or the file has no entry for the kernel
+    traffic, traffic_note = None, "no ncu capture of this configuration under profiles/"
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as fh:
+            tj = json.load(fh)
+        ent = tj.get(dom)
+        if ent and ent["graphs"] == G and ent["batch"] == B and ent["config"] == args.config:
+            traffic, traffic_note = ent["dram_bytes_per_launch"], "from profile, not live: " + ent["source"]
+    except (OSError, ValueError, KeyError):
+        pass
     ach = ach_dd if dom == "k_batch_dd" else ach_f64
     roofline = {"bound": "alu", "kernel": dom, "achieved": ach / 1e12, "peak": peak_flops / 1e12, "unit": "TFLOP/s", "frac": ach / peak_flops,
-                "traffic": 73.74e9 if (dom == "k_batch_f64" and G == 256 and B == 37888 and args.config == 4) else None,
-                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of k_batch_f64 in this launch configuration, one ncu --set full capture "
-                                "(profiles/r1_v6_ncu_f64_fullconfig_details.txt: 35.8 GB read + 37.9 GB written in a 1.75 s launch = 42 GB/s, 0.6 % of HBM bandwidth); the "
-                                "algorithmic bytes are ~0 (no per-sample input or output): the reads are the table streams missing L2 (2.3 GB of tables), the writes per-thread stack (node values, graded sums)",
+                "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": "FP64 FMA peak measured live by mc_fp64_peak (MEASURED_PEAKS.json has no FP64 entry)",
                 "kernels": {"k_batch_f64": {"ms_per_step": ms_f64 / args.steps, "achieved_tflops": ach_f64 / 1e12, "frac": ach_f64 / peak_flops, "points_per_step": G * B},
                             "k_batch_dd": {"ms_per_step": ms_dd / args.steps, "achieved_tflops": ach_dd / 1e12, "frac": ach_dd / peak_flops,
                                            "points_per_step": float(c[0].sum()) / args.steps,
                                            "note": "double-double: one algorithmic flop costs 5-6 binary64 instructions (pair arithmetic), so frac is bounded by ~0.18"},
                             "k_batch_qd": {"ms_per_step": ms_qd / args.steps, "points_per_step": n_qd / args.steps}}}
+    # ---- the same step under the purely relative precision policy (w_abs_tol = 0: north_star's literal reading, a point is
+    #      accepted in binary64 only if its relative round-off bound holds), one warm-up + one timed step ----
+    second = None
+    if not args.no_second_policy:
+        for d in diagrams:
+            d.set_precision(w_abs_tol=0.0)
+        batch_rel = mc.Batch(diagrams, B)
+        for d in diagrams:
+            d.set_precision()                      # back to the defaults (the first batch copied its values at creation)
+        s_rel = torch.zeros(2, G, dtype=torch.float64, device="cuda")
+        c_rel = torch.zeros(2, G, dtype=torch.int64, device="cuda")
+        f0 = state["first"]
+        batch_rel.integrate(f0, B, seed, stream, s_rel[0], s_rel[1], c_rel[0], c_rel[1])
+        s_rel.zero_(); c_rel.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier(); e0.record()
+        batch_rel.integrate(f0 + B, B, seed, stream, s_rel[0], s_rel[1], c_rel[0], c_rel[1])
+        e1.record(); barrier()
+        ms_rel = e0.elapsed_time(e1)
+        # the default policy on the same sample range, for a like-for-like difference of the sums
+        s_def = torch.zeros(2, G, dtype=torch.float64, device="cuda")
+        c_def = torch.zeros(2, G, dtype=torch.int64, device="cuda")
+        batch.integrate(f0 + B, B, seed, stream, s_def[0], s_def[1], c_def[0], c_def[1])
+        barrier()
+        second = {"policy": "relative only (w_abs_tol = 0)", "value": world * G * B / (ms_rel * 1e-3), "unit": UNIT, "ms_per_step": ms_rel, "steps": 1,
+                  "flagged_fraction": float(c_rel[0].sum().item()) / (G * B), "flagged_fraction_default_same_range": float(c_def[0].sum().item()) / (G * B),
+                  "max_abs_difference_of_estimates": float(((s_rel[0] - s_def[0]).abs() / B).max().item()),
+                  "sum_of_estimates": float((s_rel[0] / B).sum().item()), "sum_of_estimates_default_same_range": float((s_def[0] / B).sum().item())}
+        del batch_rel
     # ---- end to end through the public host-pointer API (mc_batch_integrate_host: results copied back every call) ----
     barrier()
     t0 = time.perf_counter()
@@ -256,13 +308,14 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[%d]: %d seeded 5-loop graphs without lepton loops, %d points per graph per step" % (args.config, G, B) if args.config == 4
                        else "configs[%d]: %d graphs, %d points per graph per step" % (args.config, G, B),
-                       "n_graphs": G, "batch": B, "seed": seed, "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
+                       "n_graphs": G, "batch": B, "seed": seed, "second_policy": second,
+                       "headline_policy": "relative OR absolute acceptance (w_abs_tol = 1e-10 on the weight f/p; DESIGN.md section 6)", "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
                        "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "precision": precision, "dropped": int(c[1].sum()),
                        "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
                        "algorithmic_flop_per_sample_mean": sum(flop) / G, "classes": classes},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = oracle_run(args, graphs, seed, 1, 0)
+        r = oracle_run(args, graphs, seed, 1, 1)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
                                 "prepare_s": r["prepare_s"], "sigma2_time_s": r["sigma2_time"]}
     if rank == 0:

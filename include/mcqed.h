@@ -16,8 +16,13 @@
  * that touches the device returns MC_ECUDA when no CUDA device / driver is usable.
  *
  * Conventions. All functions return 0 (MC_OK) or a negative error code; nothing throws across the
- * boundary; no global state; handles are thread-safe for concurrent reads. "HOST" / "DEVICE" says
- * where a pointer must live. Line index convention (R1): electron line t (joining path
+ * boundary. Global state: the launch counter behind mc_kernel_launch_count and the static scratch of
+ * mc_integrate_static, nothing else. A handle (mc_diagram, mc_batch) owns device scratch that every
+ * device call on it writes (partial sums, flagged lists, counters): introspection calls may run concurrently,
+ * but at most ONE device call (mc_integrate*, mc_eval_*, mc_batch_integrate*) per handle may be in flight at a
+ * time — calls on one stream are ordered and safe, calls on the same handle from two streams or threads race on
+ * the scratch and return wrong sums without an error. Distinct handles are independent.
+ * "HOST" / "DEVICE" says where a pointer must live. Line index convention (R1): electron line t (joining path
  * positions t,t+1) has index t, photon i (chords sorted by their first end) has index 2L+i; M=3L.
  */
 #ifndef MCQED_H
@@ -174,6 +179,20 @@ int mc_batch_integrate(mc_batch *, uint64_t first_sample, uint64_t n_samples, ui
 int mc_batch_integrate_host(mc_batch *, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
                             double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped);
 void mc_batch_free(mc_batch *);
+
+/* Sample allocation across the graphs of a set (the deliverable is a sum over thousands of graphs whose
+ * individual errors differ by orders of magnitude; the paper does not disclose its allocation).
+ *   mc_batch_integrate_counts: as mc_batch_integrate, but diagram j processes sample indices first_sample[j] ..
+ *     first_sample[j] + n_samples[j] - 1 (HOST arrays of n_diagrams elements; n_samples[j] may be 0; ranges longer than the
+ *     batch capacity are split into passes). The arrays are copied to the device at the start of every pass (synchronises
+ *     the stream once per pass); outputs as in mc_batch_integrate (DEVICE, accumulated into).
+ *   mc_allocate_samples: the split of a cost budget sum_j n_j cost_j = budget that minimises sum_j sigma_j^2 / n_j:
+ *     n_j ~ sigma_j / sqrt(cost_j), at least n_min each. sigma_j: per-sample standard deviation of the weight of diagram j (from
+ *     a pilot pass), cost_j: cost per sample in any unit (e.g. flop_per_sample of mc_diagram_info). HOST arrays. */
+int mc_batch_integrate_counts(mc_batch *, const uint64_t *first_sample, const uint64_t *n_samples, uint64_t seed, uint32_t flags,
+                              void *cuda_stream, double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged,
+                              unsigned long long *out_n_dropped);
+int mc_allocate_samples(const double *sigma, const double *cost, int32_t n_diagrams, double budget, uint64_t n_min, uint64_t *n_out);
 
 /* Parity hook: per-point values for comparison with the oracle. DEVICE outputs, any may be NULL:
  * z_out n*M (row = point, column = line index), order_out n*M (the Hepp sector j_1..j_M),

@@ -18,7 +18,7 @@ FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
     "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags", "mc_diagram_set_precision",
-    "mc_integrate", "mc_integrate_host", "mc_integrate_static", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
+    "mc_integrate", "mc_integrate_host", "mc_integrate_static", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_integrate_counts", "mc_allocate_samples", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
 
@@ -78,6 +78,8 @@ def lib():
         L.mc_batch_create.argtypes = [C.POINTER(vp), C.c_int32, u64, C.POINTER(vp)]
         L.mc_batch_integrate.argtypes = [vp, u64, u64, u64, C.c_uint32, vp, vp, vp, vp, vp]
         L.mc_batch_integrate_host.argtypes = [vp, u64, u64, u64, C.c_uint32, vp, vp, vp, vp, vp]
+        L.mc_batch_integrate_counts.argtypes = [vp, vp, vp, u64, C.c_uint32, vp, vp, vp, vp, vp]
+        L.mc_allocate_samples.argtypes = [dp, dp, C.c_int32, C.c_double, u64, C.POINTER(C.c_uint64)]
         L.mc_batch_free.argtypes = [vp]
         L.mc_batch_free.restype = None
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -234,12 +236,29 @@ class Batch:
         _check(lib().mc_batch_integrate(self.h, first_sample, n_samples, seed, flags, _ptr(stream), _ptr(out_sum), _ptr(out_sumsq),
                                         _ptr(out_n_flagged), _ptr(out_n_dropped)), "mc_batch_integrate")
 
+    def integrate_counts(self, first_samples, n_samples, seed, stream, out_sum, out_sumsq, out_n_flagged, out_n_dropped, flags=0):
+        """mc_batch_integrate_counts: per-diagram sample ranges (host sequences of len(diagrams) integers)"""
+        f = np.ascontiguousarray(first_samples, np.uint64)
+        n = np.ascontiguousarray(n_samples, np.uint64)
+        assert len(f) == len(n) == len(self.diagrams)
+        _check(lib().mc_batch_integrate_counts(self.h, _ptr(f), _ptr(n), seed, flags, _ptr(stream), _ptr(out_sum), _ptr(out_sumsq),
+                                               _ptr(out_n_flagged), _ptr(out_n_dropped)), "mc_batch_integrate_counts")
+
     def integrate_host(self, first_sample, n_samples, seed, stream=None, flags=0):
         n = len(self.diagrams)
         s, s2, nf, nd = np.zeros(n), np.zeros(n), np.zeros(n, np.uint64), np.zeros(n, np.uint64)
         _check(lib().mc_batch_integrate_host(self.h, first_sample, n_samples, seed, flags, _ptr(stream), _ptr(s), _ptr(s2), _ptr(nf), _ptr(nd)),
                "mc_batch_integrate_host")
         return s, s2, nf, nd
+
+
+def allocate_samples(sigma, cost, budget, n_min=1):
+    """mc_allocate_samples: n_j ~ sigma_j / sqrt(cost_j) with sum n_j cost_j = budget"""
+    sg, cs = np.ascontiguousarray(sigma, np.float64), np.ascontiguousarray(cost, np.float64)
+    out = np.zeros(len(sg), np.uint64)
+    dp = C.POINTER(C.c_double)
+    _check(lib().mc_allocate_samples(sg.ctypes.data_as(dp), cs.ctypes.data_as(dp), len(sg), float(budget), int(n_min), out.ctypes.data_as(C.POINTER(C.c_uint64))), "mc_allocate_samples")
+    return out
 
 
 def kernel_launch_count():

@@ -76,7 +76,11 @@ struct BatchDiag {
 struct BatchView {
   const BatchDiag *dg;             // [nd]
   int nd; uint32_t cap;            // diagrams; capacity (points per diagram per call, multiple of PTS_F64)
-  uint32_t ipd;                    // binary64 items per diagram in this call
+  uint32_t ipd;                    // binary64 items per diagram in this call (uniform calls: every diagram gets the same range)
+  // per-diagram sample ranges (mc_batch_integrate_counts; nullptr in a uniform call): first item, first sample index, samples
+  const uint32_t *f64_start;       // [nd+1]
+  const uint64_t *v_first;         // [nd]
+  const uint32_t *v_n;             // [nd]
   uint32_t *item_cnt;              // [nd*cap/PTS_F64] flagged points of a binary64 item
   uint32_t *flag_raw;              // [nd*cap] item-local lists (relative sample indices), entry b*PTS_F64+k of diagram d
   uint32_t *flag_list;             // [nd*cap] compacted, ascending
@@ -95,6 +99,7 @@ struct mc_batch {
   int grid_f64 = 0, grid_dd = 0, grid_qd = 0;
   size_t smem_f64 = 0, smem_dd = 0, smem_qd = 0;
   void *d_mem = nullptr;                   // one device allocation holding every array of BatchView
+  uint32_t *d_f64_start = nullptr; uint64_t *d_v_first = nullptr; uint32_t *d_v_n = nullptr;   // inside d_mem (per-diagram ranges)
   mqk::BatchView view{};                   // the kernel argument (pointers into d_mem)
 };
 

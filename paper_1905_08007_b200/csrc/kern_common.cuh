@@ -58,6 +58,10 @@ __device__ __forceinline__ int batch_find(const uint32_t *start, int nd, uint32_
   return lo;
 }
 
+// sample range of diagram d in this call: uniform (first, n) or the per-diagram arrays of mc_batch_integrate_counts
+__device__ __forceinline__ uint64_t batch_first(const BatchView &bv, int d, uint64_t first) { return bv.v_first ? bv.v_first[d] : first; }
+__device__ __forceinline__ uint64_t batch_n(const BatchView &bv, int d, uint64_t n) { return bv.v_n ? (uint64_t)bv.v_n[d] : n; }
+
 __device__ __forceinline__ bool bad_point(const double *z, int M, double p) {   // DESIGN.md A15
   bool bad = !(p > 0.0) || !isfinite(p);
   for (int i = 0; i < M; i++) bad |= !(z[i] >= 0x1p-600);

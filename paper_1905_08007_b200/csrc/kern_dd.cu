@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
     const unsigned long long i = (unsigned long long)(item - bv.dd_start[d]) * PTS_DD + ro.slot; const bool live = i < cnt && ro.sub == 0 && ro.gw == 0;
     const uint32_t rel = bv.flag_list[(size_t)d * bv.cap + (i < cnt ? i : cnt - 1)];
     double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
+    const double p = draw_point<false>(v, batch_first(bv, d, first) + rel, seed, z, nullptr);
     dd f, a; double amin, xmin;
     eval_integrand<dd, W_DD, true>(v, rd, z, nullptr, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};

@@ -170,12 +170,12 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
 // ------------------------------------------------------------------ batched path, binary64 tier (a1-a7 for every diagram of a batch)
 // Persistent CTAs; item = PTS_F64 consecutive sample indices of one diagram, taken from queue[0].
 // Flagged points are compacted inside the item in thread order (ballot + prefix): deterministic lists.
-__global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv, uint64_t first, uint64_t n, uint64_t seed, int scal_len, int no_dd) {
+__global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv, uint64_t first_u, uint64_t n_u, uint64_t seed, int scal_len, int no_dd) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item, s_wcnt[TPB_F64 / 32];
   const Roles<FT, 1, MQ_WL> ro(smem_raw, scal_len);
   StreamReader rd; setup_reader<1, MQ_WL>(rd, smem_raw, scal_len, sizeof(FT));
-  const uint32_t total = (uint32_t)bv.nd * bv.ipd;
+  const uint32_t total = bv.f64_start ? bv.f64_start[bv.nd] : (uint32_t)bv.nd * bv.ipd;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (;;) {
     __syncthreads();
@@ -183,7 +183,9 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     __syncthreads();
     const uint32_t item = s_item;
     if (item >= total) break;
-    const int d = (int)(item / bv.ipd); const uint32_t b = item % bv.ipd;
+    const int d = bv.f64_start ? batch_find(bv.f64_start, bv.nd, item) : (int)(item / bv.ipd);
+    const uint32_t b = bv.f64_start ? item - bv.f64_start[d] : item % bv.ipd;
+    const uint64_t first = batch_first(bv, d, first_u), n = batch_n(bv, d, n_u);
     const DiagView v = make_view(bv.dg[d].blob);
     MqPrec pr = bv.dg[d].pr;
     if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
@@ -229,9 +231,10 @@ __global__ void __launch_bounds__(128) k_batch_compact(BatchView bv) {
   uint32_t *out = bv.flag_list + (size_t)d * bv.cap;
   if (t == 0) s_base = 0;
   __syncthreads();
-  for (uint32_t b0 = 0; b0 < bv.ipd; b0 += 128) {
+  const uint32_t ipd = bv.f64_start ? bv.f64_start[d + 1] - bv.f64_start[d] : bv.ipd;
+  for (uint32_t b0 = 0; b0 < ipd; b0 += 128) {
     const uint32_t b = b0 + t;
-    const unsigned c = b < bv.ipd ? cnt[b] : 0u;
+    const unsigned c = b < ipd ? cnt[b] : 0u;
     sc[t] = c;
     __syncthreads();
     for (int off = 1; off < 128; off <<= 1) {        // inclusive scan
@@ -262,8 +265,9 @@ __global__ void k_batch_finish(BatchView bv, int tiers, double *out_sum, double 
   if (d == 0) bv.queue[0] = 0ull;
   if (d >= bv.nd) return;
   KahanPair a{0.0, 0.0}, b{0.0, 0.0};
-  const double *p = bv.part_f64 + (size_t)d * bv.ipd * 4;
-  for (uint32_t i = 0; i < bv.ipd; i++) { a.merge(p[i * 4], p[i * 4 + 1]); b.merge(p[i * 4 + 2], p[i * 4 + 3]); }
+  const uint32_t ipd = bv.f64_start ? bv.f64_start[d + 1] - bv.f64_start[d] : bv.ipd;
+  const double *p = bv.part_f64 + (size_t)(bv.f64_start ? bv.f64_start[d] : d * bv.ipd) * 4;
+  for (uint32_t i = 0; i < ipd; i++) { a.merge(p[i * 4], p[i * 4 + 1]); b.merge(p[i * 4 + 2], p[i * 4 + 3]); }
   unsigned long long ndrop = bv.ndrop[d];
   if (tiers > 1)
     for (uint32_t i = bv.dd_start[d]; i < bv.dd_start[d + 1]; i++) { const double *q = bv.part_dd + (size_t)i * 4; a.merge(q[0], q[1]); b.merge(q[2], q[3]); }

@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(TPB_QD) k_batch_qd(BatchView bv, uint64_t firs
     const DiagView v = make_view(bv.dg[d].blob);
     const uint32_t rel = bv.lost_list[(size_t)d * bv.lostcap + (item - bv.qd_start[d])];
     double z[MQ_MAXM];
-    const double p = draw_point<false>(v, first + rel, seed, z, nullptr);
+    const double p = draw_point<false>(v, batch_first(bv, d, first) + rel, seed, z, nullptr);
     const double fd = qd_point(v, rd, ro, z);
     if (threadIdx.x == 0) {
       double *dst = bv.part_qd + (size_t)item * 4;

@@ -144,12 +144,12 @@ int mc_integrate_host(const mc_diagram *d, uint64_t first_sample, uint64_t n_sam
   cudaStream_t st = (cudaStream_t)cuda_stream;
   struct Out { double s, s2; unsigned long long nf, nd; } *dev = nullptr, host{0, 0, 0, 0};
   MQ_CK(cudaMallocAsync((void **)&dev, sizeof(Out), st));
-  MQ_CK(cudaMemsetAsync(dev, 0, sizeof(Out), st));
-  int rc = mc_integrate(d, first_sample, n_samples, seed, cuda_stream, &dev->s, &dev->s2, &dev->nf, &dev->nd);
-  if (rc != MC_OK) { cudaFreeAsync(dev, st); return rc; }
-  MQ_CK(cudaMemcpyAsync(&host, dev, sizeof(Out), cudaMemcpyDeviceToHost, st));
-  MQ_CK(cudaFreeAsync(dev, st));
-  MQ_CK(cudaStreamSynchronize(st));
+  int rc = cudaMemsetAsync(dev, 0, sizeof(Out), st) == cudaSuccess ? MC_OK : MC_ECUDA;      // every exit below frees dev
+  if (rc == MC_OK) rc = mc_integrate(d, first_sample, n_samples, seed, cuda_stream, &dev->s, &dev->s2, &dev->nf, &dev->nd);
+  if (rc == MC_OK && cudaMemcpyAsync(&host, dev, sizeof(Out), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = MC_ECUDA;
+  if (cudaFreeAsync(dev, st) != cudaSuccess && rc == MC_OK) rc = MC_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == MC_OK) rc = MC_ECUDA;
+  if (rc != MC_OK) return rc;
   if (sum) *sum = host.s;
   if (sumsq) *sumsq = host.s2;
   if (n_flagged) *n_flagged = host.nf;
@@ -237,7 +237,8 @@ int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint6
   auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
   const size_t o_dg = take(nd * sizeof(mqk::BatchDiag)), o_cnt = take(nd * ipd * 4), o_raw = take(nd * b->cap * 4), o_list = take(nd * b->cap * 4),
                o_lost = take(nd * b->lostcap * 4), o_nf = take(nd * 8), o_nl = take(nd * 8), o_ndp = take(nd * 8), o_dds = take((nd + 1) * 4),
-               o_qds = take((nd + 1) * 4), o_p1 = take(nd * ipd * 32), o_p2 = take(nd * idd * 32), o_p3 = take(nd * iqd * 32), o_q = take(32);
+               o_qds = take((nd + 1) * 4), o_p1 = take(nd * ipd * 32), o_p2 = take(nd * idd * 32), o_p3 = take(nd * iqd * 32), o_q = take(32),
+               o_fs = take((nd + 1) * 4), o_vf = take(nd * 8), o_vn = take(nd * 4);
   if (cudaMalloc(&b->d_mem, off) != cudaSuccess) { delete b; return MC_ENOMEM; }
   if (cudaMemset(b->d_mem, 0, off) != cudaSuccess) { mc_batch_free(b); return MC_ECUDA; }
   char *base = (char *)b->d_mem;
@@ -252,6 +253,8 @@ int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint6
   v.dd_start = (uint32_t *)(base + o_dds); v.qd_start = (uint32_t *)(base + o_qds);
   v.part_f64 = (double *)(base + o_p1); v.part_dd = (double *)(base + o_p2); v.part_qd = (double *)(base + o_p3);
   v.queue = (unsigned long long *)(base + o_q);
+  v.f64_start = nullptr; v.v_first = nullptr; v.v_n = nullptr;
+  b->d_f64_start = (uint32_t *)(base + o_fs); b->d_v_first = (uint64_t *)(base + o_vf); b->d_v_n = (uint32_t *)(base + o_vn);
   b->smem_f64 = mq_batch_smem_f64(b->scal_len); b->smem_dd = mq_batch_smem_dd(b->scal_len); b->smem_qd = mq_batch_smem_qd(b->scal_len);
   if (mq_batch_config_f64(b->smem_f64, &b->grid_f64) != 0 || mq_batch_config_dd(b->smem_dd, &b->grid_dd) != 0 || mq_batch_config_qd(b->smem_qd, &b->grid_qd) != 0) {
     mc_batch_free(b); return MC_ECUDA;
@@ -264,35 +267,87 @@ void mc_batch_free(mc_batch *b) {
   if (b->d_mem) cudaFree(b->d_mem);
   delete b;
 }
+namespace {
+// one pass of the three tiers over the sample ranges described by v (uniform: first, n; per diagram: v.f64_start / v_first / v_n)
+void batch_pass(mc_batch *b, const mqk::BatchView &v, uint64_t items, uint64_t first, uint64_t n, uint64_t seed, uint32_t flags, mq_stream st,
+                double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
+  const bool no_dd = flags & 1u, no_qd = flags & 2u;
+  mq_launch_batch_f64(v, (int)std::min<uint64_t>((uint64_t)b->grid_f64, items), b->smem_f64, first, n, seed, b->scal_len, no_dd ? 1 : 0, st);
+  mq_launch_batch_compact(v, st);
+  g_launches += 2;
+  if (!no_dd) {
+    mq_launch_batch_ranges(v, 1, st);
+    mq_launch_batch_dd(v, b->grid_dd, b->smem_dd, first, seed, b->scal_len, st);
+    g_launches += 2;
+    if (!no_qd) {
+      mq_launch_batch_ranges(v, 2, st);
+      mq_launch_batch_qd(v, b->grid_qd, b->smem_qd, first, seed, b->scal_len, st);
+      g_launches += 2;
+    }
+  }
+  mq_launch_batch_finish(v, no_dd ? 1 : no_qd ? 2 : 3, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
+  g_launches++;
+}
+}  // namespace
+
 int mc_batch_integrate(mc_batch *b, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
                        double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
   if (!b) return MC_EINVAL;
   mq_stream st = (mq_stream)cuda_stream;
-  const bool no_dd = flags & 1u, no_qd = flags & 2u;
   for (uint64_t done = 0; done < n_samples; done += b->cap) {
     const uint64_t n = std::min<uint64_t>(b->cap, n_samples - done);
     mqk::BatchView v = b->view;
     v.ipd = (uint32_t)((n + mqk::PTS_F64 - 1) / mqk::PTS_F64);
-    const uint64_t items = (uint64_t)v.ipd * v.nd;
-    mq_launch_batch_f64(v, (int)std::min<uint64_t>((uint64_t)b->grid_f64, items), b->smem_f64, first_sample + done, n, seed, b->scal_len, no_dd ? 1 : 0, st);
-    mq_launch_batch_compact(v, st);
-    g_launches += 2;
-    if (!no_dd) {
-      mq_launch_batch_ranges(v, 1, st);
-      mq_launch_batch_dd(v, b->grid_dd, b->smem_dd, first_sample + done, seed, b->scal_len, st);
-      g_launches += 2;
-      if (!no_qd) {
-        mq_launch_batch_ranges(v, 2, st);
-        mq_launch_batch_qd(v, b->grid_qd, b->smem_qd, first_sample + done, seed, b->scal_len, st);
-        g_launches += 2;
-      }
-    }
-    mq_launch_batch_finish(v, no_dd ? 1 : no_qd ? 2 : 3, out_sum, out_sumsq, out_n_flagged, out_n_dropped, st);
-    g_launches++;
+    batch_pass(b, v, (uint64_t)v.ipd * v.nd, first_sample + done, n, seed, flags, st, out_sum, out_sumsq, out_n_flagged, out_n_dropped);
   }
   MQ_CK(cudaGetLastError());
   return MC_OK;
 }
+
+int mc_batch_integrate_counts(mc_batch *b, const uint64_t *first_sample, const uint64_t *n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
+                              double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
+  if (!b || !first_sample || !n_samples) return MC_EINVAL;
+  cudaStream_t cst = (cudaStream_t)cuda_stream;
+  const size_t nd = b->diags.size();
+  uint64_t longest = 0;
+  for (size_t d = 0; d < nd; d++) longest = std::max(longest, n_samples[d]);
+  std::vector<uint32_t> start(nd + 1), vn(nd);
+  std::vector<uint64_t> vf(nd);
+  for (uint64_t done = 0; done < longest; done += b->cap) {        // diagrams whose range is longer than the capacity take several passes
+    uint64_t items = 0;
+    for (size_t d = 0; d < nd; d++) {
+      const uint64_t left = n_samples[d] > done ? n_samples[d] - done : 0, n = std::min<uint64_t>(b->cap, left);
+      start[d] = (uint32_t)items; vn[d] = (uint32_t)n; vf[d] = first_sample[d] + done;
+      items += (n + mqk::PTS_F64 - 1) / mqk::PTS_F64;
+    }
+    if (items > 0xFFFFFFFFull) return MC_EINVAL;
+    start[nd] = (uint32_t)items;
+    if (items == 0) continue;
+    MQ_CK(cudaMemcpyAsync(b->d_f64_start, start.data(), (nd + 1) * 4, cudaMemcpyHostToDevice, cst));
+    MQ_CK(cudaMemcpyAsync(b->d_v_first, vf.data(), nd * 8, cudaMemcpyHostToDevice, cst));
+    MQ_CK(cudaMemcpyAsync(b->d_v_n, vn.data(), nd * 4, cudaMemcpyHostToDevice, cst));
+    MQ_CK(cudaStreamSynchronize(cst));                              // the host vectors are reused by the next pass
+    mqk::BatchView v = b->view;
+    v.ipd = 0; v.f64_start = b->d_f64_start; v.v_first = b->d_v_first; v.v_n = b->d_v_n;
+    batch_pass(b, v, items, 0, 0, seed, flags, (mq_stream)cuda_stream, out_sum, out_sumsq, out_n_flagged, out_n_dropped);
+  }
+  MQ_CK(cudaGetLastError());
+  return MC_OK;
+}
+
+/* N_j ~ sigma_j / sqrt(cost_j): the split of a total cost budget that minimises sum_j sigma_j^2 / N_j (Neyman allocation with
+ * unequal costs); every diagram gets at least n_min samples. sigma_j = the per-sample standard deviation of the weight. */
+int mc_allocate_samples(const double *sigma, const double *cost, int32_t n_diagrams, double budget, uint64_t n_min, uint64_t *n_out) {
+  if (!sigma || !cost || !n_out || n_diagrams < 1 || !(budget > 0)) return MC_EINVAL;
+  double norm = 0;
+  for (int j = 0; j < n_diagrams; j++) { if (!(cost[j] > 0) || !(sigma[j] >= 0)) return MC_EINVAL; norm += sigma[j] * std::sqrt(cost[j]); }
+  for (int j = 0; j < n_diagrams; j++) {
+    const double n = norm > 0 ? budget * sigma[j] / (std::sqrt(cost[j]) * norm) : budget / (cost[j] * n_diagrams);
+    n_out[j] = std::max<uint64_t>(n_min, (uint64_t)std::llround(n));
+  }
+  return MC_OK;
+}
+
 int mc_batch_integrate_host(mc_batch *b, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
                             double *sum, double *sumsq, unsigned long long *n_flagged, unsigned long long *n_dropped) {
   if (!b) return MC_EINVAL;
@@ -300,17 +355,15 @@ int mc_batch_integrate_host(mc_batch *b, uint64_t first_sample, uint64_t n_sampl
   const size_t nd = b->diags.size();
   char *dev = nullptr;
   MQ_CK(cudaMallocAsync((void **)&dev, nd * 32, st));
-  MQ_CK(cudaMemsetAsync(dev, 0, nd * 32, st));
   double *ds = (double *)dev, *ds2 = ds + nd; unsigned long long *dnf = (unsigned long long *)(ds2 + nd), *dnd = dnf + nd;
-  int rc = mc_batch_integrate(b, first_sample, n_samples, seed, flags, cuda_stream, ds, ds2, dnf, dnd);
-  if (rc != MC_OK) { cudaFreeAsync(dev, st); return rc; }
-  if (sum) MQ_CK(cudaMemcpyAsync(sum, ds, nd * 8, cudaMemcpyDeviceToHost, st));
-  if (sumsq) MQ_CK(cudaMemcpyAsync(sumsq, ds2, nd * 8, cudaMemcpyDeviceToHost, st));
-  if (n_flagged) MQ_CK(cudaMemcpyAsync(n_flagged, dnf, nd * 8, cudaMemcpyDeviceToHost, st));
-  if (n_dropped) MQ_CK(cudaMemcpyAsync(n_dropped, dnd, nd * 8, cudaMemcpyDeviceToHost, st));
-  MQ_CK(cudaFreeAsync(dev, st));
-  MQ_CK(cudaStreamSynchronize(st));
-  return MC_OK;
+  // every exit after the allocation goes through the free below
+  int rc = cudaMemsetAsync(dev, 0, nd * 32, st) == cudaSuccess ? MC_OK : MC_ECUDA;
+  if (rc == MC_OK) rc = mc_batch_integrate(b, first_sample, n_samples, seed, flags, cuda_stream, ds, ds2, dnf, dnd);
+  auto back = [&](void *dst, const void *src) { if (rc == MC_OK && dst && cudaMemcpyAsync(dst, src, nd * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = MC_ECUDA; };
+  back(sum, ds); back(sumsq, ds2); back(n_flagged, dnf); back(n_dropped, dnd);
+  if (cudaFreeAsync(dev, st) != cudaSuccess && rc == MC_OK) rc = MC_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == MC_OK) rc = MC_ECUDA;
+  return rc;
 }
 
 unsigned long long mc_kernel_launch_count(void) { return g_launches.load(); }
