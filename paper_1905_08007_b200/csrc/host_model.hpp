@@ -245,7 +245,9 @@ struct SamplerTables {
   std::vector<double> deg, invdeg, Z;
   double C = 0;
 
-  void build(const VertexGraph &g, const ForestTerms &ft, double dfloor, double dcap) {
+  // dfloor_ir: the value on sets whose I-closure is the whole graph (the soft-photon sets of PAPER.md:78); <= 0: same as dfloor
+  void build(const VertexGraph &g, const ForestTerms &ft, double dfloor, double dcap, double dfloor_ir_in = 0.0) {
+    const double dfloor_ir = dfloor_ir_in > 0.0 ? dfloor_ir_in : dfloor;
     M = g.M; size_t n = (size_t)1 << M; uint32_t full = (uint32_t)n - 1;
     deg.assign(n, 0.0); invdeg.assign(n, 0.0); Z.assign(n, 0.0);
     // pieces of the maximal forests only: shrinking more never lowers the loop count (S5)
@@ -282,7 +284,7 @@ struct SamplerTables {
       uint32_t sb = s;   // I-closure
       for (int i = 0; i < g.L; i++) if ((s & path[i]) == path[i]) sb |= 1u << (2 * g.L + i);
       double d;
-      if (sb == full) d = dfloor;
+      if (sb == full) d = dfloor_ir;
       else {
         int best = 0;
         for (size_t f = 0; f < sets.size(); f++) {

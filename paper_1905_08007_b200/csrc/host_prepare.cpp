@@ -68,7 +68,9 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     for (int i = 0; i < uf->n_sub; i++) if (uf->seg_lo[i] != d->ft.subs[i].lo || uf->seg_hi[i] != d->ft.subs[i].hi) return MC_EINVAL;
     for (int i = 0; i < uf->n_forest; i++) if (uf->forest_mask[i] != d->ft.forests[i]) return MC_EINVAL;
   }
-  d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap);
+  double deg_floor_ir = 0.0;
+  if (const char *env = std::getenv("MCQED_DEG_IR")) deg_floor_ir = atof(env);      // experiments only
+  d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap, deg_floor_ir);
 
   // ---- term trees -> unique pieces (geoms) and nodes ----
   Builder B(*d);

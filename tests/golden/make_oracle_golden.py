@@ -54,13 +54,21 @@ def high_loop(L, indices, n, seed, first):
         for k in range(n):
             lines.append("%d %d %s %s" % (idx, k, float(r["fwide"][k]).hex(), float(r["f64"][k]).hex()))
         print("graph", idx, "done", flush=True)
-    with open(os.path.join(HERE, "oracle_points_L%d.txt" % L), "w") as fh:
-        fh.write("\n".join(lines) + "\n")
+        del d
+        with open(os.path.join(HERE, "oracle_points_L%d.txt.partial" % L), "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+    os.replace(os.path.join(HERE, "oracle_points_L%d.txt.partial" % L), os.path.join(HERE, "oracle_points_L%d.txt" % L))
 
+
+# 33 graphs of BASELINE.json configs[4] (canonical indices): the first graph of each of the nine classes of Table 1, the graph with
+# the most formula terms (2821: 40 terms), the graphs with the most self-energy subgraphs (691, 705, 6351: four each), the rest
+# spread evenly over the set; plus the three graphs of the round-1 file
+L5_GRAPHS = [3, 49, 453, 691, 692, 705, 709, 1029, 1408, 1443, 1529, 1954, 2110, 2145, 2302, 2324, 2718, 2806, 2821, 2825, 2877, 3120,
+             3304, 3625, 4026, 4651, 4984, 5454, 5512, 5660, 5957, 6290, 6351]
 
 if __name__ == "__main__":
     if sys.argv[1] == "high_loop":
-        high_loop(int(sys.argv[2]), [int(x) for x in sys.argv[3].split(",")], int(sys.argv[4]), 5, 1000)
+        high_loop(int(sys.argv[2]), L5_GRAPHS if sys.argv[3] == "default" else [int(x) for x in sys.argv[3].split(",")], int(sys.argv[4]), 5, 1000)
     if sys.argv[1] == "two_loop":
         two_loop(int(float(sys.argv[2])) if len(sys.argv) > 2 else 20000000)
     if sys.argv[1] == "three_loop":

@@ -7,11 +7,13 @@ on the same seeded points (north_star tolerances):
   * fixed-point-set sums: relative 1e-9; final estimates: within the combined 1-sigma error.
 """
 import math
+import os
 
 import numpy as np
 import pytest
 
 pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
 
 torch = pytest.importorskip("torch")
 
@@ -166,23 +168,38 @@ def test_gpu_prepared_tables_equal_host_prepared(mc):
         a.close(); b.close()
 
 
-def test_five_loop_points_against_stored_oracle_values(mc):
+def test_five_loop_points_against_stored_oracle_values(po, mc):
     """BASELINE.json configs[4] scale (L=5, M=15): per-point parity against oracle values stored by
-    tests/golden/make_oracle_golden.py (the oracle needs minutes per 5-loop graph to build its tables)"""
+    tests/golden/make_oracle_golden.py (the oracle needs minutes per 5-loop graph to build its tables): >= 30 graphs covering
+    all nine classes of Table 1, the graph with the most terms and the graphs with the most self-energy subgraphs, 64 points
+    each. Sample coordinates, densities and Hepp sectors are compared BIT-EXACTLY with the oracle's sampler run live
+    (level 0: no integrand tables needed). The batched path bench.py times (k_batch_f64 / dd / qd through
+    mc_batch_integrate_host) is compared with the oracle's fixed-point-set sums at 1e-9. The family shapes (c, kd) the
+    evaluator has static code for are all exercised by these graphs (census)."""
     from conftest import read_golden
     from paper_1905_08007_b200 import workloads
+    import sys
+    sys.path.insert(0, HERE)
+    from blob_interp import Blob
     rows = read_golden("oracle_points_L5.txt")
     gs = workloads.all_graphs(5)
     by_graph = {}
     for idx, k, fw, f64 in rows:
         by_graph.setdefault(int(idx), []).append((int(k), float.fromhex(fw), float.fromhex(f64)))
-    assert len(by_graph) >= 3
-    for idx, pts in by_graph.items():
+    assert len(by_graph) >= 30
+    assert len(set(workloads.graph_class(gs[i]) for i in by_graph)) == 9
+    st = torch.cuda.current_stream().cuda_stream
+    shapes = set()
+    ds, sums = [], []
+    for idx, pts in sorted(by_graph.items()):
         g = gs[idx]
         d = mc.Diagram(g[0], g[1], g[2])
         assert d.id() == idx
         n = len(pts)
         r = _gpu_points(mc, d, 1000, n, 5)
+        o = po.Diagram(po.OracleGraph.make(*g), level=0)
+        zo, pz, oo = o.sample(1000, n, 5)
+        assert np.array_equal(r["z"], zo) and np.array_equal(r["p"], pz) and np.array_equal(r["order"], oo), idx
         fw = np.array([p[1] for p in sorted(pts)])
         fo64 = np.array([p[2] for p in sorted(pts)])
         unfl = r["flag"] == 0
@@ -194,6 +211,48 @@ def test_five_loop_points_against_stored_oracle_values(mc):
         assert np.all(np.abs(r["f"] - fw)[acc] <= 1e-10 * r["p"][acc])
         truth = np.abs(fo64 - fw) > 1e-10 * np.abs(fw)
         assert not np.any(truth & unfl)
+        assert np.all(truth[acc])                        # flag 2 = precision loss detected: these ARE the oracle's truth-flagged points
+        w = fw / pz
+        sums.append((math.fsum(w), math.fsum(np.abs(w)), math.fsum(w * w), float(np.abs((r["f"] - fw) / pz)[acc].sum())))
+        b = Blob(d.blob())
+        for ti in range(b.h["ntable"]):
+            shapes.update((f[0], f[1]) for f in b.families(ti))
+        ds.append(d)
+    # every (c, kd) the kernels dispatch on occurs in these graphs' tables
+    want = {(c, kd) for c in range(5) for kd in range(7) if kd <= (6 if c <= 2 else 4 if c == 3 else 2)}
+    assert shapes == want, (sorted(want - shapes), sorted(shapes - want))
+    # the batched path on the same 64 points per graph
+    s1, s2, nf, nd = mc.Batch(ds, 64).integrate_host(1000, 64, 5, st)
+    for k, (ws, wa, w2, dacc) in enumerate(sums):
+        assert abs(s1[k] - ws) <= 1e-9 * wa and abs(s2[k] - w2) <= 1e-9 * w2 and nd[k] == 0, (k, s1[k], ws, wa)
+        assert dacc <= 1e-9 * wa                         # the points accepted by the absolute bound move the sum by less than 1e-9
+    for d in ds:
+        d.close()
+
+
+def test_config3_four_loop_set_builds_runs_and_matches_oracle_on_a_sample(po, mc):
+    """BASELINE.json configs[3]: the 128 seeded 4-loop graphs (seed 4). All of them build and run through the batched path; on
+    eight of them spread over the set the per-diagram sums of 256 points agree with the oracle's fixed-point-set sums (binary128
+    values) at 1e-9 and the sample points are bit-exact."""
+    from paper_1905_08007_b200 import workloads
+    graphs = workloads.config_graphs(3)
+    assert len(graphs) == 128
+    st = torch.cuda.current_stream().cuda_stream
+    ds = [mc.Diagram(*g) for _, g in graphs]
+    for (idx, _), d in zip(graphs, ds):
+        assert d.id() == idx
+    n, seed = 256, 4
+    s1, s2, nf, nd = mc.Batch(ds, 4096).integrate_host(0, n, seed, st)
+    assert not nd.any() and np.all(np.isfinite(s1)) and np.all(s2 > 0)
+    for k in range(0, 128, 16):
+        o = po.Diagram(po.OracleGraph.make(*graphs[k][1]))
+        zo, pz, oo = o.sample(0, n, seed)
+        r = _gpu_points(mc, ds[k], 0, n, seed)
+        assert np.array_equal(r["z"], zo) and np.array_equal(r["p"], pz) and np.array_equal(r["order"], oo)
+        w = o.eval_z(zo, wide=True)["fwide"] / pz
+        assert abs(s1[k] - math.fsum(w)) <= 1e-9 * math.fsum(np.abs(w)), (k, s1[k], math.fsum(w))
+        assert abs(s2[k] - math.fsum(w * w)) <= 1e-9 * math.fsum(w * w)
+    for d in ds:
         d.close()
 
 
