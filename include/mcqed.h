@@ -60,12 +60,13 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {0.75, 1e30, 3e4, 1e-2, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5).
+/* NULL => defaults {1.0, 1e30, 3e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
+ * value of Deg on the sets whose I-closure is the whole graph, the soft-photon sets (<= 0: same as deg_floor).
  * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
  *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.
  * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0).
  * flags bit 1: build no numerator tables (introspection of the combinatorics only; host handles). */
-typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; } mc_options;
+typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; double deg_floor_ir; } mc_options;
 
 /* Host-side preparation of one diagram (not on the timed path): validates the graph, enumerates
  * subgraphs/forests/terms (forest-like formula, O1), builds Deg and the sector-sum table

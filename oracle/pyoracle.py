@@ -52,7 +52,7 @@ def lib():
         for f in ("oracle_det_log2", "oracle_det_exp2"):
             getattr(_lib, f).restype = C.c_double
             getattr(_lib, f).argtypes = [C.c_double]
-        _lib.oracle_prepare_diagram.argtypes = [C.POINTER(OracleGraph), C.c_double, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
+        _lib.oracle_prepare_diagram.argtypes = [C.POINTER(OracleGraph), C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         _lib.oracle_free_diagram.argtypes = [C.c_void_p]
     return _lib
 
@@ -118,10 +118,16 @@ def philox(ctr, key):
 class Diagram:
     """One prepared diagram (combinatorics + sampler tables [+ integrand tables])."""
 
-    def __init__(self, g, deg_floor=0.75, deg_cap=1e30, level=1, prune=1):
+    def __init__(self, g, deg_floor=None, deg_cap=1e30, level=1, prune=1, deg_floor_ir=None):
+        """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (1.0, 0.5) (S5); a deg_floor given alone also is the value
+        on the soft-photon sets (the one-floor reading of round 1)"""
         self.g = g
         self.h = C.c_void_p()
-        rc = lib().oracle_prepare_diagram(C.byref(g), deg_floor, deg_cap, level, prune, C.byref(self.h))
+        if deg_floor is None:
+            deg_floor, deg_floor_ir = 1.0, (0.5 if deg_floor_ir is None else deg_floor_ir)
+        elif deg_floor_ir is None:
+            deg_floor_ir = deg_floor
+        rc = lib().oracle_prepare_diagram(C.byref(g), deg_floor, deg_cap, deg_floor_ir, level, prune, C.byref(self.h))
         if rc != 0:
             raise ValueError("oracle_prepare_diagram failed: %d" % rc)
         info = (C.c_int64 * 8)()

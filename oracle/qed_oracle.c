@@ -140,7 +140,7 @@ int oracle_graph_mirror(const oracle_graph *og, oracle_graph *out) {
 
 /* level 0: combinatorics + sampler tables; level 1: + integrand tables. max_grade_prune: 1 = skip the
  * top own grade of pieces under A and (L-U) (it vanishes identically, O4), 0 = compute it */
-int oracle_prepare_diagram(const oracle_graph *og, double deg_floor, double deg_cap, int level, int prune, oracle_diagram **out) {
+int oracle_prepare_diagram(const oracle_graph *og, double deg_floor, double deg_cap, double deg_floor_ir, int level, int prune, oracle_diagram **out) {
   oracle_diagram *d = (oracle_diagram *)calloc(1, sizeof *d);
   if (to_graph(og, &d->g)) { free(d); return -1; }
   d->id = graph_canonical_id(&d->g);
@@ -148,7 +148,7 @@ int oracle_prepare_diagram(const oracle_graph *og, double deg_floor, double deg_
   d->nforest = enum_forests(d->subs, d->nsub, d->forests);
   Term terms[MAXTERM];
   d->nterm = enum_terms(&d->g, d->subs, d->nsub, d->forests, d->nforest, terms);
-  build_deg(&d->g, d->subs, d->nsub, d->forests, d->nforest, deg_floor, deg_cap, &d->stab);
+  build_deg(&d->g, d->subs, d->nsub, d->forests, d->nforest, deg_floor, deg_cap, deg_floor_ir > 0 ? deg_floor_ir : deg_floor, &d->stab);
   d->geoms = (GeomEntry *)calloc(MAXGEOM, sizeof(GeomEntry));
   d->nodes = (Node *)calloc(MAXNODE, sizeof(Node));
   for (int t = 0; t < d->nterm; t++) {

@@ -113,9 +113,11 @@ typedef struct {
   double C;        /* normalisation of Eq.(1) */
 } SamplerTab;
 
-/* Deg(s) = clamp(|sbar| - |e(sbar)|/2 - 2 max_F sum_H loops_H(sbar∩H), floor, cap); sbar=full -> floor */
+/* Deg(s) = clamp(|sbar| - |e(sbar)|/2 - 2 max_F sum_H loops_H(sbar∩H), floor, cap); sbar=full -> floor_ir: the sets whose I-closure
+ * is the whole graph are the soft-photon sets; the infrared pin (tests/test_oracle_a.py) measures one power of the
+ * scale over a nested PAIR of such limits, so their exponent must stay near 1/2 while the UV-type sets can take 1 (S5) */
 static void build_deg(const Graph *g, const Sub *subs, int nsub, const uint32_t *forests, int nforest,
-                      double dfloor, double dcap, SamplerTab *tab) {
+                      double dfloor, double dcap, double dfloor_ir, SamplerTab *tab) {
   int M = g->M; unsigned full = (1u << M) - 1;
   tab->M = M;
   tab->deg = (double *)calloc((size_t)1 << M, sizeof(double));
@@ -141,7 +143,7 @@ static void build_deg(const Graph *g, const Sub *subs, int nsub, const uint32_t 
   for (unsigned s = 1; s < full; s++) {
     unsigned sb = i_closure(g, s);
     double d;
-    if (sb == full) d = dfloor;
+    if (sb == full) d = dfloor_ir;
     else {
       int best = 0;
       for (int f = 0; f < nforest; f++) {

@@ -57,7 +57,7 @@ struct Builder {
 int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out) {
   if (!graph || !out) return MC_EINVAL;
   std::unique_ptr<mc_diagram> d(new mc_diagram);
-  d->opt = opts ? *opts : mc_options{0.75, 1e30, 3e4, 1e-2, 0u};
+  d->opt = opts ? *opts : mc_options{1.0, 1e30, 3e4, 1e-2, 0u, 0.5};
   if (!(d->opt.deg_floor > 0) || !(d->opt.deg_cap >= d->opt.deg_floor) || !(d->opt.cond_max > 0)) return MC_EINVAL;
   if (!d->g.build(graph->loops, graph->ext_pos, graph->chord_a, graph->chord_b)) return MC_EINVAL;
   d->id = d->g.canonicalId();
@@ -68,9 +68,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     for (int i = 0; i < uf->n_sub; i++) if (uf->seg_lo[i] != d->ft.subs[i].lo || uf->seg_hi[i] != d->ft.subs[i].hi) return MC_EINVAL;
     for (int i = 0; i < uf->n_forest; i++) if (uf->forest_mask[i] != d->ft.forests[i]) return MC_EINVAL;
   }
-  double deg_floor_ir = 0.0;
-  if (const char *env = std::getenv("MCQED_DEG_IR")) deg_floor_ir = atof(env);      // experiments only
-  d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap, deg_floor_ir);
+  d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap, d->opt.deg_floor_ir);
 
   // ---- term trees -> unique pieces (geoms) and nodes ----
   Builder B(*d);
