@@ -17,6 +17,8 @@ import sys
 import threading
 import time
 
+import numpy as np
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
@@ -37,6 +39,8 @@ def parse():
     ap.add_argument("--ref-graphs", type=int, default=3, help="graphs of the workload the oracle is timed on, spread over the set")
     ap.add_argument("--no-second-policy", action="store_true", help="skip the timed step under the purely relative precision policy (w_abs_tol = 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of Eq.(1) (default: the library's, 1.0)")
+    ap.add_argument("--deg-floor-ir", type=float, default=None, help="Deg on the soft-photon sets (default: the library's, 0.25)")
     return ap.parse_args()
 
 
@@ -143,7 +147,7 @@ def run_ours(args):
     G, B = len(graphs), args.batch
     # ---- prepare (not timed as throughput; reported) ----
     t0 = time.perf_counter()
-    diagrams = [mc.Diagram(g[0], g[1], g[2]) for _, g in graphs]
+    diagrams = [mc.Diagram(g[0], g[1], g[2], deg_floor=args.deg_floor, deg_floor_ir=args.deg_floor_ir) for _, g in graphs]
     prepare_s = time.perf_counter() - t0
     infos = [d.info() for d in diagrams]
     flop = [i["flop_per_sample"] for i in infos]
@@ -247,6 +251,22 @@ def run_ours(args):
                                            "points_per_step": float(c[0].sum()) / args.steps,
                                            "note": "double-double: one algorithmic flop costs 5-6 binary64 instructions (pair arithmetic), so frac is bounded by ~0.18"},
                             "k_batch_qd": {"ms_per_step": ms_qd / args.steps, "points_per_step": n_qd / args.steps}}}
+    # ---- is the variance estimate itself trustworthy? sigma*sqrt(N) of the sum must not depend on N; a few more steps outside
+    #      the timed region, with a snapshot after each (heavy-tailed weights show up as a growing sigma*sqrt(N)) ----
+    keep2 = (sums.clone(), cnts.clone())
+    trace = []
+    for k in range(max(2, args.steps)):
+        step()
+        torch.cuda.synchronize()
+        nn = n_tot + (k + 1) * B
+        sk = sums.cpu().numpy()
+        mk = sk[0] / nn
+        trace.append(float(math.sqrt(float((np.maximum(sk[1] / nn - mk * mk, 0.0) / nn).sum()) * nn)))
+    first_s = math.sqrt(var_sum * n_tot)
+    tail = {"sigma_sqrtN_after_timed_steps": first_s, "sigma_sqrtN_with_more_steps": trace,
+            "variance_unreliable": bool(max(trace + [first_s]) > 1.25 * min(trace + [first_s])),
+            "note": "sigma*sqrt(N per graph) of the sum of estimates; it is constant in N when the variance estimate has converged"}
+    sums.copy_(keep2[0]); cnts.copy_(keep2[1])
     # ---- the same step under the purely relative precision policy (w_abs_tol = 0: north_star's literal reading, a point is
     #      accepted in binary64 only if its relative round-off bound holds), one warm-up + one timed step ----
     second = None
@@ -311,7 +331,7 @@ def run_ours(args):
                        "n_graphs": G, "batch": B, "seed": seed, "second_policy": second,
                        "headline_policy": "relative OR absolute acceptance (w_abs_tol = 1e-10 on the weight f/p; DESIGN.md section 6)", "l2": "tables of 256 diagrams (%.0f MB) exceed the 126 MB L2; no per-sample input is read" % (sum(i["table_bytes"] for i in infos) / 1e6),
                        "prepare_s": prepare_s, "flagged_fraction": flagged_frac, "precision": precision, "dropped": int(c[1].sum()),
-                       "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum),
+                       "sigma2_time_s": var_sum * ms * 1e-3, "sum_of_estimates": float((s[0] / n_tot).sum()), "sigma": math.sqrt(var_sum), "tail": tail,
                        "algorithmic_flop_per_sample_mean": sum(flop) / G, "classes": classes},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -66,23 +66,39 @@ __device__ __forceinline__ double mq_fma(double a, double b, double c) { return 
 // nothing downstream may assume an ordering (two_sum, never quick_two_sum, on values that come from here).
 // Error <= ~2^-103 (|a b| + |c|): the bound is relative to the operands, which is all a renormalising a*b + c gives
 // after a cancellation as well; the evaluator renormalises once per family (mq_norm in account()).
+// Error-free sum of two binary64 numbers in 3 FP64 instructions instead of 6 (MQ_DD_FAST2SUM = 1): FastTwoSum is exact when
+// exponent(x) >= exponent(y); the operands are ordered by comparing their high words without the sign with INTEGER compare and
+// selects, which run on the ALU pipe. MEASURED AND REJECTED on B200 (32 graphs of configs[4]): k_batch_dd 204 -> 236 ms. The
+// kernel is at 73 % FP64 pipe activity but the ordering adds 7 ALU instructions to the dependency chain of every sum, and two
+// warps per scheduler cannot hide it. Kept behind the switch for the record; default 0 = Knuth's branch-free two_sum.
+#ifndef MQ_DD_FAST2SUM
+#define MQ_DD_FAST2SUM 0
+#endif
+__device__ __forceinline__ dd dd_two_sum_ord(double a, double b) {
+#if MQ_DD_FAST2SUM
+  const bool sw = (unsigned)(__double2hiint(a) & 0x7fffffff) < (unsigned)(__double2hiint(b) & 0x7fffffff);
+  const double x = sw ? b : a, y = sw ? a : b;
+  const double s = __dadd_rn(x, y);
+  return dd(s, __dadd_rn(y, -__dadd_rn(s, -x)));
+#else
+  return dd_two_sum(a, b);
+#endif
+}
 __device__ __forceinline__ dd mq_fma(dd a, dd b, dd c) {
   const double p = __dmul_rn(a.hi, b.hi);
   double e = __fma_rn(a.hi, b.hi, -p);
   e = __fma_rn(a.hi, b.lo, e);
   e = __fma_rn(a.lo, b.hi, e);
-  const double s = __dadd_rn(p, c.hi), v = __dadd_rn(s, -p);
-  const double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c.hi, -v));
-  return dd(s, __dadd_rn(__dadd_rn(e, c.lo), t));
+  const dd st = dd_two_sum_ord(p, c.hi);
+  return dd(st.hi, __dadd_rn(__dadd_rn(e, c.lo), st.lo));
 }
 __device__ __forceinline__ double mq_fma_c(double coef, double x, double c0, double) { return fma(coef, x, c0); }   // coef*x + c0
 __device__ __forceinline__ dd mq_fma_c(double coef, dd x, double c0, dd) {   // coef*x + c0, coef and c0 binary64 (exact table entries); 10 flops
   const double p = __dmul_rn(coef, x.hi);
   double e = __fma_rn(coef, x.hi, -p);
   e = __fma_rn(coef, x.lo, e);
-  const double s = __dadd_rn(p, c0), v = __dadd_rn(s, -p);
-  const double t = __dadd_rn(__dadd_rn(p, -__dadd_rn(s, -v)), __dadd_rn(c0, -v));
-  return dd(s, __dadd_rn(t, e));
+  const dd st = dd_two_sum_ord(p, c0);
+  return dd(st.hi, __dadd_rn(st.lo, e));
 }
 // product of two pairs without renormalisation (5 flops); same remark as mq_fma
 __device__ __forceinline__ dd mq_mul(dd a, dd b) {

@@ -453,3 +453,23 @@ def test_three_loop_full_size_soft_pin(mc):
     b.close()
     for d in ds:
         d.close()
+
+
+def test_estimates_independent_of_deg_on_three_loop_graphs(mc):
+    """P11 on the GPU: Deg only shapes the density, so two different Deg tables (the default two floors
+    and the single floor 0.75 of round 1, with a cap) must give estimates that agree within their combined error, graph by graph"""
+    from paper_1905_08007_b200 import workloads
+    st = torch.cuda.current_stream().cuda_stream
+    gs = [workloads.all_graphs(3)[i] for i in (0, 8, 18, 29, 38, 47)]
+    n = 2_000_000
+    res = []
+    for kw in ({}, {"deg_floor": 0.75, "deg_cap": 2.0}):
+        ds = [mc.Diagram(*g, **kw) for g in gs]
+        s1, s2, nf, nd = mc.Batch(ds, 1 << 20).integrate_host(0, n, 3, st)
+        assert not nd.any()
+        mean = s1 / n
+        res.append((mean, np.sqrt(np.maximum(s2 / n - mean * mean, 0.0) / n)))
+        for d in ds:
+            d.close()
+    pull = (res[0][0] - res[1][0]) / np.hypot(res[0][1], res[1][1])
+    assert np.all(np.abs(pull) < 4.0) and np.sqrt((pull ** 2).mean()) < 2.0, pull
