@@ -14,28 +14,38 @@ namespace mqk {
 using FT = std::conditional<NP_F64 == 4, pt4, std::conditional<NP_F64 == 2, pt2, double>::type>::type;
 using FM = MagOf<FT>::type;
 constexpr int NP = PtsOf<FT>::n;
-// DISTK: the MQ_WL lanes of a point group carry NP = MQ_WL points; lane role k draws point k and computes its scalars in plain
-// binary64 (no redundant work across the lane roles); role 0 (the owner) gathers densities and flags with shuffles
+// DISTK: the MQ_WL lanes of a point group carry NP = MQ_WL points; lane role k draws point k, computes its scalars and assembles
+// its nodes and terms in plain binary64, and FINALISES it (precision decision, weight, sums): outside the family evaluation the
+// kernel is "one point per lane" with no redundant work across the lane roles. Otherwise lane role 0 (the owner) finalises
+// all NP points of its group.
 constexpr bool DISTK = NP > 1 && NP == MQ_WL;
-constexpr int PPW = 32 / MQ_WL;                        // point groups per warp; role k of a group sits PPW * k lanes after role 0
+constexpr int NF = DISTK ? 1 : NP;                     // points finalised by one lane
 
-// this lane's part of the draw and the owner's view of it: p[k], bad[k] of the NP points of the group
-struct GroupDraw { double p[NP]; bool bad[NP]; };
-template <bool WANT_ORDER>
-__device__ __forceinline__ void draw_group(const DiagView &v, uint64_t first, uint64_t i0, uint64_t n, uint64_t seed, int sub, FM *z, double *zl, int32_t *ord, GroupDraw &gd) {
+// the points this lane finalises after the evaluation: sample index (relative), density, hard flag, value, magnitude, amin, xmin
+struct LanePts {
+  uint64_t idx[NF]; double p[NF], f[NF], a[NF], amin[NF], xmin[NF]; bool bad[NF], live[NF];
+};
+// draws the lane's point(s) (a1-a3) and runs the evaluator (a4-a6). CTA-collective.
+template <bool WANT_ORDER, int W, class RO>
+__device__ __forceinline__ void eval_group(const DiagView &v, StreamReader &rd, const RO &ro, uint64_t first, uint64_t i0, uint64_t n, uint64_t seed,
+                                           const double *z_in, double *zl, int32_t *ord, FM *z, LanePts &lp) {
   const int M = v.h->M;
   if constexpr (DISTK) {
-    const uint64_t im = i0 + (uint64_t)sub;
-    const double pl = draw_point<WANT_ORDER>(v, first + (im < n ? im : n - 1), seed, zl, ord);
-    const bool badl = bad_point(zl, M, pl);
-    const int l0 = (threadIdx.x & 31) % PPW;
-#pragma unroll
-    for (int k = 0; k < NP; k++) { gd.p[k] = __shfl_sync(0xffffffffu, pl, l0 + k * PPW); gd.bad[k] = __shfl_sync(0xffffffffu, (int)badl, l0 + k * PPW) != 0; }
+    const uint64_t im = i0 + (uint64_t)ro.sub, ic = im < n ? im : n - 1;          // surplus slots redo the last point
+    if (z_in) { for (int j = 0; j < MQ_MAXM; j++) zl[j] = j < M ? z_in[ic * M + j] : 0.0; lp.p[0] = 1.0; lp.bad[0] = false; }
+    else { lp.p[0] = draw_point<WANT_ORDER>(v, first + ic, seed, zl, ord); lp.bad[0] = bad_point(zl, M, lp.p[0]); }
+    lp.idx[0] = im; lp.live[0] = im < n;
   } else {
-    draw_points<FT, WANT_ORDER>(v, first, i0, n, seed, z, gd.p, ord);
+    if (z_in) {
+      for (int k = 0; k < NP; k++) { const uint64_t i = i0 + k < n ? i0 + k : n - 1; for (int j = 0; j < MQ_MAXM; j++) mq_setc(z[j], k, j < M ? z_in[i * M + j] : 0.0); lp.p[k] = 1.0; }
+    } else draw_points<FT, WANT_ORDER>(v, first, i0, n, seed, z, lp.p, ord);
 #pragma unroll
-    for (int k = 0; k < NP; k++) gd.bad[k] = bad_point(z, k, M, gd.p[k]);
+    for (int k = 0; k < NP; k++) { lp.idx[k] = i0 + k; lp.live[k] = i0 + k < n && ro.sub == 0; lp.bad[k] = z_in ? false : bad_point(z, k, M, lp.p[k]); }
   }
+  FT f, a; FM amin, xmin;
+  eval_integrand<FT, W, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
+#pragma unroll
+  for (int k = 0; k < NF; k++) { lp.f[k] = mq_comp(f, k); lp.a[k] = mq_comp(a, k); lp.amin[k] = mq_comp(amin, k); lp.xmin[k] = mq_comp(xmin, k); }
 }
 
 // a1-a7 in binary64. Flagged points are appended to flag_list (sample index) and not accumulated here.
@@ -47,24 +57,19 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_integrate_f64(const ui
   const Roles<FT, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
   StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(FT));
   KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
-  // the evaluator is CTA-collective (it stages the table stream through shared memory and splits the families of a
-  // point group over W warps): every thread of the CTA runs the same number of iterations; slots past the end
-  // re-evaluate the last point and discard it; only the owner warp (gw = 0) of a group draws and accumulates
+  // the evaluator is CTA-collective (it stages the table stream through shared memory): every thread of the CTA runs the same
+  // number of iterations; slots past the end re-evaluate the last point and discard it
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; GroupDraw gd;
-    draw_group<false>(v, first, i0, n, seed, ro.sub, z, zl, nullptr, gd);
-    FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if (ro.gw != 0 || ro.sub != 0) continue;
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; LanePts lp;
+    eval_group<false, W_F64>(v, rd, ro, first, i0, n, seed, nullptr, zl, nullptr, z, lp);
 #pragma unroll
-    for (int k = 0; k < NP; k++) {
-      if (i0 + k >= n) continue;
-      const double fk = mq_comp(f, k);
-      const bool flag = tier_decision(gd.bad[k], fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), gd.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
-      if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + i0 + k; }
-      else { const double w = fk / gd.p[k]; s1.add(w); s2.add(w * w); }
+    for (int k = 0; k < NF; k++) {
+      if (!lp.live[k]) continue;
+      const bool flag = tier_decision(lp.bad[k], lp.f[k], lp.a[k], lp.amin[k], lp.xmin[k], lp.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+      if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + lp.idx[k]; }
+      else { const double w = lp.f[k] / lp.p[k]; s1.add(w); s2.add(w * w); }
     }
   }
   block_reduce_store(s1, s2, partial);
@@ -101,33 +106,19 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_points(const uint64_t *__rest
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; int32_t ord[(DISTK ? 1 : NP) * MQ_MAXM]; GroupDraw gd;
-    draw_group<true>(v, first, i0, n, seed, ro.sub, z, zl, ord, gd);
-    FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if constexpr (DISTK) {                           // every lane role writes the coordinates of the point it drew
-      const uint64_t i = i0 + (uint64_t)ro.sub;
-      if (i < n) {
-        if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = zl[j];
-        if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[j];
-      }
-    }
-    if (ro.gw != 0 || ro.sub != 0) continue;
-    for (int k = 0; k < NP; k++) {
-      const uint64_t i = i0 + k;
-      if (i >= n) continue;
-      const double fk = mq_comp(f, k);
-      const double *p = gd.p;
-      const int dec = tier_decision(gd.bad[k], fk, mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; int32_t ord[NF * MQ_MAXM]; LanePts lp;
+    eval_group<true, W_F64>(v, rd, ro, first, i0, n, seed, nullptr, zl, ord, z, lp);
+    for (int k = 0; k < NF; k++) {
+      if (!lp.live[k]) continue;
+      const uint64_t i = lp.idx[k];
+      const int dec = tier_decision(lp.bad[k], lp.f[k], lp.a[k], lp.amin[k], lp.xmin[k], lp.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol);
       const bool flag = dec == 1;
-      if constexpr (!DISTK) {
-        if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = mq_comp(z[j], k);
-        if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[k * MQ_MAXM + j];
-      }
-      if (p_out) p_out[i] = p[k];
-      if (f_out) f_out[i] = fk;
-      if (f64_out) f64_out[i] = fk;
-      if (cond_out) cond_out[i] = mq_comp(a, k) / fabs(fk);
+      if (z_out) for (int j = 0; j < M; j++) z_out[i * M + j] = DISTK ? zl[j] : mq_comp(z[DISTK ? 0 : j], k);
+      if (order_out) for (int j = 0; j < M; j++) order_out[i * M + j] = ord[k * MQ_MAXM + j];
+      if (p_out) p_out[i] = lp.p[k];
+      if (f_out) f_out[i] = lp.f[k];
+      if (f64_out) f64_out[i] = lp.f[k];
+      if (cond_out) cond_out[i] = lp.a[k] / fabs(lp.f[k]);
       if (flag_out) flag_out[i] = (uint8_t)dec;      // 0 accepted (relative), 1 re-evaluated in double-double, 2 accepted by the absolute bound on w
       if (flag && flag_list) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = i; }
     }
@@ -138,31 +129,19 @@ __global__ void __launch_bounds__(TPB_EVAL) k_eval_z_f64(const uint64_t *__restr
                                                          double *f64_out, double *cond_out, double *aux_out) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
-  const int M = v.h->M;
   const Roles<FT, W_F64, MQ_WL> ro(smem_raw, v.h->max_scal_len);
   StreamReader rd; setup_reader<W_F64, MQ_WL>(rd, smem_raw, v.h->max_scal_len, sizeof(FT));
   const uint64_t per = (uint64_t)ro.P * NP;
   for (uint64_t base = (uint64_t)blockIdx.x * per; base < n; base += (uint64_t)gridDim.x * per) {
     const uint64_t i0 = base + (uint64_t)ro.slot * NP;
-    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1];
-    if constexpr (DISTK) {
-      const uint64_t i = i0 + ro.sub < n ? i0 + ro.sub : n - 1;               // surplus slots redo the last point
-      for (int j = 0; j < MQ_MAXM; j++) zl[j] = j < M ? z_in[i * M + j] : 0.0;
-    } else {
-      for (int k = 0; k < NP; k++) {
-        const uint64_t i = i0 + k < n ? i0 + k : n - 1;
-        for (int j = 0; j < MQ_MAXM; j++) mq_setc(z[j], k, j < M ? z_in[i * M + j] : 0.0);
-      }
-    }
-    FT f, a; FM amin, xmin;
-    eval_integrand<FT, W_F64, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, ro.gw, ro.sub, f, a, amin, xmin);
-    if (ro.gw != 0 || ro.sub != 0) continue;
-    for (int k = 0; k < NP; k++) {
-      const uint64_t i = i0 + k;
-      if (i >= n) continue;
-      if (f64_out) f64_out[i] = mq_comp(f, k);
-      if (cond_out) cond_out[i] = mq_comp(a, k) / fabs(mq_comp(f, k));
-      if (aux_out) { aux_out[2 * i] = mq_comp(amin, k); aux_out[2 * i + 1] = mq_comp(xmin, k); }
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; LanePts lp;
+    eval_group<false, W_F64>(v, rd, ro, 0, i0, n, 0, z_in, zl, nullptr, z, lp);
+    for (int k = 0; k < NF; k++) {
+      if (!lp.live[k]) continue;
+      const uint64_t i = lp.idx[k];
+      if (f64_out) f64_out[i] = lp.f[k];
+      if (cond_out) cond_out[i] = lp.a[k] / fabs(lp.f[k]);
+      if (aux_out) { aux_out[2 * i] = lp.amin[k]; aux_out[2 * i + 1] = lp.xmin[k]; }
     }
   }
 }
@@ -190,17 +169,13 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     MqPrec pr = bv.dg[d].pr;
     if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
     const uint64_t i0 = (uint64_t)b * PTS_F64 + (uint64_t)ro.slot * NP;
-    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; GroupDraw gd;
-    draw_group<false>(v, first, i0, n, seed, ro.sub, z, zl, nullptr, gd);
-    const double *p = gd.p;
-    FT f, a; FM amin, xmin;
-    eval_integrand<FT, 1, true>(v, rd, z, zl, ro.S, ro.P, ro.xT, ro.xA, 0, ro.sub, f, a, amin, xmin);
-    // flagged points of the item, compacted in (lane, point) order = ascending sample index
-    bool flag[NP]; unsigned bal[NP]; unsigned mine = 0, wsum = 0;
+    FM z[DISTK ? 1 : MQ_MAXM]; double zl[DISTK ? MQ_MAXM : 1]; LanePts lp;
+    eval_group<false, 1>(v, rd, ro, first, i0, n, seed, nullptr, zl, nullptr, z, lp);
+    // flagged points of the item, compacted in (warp, lane, point) order: a deterministic list
+    bool flag[NF]; unsigned bal[NF]; unsigned mine = 0, wsum = 0;
 #pragma unroll
-    for (int k = 0; k < NP; k++) {
-      const bool live = i0 + k < n && ro.sub == 0;
-      flag[k] = live && tier_decision(gd.bad[k], mq_comp(f, k), mq_comp(a, k), mq_comp(amin, k), mq_comp(xmin, k), p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
+    for (int k = 0; k < NF; k++) {
+      flag[k] = lp.live[k] && tier_decision(lp.bad[k], lp.f[k], lp.a[k], lp.amin[k], lp.xmin[k], lp.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
       bal[k] = __ballot_sync(0xffffffffu, flag[k]);
       mine += __popc(bal[k] & ((1u << lane) - 1u)); wsum += __popc(bal[k]);
     }
@@ -212,9 +187,9 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     KahanPair s1{0.0, 0.0}, s2{0.0, 0.0};
     unsigned pos = before + mine;
 #pragma unroll
-    for (int k = 0; k < NP; k++) {
-      if (flag[k]) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + pos++] = (uint32_t)(i0 + k);
-      else if (i0 + k < n && ro.sub == 0) { const double w = mq_comp(f, k) / p[k]; s1.add(w); s2.add(w * w); }
+    for (int k = 0; k < NF; k++) {
+      if (flag[k]) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + pos++] = (uint32_t)lp.idx[k];
+      else if (lp.live[k]) { const double w = lp.f[k] / lp.p[k]; s1.add(w); s2.add(w * w); }
     }
     if (threadIdx.x == 0) bv.item_cnt[(size_t)d * (bv.cap / PTS_F64) + b] = all;
     block_reduce_to(s1, s2, bv.part_f64 + (size_t)item * 4);

@@ -702,9 +702,13 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   constexpr bool DIST = LANES && !SPREAD && NPT > 1 && NPT == MQ_WL;
   StreamReader rd = rd_io;                             // work on a register copy (the caller's object lives in local memory across this call)
   const DevHeader &h = *v.h;
-  T nodeval[MQ_MAXNODEVAL];
-  M nodeabs[TRACK ? MQ_MAXNODEVAL : 1];
-  T nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
+  // node values: per lane. DIST: lane role k assembles the nodes and terms of point k in plain binary64 (TT = MM = double), so
+  // the four roles share that work too and the per-thread arrays are binary64; otherwise the owner lane does all points
+  using TT = typename std::conditional<DIST, double, T>::type;
+  using MM = typename std::conditional<DIST, double, M>::type;
+  TT nodeval[MQ_MAXNODEVAL];
+  MM nodeabs[TRACK ? MQ_MAXNODEVAL : 1];
+  TT nodeU[MQ_MAXNODE], nodeV[MQ_MAXNODE];
   M amin(1.0), xmin(1.0);
   double amin_l = 1.0, xmin_l = 1.0;                   // DIST: of this lane's point
   const bool owner = gw == 0 && sub == 0 && (!SPREAD || threadIdx.x == 0);   // the lane whose f_out is used
@@ -715,17 +719,9 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
     T U = T(1.0), V = T(0.0), G = T(1.0); M Rp(1.0);
     if constexpr (LANES) __syncwarp();                 // every lane role has finished reading S of the previous piece
     if constexpr (SPREAD) __syncthreads();             // (entry-parallel) nobody still reads S of the previous piece
-    if constexpr (DIST) {
-      double Ul, Vl, Gl, Rl;
-      piece_scalars<double>(g, zl, SComp<NPT>(S, stride, sub), true, Ul, Vl, Gl, Rl, amin_l, xmin_l);
-      const int l0 = (threadIdx.x & 31) % (32 / MQ_WL);          // lane of role 0 of this point group; role k sits at l0 + k * (32 / MQ_WL)
-#pragma unroll
-      for (int k = 0; k < NPT; k++) {
-        const int src = l0 + k * (32 / MQ_WL);
-        mq_setc(U, k, __shfl_sync(0xffffffffu, Ul, src)); mq_setc(V, k, __shfl_sync(0xffffffffu, Vl, src));
-        mq_setc(G, k, __shfl_sync(0xffffffffu, Gl, src)); mq_setc(Rp, k, __shfl_sync(0xffffffffu, Rl, src));
-      }
-    } else piece_scalars<T>(g, z, SWhole<T>{S, stride}, SPREAD ? threadIdx.x == 0 : sub == 0, U, V, G, Rp, amin, xmin);
+    double Ul = 1.0, Vl = 0.0, Gl = 1.0, Rl = 1.0;              // DIST: U, V, G, Rp of this lane's point
+    if constexpr (DIST) piece_scalars<double>(g, zl, SComp<NPT>(S, stride, sub), true, Ul, Vl, Gl, Rl, amin_l, xmin_l);
+    else piece_scalars<T>(g, z, SWhole<T>{S, stride}, SPREAD ? threadIdx.x == 0 : sub == 0, U, V, G, Rp, amin, xmin);
     if constexpr (SPREAD) __syncthreads();              // S of this piece is complete before any warp gathers from it
     else if constexpr (LANES) __syncwarp();
     const int npat = 1 << g.nS;
@@ -807,7 +803,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
             }
           }
       }
-      if constexpr (!SPREAD) {                         // the families' magnitudes leave out prod max(1,|r_inner|) <= Rp
+      if constexpr (!SPREAD && !DIST) {                // the families' magnitudes leave out prod max(1,|r_inner|) <= Rp (DIST: applied at the assembly)
         for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) Na[o][p][c] = Na[o][p][c] * Rp;
@@ -818,28 +814,32 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
 #pragma unroll
           for (int c = 0; c < MQ_NGRADE; c++) { N[0][p][c] = N[0][p][c] * i12; if constexpr (TRACK) Na[0][p][c] = Na[0][p][c] * M(1.0 / 12.0); }
       }
-      // nodes that use this table: combine with the children's graded values. Only the owner lane of a point does this
-      // (the other lane role holds the same totals: doing it twice would only double the local-memory traffic)
-      if (owner)
+      // nodes that use this table: combine with the children's graded values. DIST: every lane role does it for its own point
+      // (component `sub` of the totals, binary64); otherwise only the owner lane of a point (the other roles hold the same totals)
+      auto nval = [&](const T &x) -> TT { if constexpr (DIST) return mq_comp(x, sub); else return x; };
+      auto naval = [&](const M &x) -> MM { if constexpr (DIST) return mq_comp(x, sub) * Rl; else return x; };
+      TT Uq, Vq, Gq;
+      if constexpr (DIST) { Uq = Ul; Vq = Vl; Gq = Gl; } else { Uq = U; Vq = V; Gq = G; }
+      if (DIST || owner)
       for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {
         const DevNode &nd = v.node[ni];
-        T Up = U, Vs = V;
+        TT Up = Uq, Vs = Vq;
         for (int k = 0; k < nd.nchild; k++) { Up = Up * nodeU[nd.child[k]]; Vs = Vs + nodeV[nd.child[k]]; }
         nodeU[ni] = Up; nodeV[ni] = Vs;
         for (int o = 0; o < nd.nout; o++) {
-          T tot[MQ_NGRADE]; M tota[MQ_NGRADE];
+          TT tot[MQ_NGRADE]; MM tota[MQ_NGRADE];
 #pragma unroll
-          for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = T(0.0); tota[c] = M(0.0); }
+          for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = TT(0.0); tota[c] = MM(0.0); }
           for (int p = 0; p < npat; p++) {
-            T acc[MQ_NGRADE]; M acca[MQ_NGRADE];
+            TT acc[MQ_NGRADE]; MM acca[MQ_NGRADE];
 #pragma unroll
-            for (int c = 0; c < MQ_NGRADE; c++) { acc[c] = N[o][p][c] * G; if constexpr (TRACK) acca[c] = Na[o][p][c] * mq_mag(G); }
+            for (int c = 0; c < MQ_NGRADE; c++) { acc[c] = nval(N[o][p][c]) * Gq; if constexpr (TRACK) acca[c] = naval(Na[o][p][c]) * mq_mag(Gq); }
             for (int k = 0; k < nd.nchild; k++) {
               const DevNode &ch = v.node[nd.child[k]];
               const int pb = g.child_patbit[k];
               const int which = (pb >= 0 && (p >> pb & 1)) ? 1 : 0;      // S-child: a (0) or b (1); V-child: its single value
-              graded_mul<T>(acc, &nodeval[ch.val_off + which * ch.ngr], ch.ngr);
-              if constexpr (TRACK) graded_mul<M>(acca, &nodeabs[ch.val_off + which * ch.ngr], ch.ngr);
+              graded_mul<TT>(acc, &nodeval[ch.val_off + which * ch.ngr], ch.ngr);
+              if constexpr (TRACK) graded_mul<MM>(acca, &nodeabs[ch.val_off + which * ch.ngr], ch.ngr);
             }
 #pragma unroll
             for (int c = 0; c < MQ_NGRADE; c++) { tot[c] = tot[c] + acc[c]; if constexpr (TRACK) tota[c] += acca[c]; }
@@ -851,32 +851,27 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   }
   // a6: terms.  f = sum sign * sum_{c<L} (L-c-1)! N_c / (Uprod^2 Vsum^(L-c))
   const int L = h.L;
-  T f = T(0.0), asum = T(0.0);
-  if (owner)
+  TT f = TT(0.0), asum = TT(0.0);
+  if (DIST || owner)
   for (int t = 0; t < h.nterm; t++) {
     const DevTerm tm = v.term[t];
     const DevNode &nd = v.node[tm.root];
-    const T U2 = nodeU[tm.root] * nodeU[tm.root], Vs = nodeV[tm.root];
-    T Vp = T(1.0);
+    const TT U2 = nodeU[tm.root] * nodeU[tm.root], Vs = nodeV[tm.root];
+    TT Vp = TT(1.0);
     double fact = 1.0;
     for (int c = L - 1; c >= 0; c--) {
       Vp = Vp * Vs;
       if (L - c - 1 > 0) fact *= (double)(L - c - 1);
-      const T scale = T(fact * (double)tm.sign) / (U2 * Vp);
-      const T contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : T(0.0)) * scale;
+      const TT scale = TT(fact * (double)tm.sign) / (U2 * Vp);
+      const TT contrib = (c < nd.ngr ? nodeval[nd.val_off + c] : TT(0.0)) * scale;
       f = f + contrib;
-      if constexpr (TRACK) asum = asum + T(c < nd.ngr ? nodeabs[nd.val_off + c] * mq_absd(mq_mag(scale)) : M(0.0));
+      if constexpr (TRACK) asum = asum + TT(c < nd.ngr ? nodeabs[nd.val_off + c] * mq_absd(mq_mag(scale)) : MM(0.0));
       else asum = asum + mq_abs(contrib);
     }
   }
-  if constexpr (DIST) {
-    const int l0 = (threadIdx.x & 31) % (32 / MQ_WL);
-#pragma unroll
-    for (int k = 0; k < NPT; k++) {
-      mq_setc(amin, k, __shfl_sync(0xffffffffu, amin_l, l0 + k * (32 / MQ_WL))); mq_setc(xmin, k, __shfl_sync(0xffffffffu, xmin_l, l0 + k * (32 / MQ_WL)));
-    }
-  }
-  f_out = f; abs_out = asum; amin_out = amin; xmin_out = xmin;
+  // DIST: every lane returns the values of ITS point (broadcast into all components of the outputs)
+  if constexpr (DIST) { f_out = T(f); abs_out = T(asum); amin_out = M(amin_l); xmin_out = M(xmin_l); rd_io = rd; return; }
+  if constexpr (!DIST) { f_out = f; abs_out = asum; amin_out = amin; xmin_out = xmin; }
   rd_io = rd;
 }
 

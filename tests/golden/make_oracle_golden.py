@@ -44,7 +44,7 @@ def three_loop(n):
 def high_loop(L, indices, n, seed, first):
     """per-point oracle values at L=4,5 (the oracle's table build takes minutes per graph at L=5):
     sample index range, seed and, per point, the binary128 value rounded to binary64 (hex) and the binary64 value"""
-    lines = ["# Oracle per-point integrand values, loop order %d, points first_sample=%d..+%d of seed %d, default Deg (floor 1.0, 0.25 on the soft-photon sets: DESIGN.md S5)." % (L, first, n, seed),
+    lines = ["# Oracle per-point integrand values, loop order %d, points first_sample=%d..+%d of seed %d, default Deg (floor 0.75, 0.5 on the soft-photon sets: DESIGN.md S5)." % (L, first, n, seed),
              "# Written by make_oracle_golden.py (oracle only). Values of L>=4 graphs are 'parity unpinned' by the paper (DESIGN.md section 3).",
              "# graph_index point fwide(hex) f64(hex)"]
     for idx in indices:
