@@ -322,7 +322,7 @@ def run_ours(args):
         cts = torch.bincount(fl.long(), minlength=3).cpu().numpy()
         mix = [mix[i] + int(cts[i]) for i in range(3)]
     mixn = float(sum(mix))
-    precision = {"cond_max": 3e4, "amin_min": 1e-2, "w_abs_tol": 1e-10, "dd_cond_max": 1e26,
+    precision = {"cond_max": 2.8e4, "amin_min": 1e-2, "w_abs_tol": 1e-10, "dd_cond_max": 1e26,
                  "sample_mix": {"accepted_relative": mix[0] / mixn, "reevaluated_dd": mix[1] / mixn, "accepted_absolute": mix[2] / mixn, "points": int(mixn)}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

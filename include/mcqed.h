@@ -60,7 +60,7 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {0.75, 1e30, 3e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
+/* NULL => defaults {0.75, 1e30, 2.8e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
  * value of Deg on the sets whose I-closure is the whole graph, the soft-photon sets (<= 0: same as deg_floor).
  * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
  *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.
@@ -106,13 +106,14 @@ int mc_diagram_set_flags(mc_diagram *, uint32_t flags);
  * the paper gives no thresholds). Every tier carries next to f a running bound a on the sum of |monomial| (it sees the
  * cancellation between terms, pieces, families, pairings and inside a coefficient block), amin = the smallest |A_t| and
  * xmin = the smallest pivot ratio / g_t of the point. A tier's value is ACCEPTED if
- *   (relative) a <= cond * |f| and min(amin, xmin) >= inner_min, with (cond, inner_min) = (cond_max, amin_min) in binary64
- *              (then |df| <= 1e-10 |f|) and (dd_cond_max, 1/dd_cond_max) in double-double, or
+ *   (relative) a <= cond * |f| * min(1, amin, xmin) and min(amin, xmin) >= inner_min, with (cond, inner_min) = (cond_max, amin_min)
+ *              in binary64 (cond_max = 2.8e4 = 1e-10 / unit: the round-off model unit * a / min(1, amin, xmin) is below 1e-10 |f|)
+ *              and (dd_cond_max, 1/dd_cond_max) in double-double, or
  *   (absolute) unit * a <= w_abs_tol * p * min(1, xmin), unit = 32 ulp of the tier's arithmetic (64 in double-double): the
  *              round-off bound on the WEIGHT w = f/p is below w_abs_tol. The Monte Carlo sums need absolute accuracy of the
  *              weights; deep in the corners of the simplex the subtracted integrand loses all relative precision while f/p
  *              is 1e-20 and smaller.
- * Otherwise the point goes to the next tier (binary64 -> double-double -> quad-double). Defaults: cond_max = 3e4, amin_min =
+ * Otherwise the point goes to the next tier (binary64 -> double-double -> quad-double). Defaults: cond_max = 2.8e4, amin_min =
  * 1e-2 (mc_options); dd_cond_max = 1e26; w_abs_tol = 1e-10 (0 switches the absolute criterion off). A batch copies the
  * values when it is created. HOST. MC_EINVAL on cond_max <= 0, dd_cond_max < 1, w_abs_tol < 0. */
 int mc_diagram_set_precision(mc_diagram *, double cond_max, double amin_min, double dd_cond_max, double w_abs_tol);
@@ -214,6 +215,14 @@ int mc_eval_z(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_str
 /* Integrand at caller-supplied points in the third precision tier (quad-double, ~212 bits), rounded to binary64.
  * DEVICE z_in n*M, DEVICE fqd_out n. */
 int mc_eval_z_qd(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream, double *fqd_out);
+
+/* Integrand at caller-supplied points in binary64 INTERVAL arithmetic with directed rounding (the paper controls
+ * round-off by interval arithmetic): [lo_out[i], hi_out[i]] contains the true value of the subtracted integrand at the binary64
+ * coordinates z_in[i] (table coefficients are exact), whatever the cancellation between the terms; (-inf, +inf) when an interval
+ * division met 0. The width tells how much binary64 can be trusted at the point; the library's own precision decision uses the
+ * cheaper bound of mc_diagram_set_precision, this call is the rigorous cross-check (about the cost of a double-double evaluation).
+ * DEVICE z_in n*M, DEVICE lo_out, hi_out n. */
+int mc_eval_z_interval(const mc_diagram *, uint64_t n, const double *z_in, void *cuda_stream, double *lo_out, double *hi_out);
 
 /* Number of kernels this library has launched in the calling process (for gpu_launches in bench.py). */
 unsigned long long mc_kernel_launch_count(void);

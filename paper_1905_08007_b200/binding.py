@@ -18,7 +18,7 @@ FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 EXPORTS = [
     "mc_prepare_diagram", "mc_prepare_diagram_host", "mc_free_diagram", "mc_diagram_info", "mc_diagram_id",
     "mc_diagram_subgraphs", "mc_diagram_forests", "mc_diagram_terms", "mc_diagram_sampler_tables", "mc_diagram_blob", "mc_diagram_set_flags", "mc_diagram_set_precision",
-    "mc_integrate", "mc_integrate_host", "mc_integrate_static", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_integrate_counts", "mc_allocate_samples", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_kernel_launch_count", "mc_fp64_peak",
+    "mc_integrate", "mc_integrate_host", "mc_integrate_static", "mc_batch_create", "mc_batch_integrate", "mc_batch_integrate_host", "mc_batch_integrate_counts", "mc_allocate_samples", "mc_batch_free", "mc_eval_points", "mc_eval_z", "mc_eval_z_qd", "mc_eval_z_interval", "mc_kernel_launch_count", "mc_fp64_peak",
     "mc_strerror", "mc_version",
 ]
 
@@ -86,6 +86,7 @@ def lib():
         L.mc_eval_points.argtypes = [vp, u64, u64, u64, vp, vp, vp, vp, vp, vp, vp, vp]
         L.mc_eval_z.argtypes = [vp, u64, vp, vp, vp, vp, vp, vp]
         L.mc_eval_z_qd.argtypes = [vp, u64, vp, vp, vp]
+        L.mc_eval_z_interval.argtypes = [vp, u64, vp, vp, vp, vp]
         L.mc_kernel_launch_count.restype = C.c_ulonglong
         L.mc_fp64_peak.argtypes = [C.c_int, vp, dp, dp]
         L.mc_strerror.restype = C.c_char_p
@@ -122,7 +123,7 @@ def make_graph(loops, ext_pos, chords):
 class Diagram:
     """RAII handle around mc_diagram*"""
 
-    def __init__(self, loops, ext_pos, chords, deg_floor=None, deg_cap=1e30, cond_max=3e4, amin_min=1e-2, flags=0, host_only=False, forests=None, deg_floor_ir=None):
+    def __init__(self, loops, ext_pos, chords, deg_floor=None, deg_cap=1e30, cond_max=2.8e4, amin_min=1e-2, flags=0, host_only=False, forests=None, deg_floor_ir=None):
         """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (0.75, 0.5) (mc_options); a deg_floor given alone also is the value on
         the soft-photon sets"""
         self.loops, self.M = loops, 3 * loops
@@ -186,7 +187,7 @@ class Diagram:
     def set_flags(self, flags):
         _check(lib().mc_diagram_set_flags(self.h, flags), "mc_diagram_set_flags")
 
-    def set_precision(self, cond_max=3e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=1e-10):
+    def set_precision(self, cond_max=2.8e4, amin_min=1e-2, dd_cond_max=1e26, w_abs_tol=1e-10):
         _check(lib().mc_diagram_set_precision(self.h, cond_max, amin_min, dd_cond_max, w_abs_tol), "mc_diagram_set_precision")
 
     def blob(self):
@@ -217,6 +218,9 @@ class Diagram:
 
     def eval_z_qd(self, n, z_in, stream, fqd):
         _check(lib().mc_eval_z_qd(self.h, n, _ptr(z_in), _ptr(stream), _ptr(fqd)), "mc_eval_z_qd")
+
+    def eval_z_interval(self, n, z_in, stream, lo, hi):
+        _check(lib().mc_eval_z_interval(self.h, n, _ptr(z_in), _ptr(stream), _ptr(lo), _ptr(hi)), "mc_eval_z_interval")
 
     def eval_z(self, n, z_in, stream=None, f64=None, fdd=None, cond=None, aux=None):
         _check(lib().mc_eval_z(self.h, n, _ptr(z_in), _ptr(stream), _ptr(f64), _ptr(fdd), _ptr(cond), _ptr(aux)), "mc_eval_z")

@@ -26,6 +26,7 @@ UNITS = {  # object -> (compiler, source, dependencies)
     "kern_f64.o": ("nvcc", "kern_f64.cu", KERN),
     "kern_dd.o": ("nvcc", "kern_dd.cu", KERN),
     "kern_qd.o": ("nvcc", "kern_qd.cu", KERN + ["qd_arith.cuh"]),
+    "kern_iv.o": ("nvcc", "kern_iv.cu", KERN + ["iv_arith.cuh"]),
     "prep_kernel.o": ("nvcc", "prep_kernel.cu", ["device_layout.h"]),
 }
 

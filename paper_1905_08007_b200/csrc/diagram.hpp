@@ -127,6 +127,8 @@ void mq_launch_eval_points_dd(const mc_diagram *d, uint64_t first, uint64_t seed
 void mq_launch_eval_z_f64(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *f64_out, double *cond_out, double *aux_out, mq_stream st);
 void mq_launch_eval_z_dd(const mc_diagram *d, int grid, uint64_t n, const double *z_in, double *fdd_out, mq_stream st);
 int mq_fp64_peak(int iters, mq_stream st, double *flops, double *ms);
+// interval tier (kern_iv.cu): enclosure [lo, hi] of the integrand at given points
+int mq_launch_eval_z_iv(const mc_diagram *d, uint64_t n, const double *z_in, double *lo_out, double *hi_out, mq_stream st);
 // binary64 tier with the scratch in a file-scope device array (kern_f64.cu); allocates nothing
 int mq_static_integrate_f64(const mc_diagram *d, uint64_t first, uint64_t n, uint64_t seed, mqk::MqPrec pr,
                             double *out_sum, double *out_sumsq, unsigned long long *out_nflag, unsigned long long *out_ndrop, mq_stream st);

@@ -95,7 +95,8 @@ __device__ __forceinline__ void draw_points(const DiagView &v, uint64_t first, u
 // coefficient block x |pairing weight| x |scalar factors|, through the whole tree), amin = min |A_t| over the electron lines
 // of every piece, xmin = min over pieces of (pivot / diagonal of the loop-matrix elimination, g_t = 1 + A_t): the quantities
 // every operand is divided by. unit = 32 (binary64) / 64 (double-double) ulp of the tier's arithmetic.
-//   0: accepted, relative round-off bound met (a <= cond_max |f| and min(amin, xmin) >= inner_min): |df| <= 1e-10 |f| in tier 1
+//   0: accepted, relative round-off bound met (a <= cond_max |f| min(1, amin, xmin) and min(amin, xmin) >= inner_min): with
+//      cond_max = 2.8e4 = 1e-10 / unit in tier 1 this is unit * a / min(1, amin, xmin) <= 1e-10 |f|
 //   2: precision loss detected, but the absolute round-off bound on the WEIGHT w = f/p is below w_abs_tol: the
 //      Monte Carlo sums need absolute, not relative, accuracy of w (PAPER.md:91 controls the round-off error of the result)
 //   1: handed to the next tier
@@ -103,7 +104,10 @@ __device__ __forceinline__ void draw_points(const DiagView &v, uint64_t first, u
 #define MQ_UNIT_DD (64.0 * 0x1p-103)
 __device__ __forceinline__ int tier_decision(bool hard, double f, double a, double amin, double xmin, double p, double cond_max, double inner_min, double unit, double w_abs_tol) {
   if (hard || !isfinite(f) || !isfinite(a)) return 1;
-  if (a <= cond_max * fabs(f) && fmin(amin, xmin) >= inner_min) return 0;
+  // relative: the error model is unit * a / min(1, xmin, amin) (every operand of a slot is divided by g_t and the pivots, the scalar
+  // factors of insertion pieces are the A_t), so the divisor belongs INSIDE the bound; inner_min stays as a floor on it
+  const double inner = fmin(amin, xmin);
+  if (a <= cond_max * fabs(f) * fmin(1.0, inner) && inner >= inner_min) return 0;
   if (unit * a <= w_abs_tol * p * fmin(1.0, xmin)) return 2;
   return 1;
 }

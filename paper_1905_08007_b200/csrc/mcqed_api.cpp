@@ -216,6 +216,14 @@ int mc_eval_z_qd(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda
   return MC_OK;
 }
 
+int mc_eval_z_interval(const mc_diagram *d, uint64_t n, const double *z_in, void *cuda_stream, double *lo_out, double *hi_out) {
+  if (!d || !d->on_device || !z_in || !lo_out || !hi_out) return MC_EINVAL;
+  if (n == 0) return MC_OK;
+  if (mq_launch_eval_z_iv(d, n, z_in, lo_out, hi_out, (mq_stream)cuda_stream) != 0) return MC_ECUDA;
+  g_launches++;
+  return MC_OK;
+}
+
 // ---- batched path ----
 int mc_batch_create(const mc_diagram *const *diagrams, int32_t n_diagrams, uint64_t max_samples_per_call, mc_batch **out) {
   if (!diagrams || n_diagrams < 1 || !out || max_samples_per_call < 1 || max_samples_per_call > (1ull << 30)) return MC_EINVAL;
