@@ -141,6 +141,9 @@ template <class T, int W, int WLX> struct Roles {
 template <int W, int WLX> __device__ __forceinline__ void setup_reader(StreamReader &rd, unsigned char *smem, int scal_len, size_t elem) {
   const size_t s = smem_head_bytes(scal_len, blockDim.x, elem, W, WLX);
   rd.init(reinterpret_cast<uint64_t *>(smem + s), reinterpret_cast<uint64_t *>(smem + s + 2 * MQ_CHUNK_WORDS * 8));
+#if MQ_DEVICE_ASSERTS
+  rd.dbg_scal_len = scal_len;
+#endif
 }
 
 

@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_integrate_f64(const ui
     for (int k = 0; k < NF; k++) {
       if (!lp.live[k]) continue;
       const bool flag = tier_decision(lp.bad[k], lp.f[k], lp.a[k], lp.amin[k], lp.xmin[k], lp.p[k], pr.cond_max, pr.amin_min, MQ_UNIT_F64, pr.w_abs_tol) == 1;
-      if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); flag_list[slot] = first + lp.idx[k]; }
+      if (flag) { unsigned long long slot = atomicAdd(&counters[0], 1ull); MQ_DASSERT(slot < n); flag_list[slot] = first + lp.idx[k]; }
       else { const double w = lp.f[k] / lp.p[k]; s1.add(w); s2.add(w * w); }
     }
   }
@@ -165,7 +165,9 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     const int d = bv.f64_start ? batch_find(bv.f64_start, bv.nd, item) : (int)(item / bv.ipd);
     const uint32_t b = bv.f64_start ? item - bv.f64_start[d] : item % bv.ipd;
     const uint64_t first = batch_first(bv, d, first_u), n = batch_n(bv, d, n_u);
+    MQ_DASSERT(d >= 0 && d < bv.nd && (uint64_t)(b + 1) * PTS_F64 <= (uint64_t)bv.cap);       // the item's slice of the per-diagram lists
     const DiagView v = make_view(bv.dg[d].blob);
+    MQ_DASSERT(v.h->max_scal_len <= scal_len && v.h->wl == MQ_WL);
     MqPrec pr = bv.dg[d].pr;
     if (no_dd) { pr.cond_max = 1e300; pr.amin_min = -1.0; }
     const uint64_t i0 = (uint64_t)b * PTS_F64 + (uint64_t)ro.slot * NP;
@@ -188,7 +190,7 @@ __global__ void __launch_bounds__(TPB_F64, MQ_MINB_F64) k_batch_f64(BatchView bv
     unsigned pos = before + mine;
 #pragma unroll
     for (int k = 0; k < NF; k++) {
-      if (flag[k]) bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + pos++] = (uint32_t)lp.idx[k];
+      if (flag[k]) { MQ_DASSERT(pos < (unsigned)PTS_F64); bv.flag_raw[(size_t)d * bv.cap + (size_t)b * PTS_F64 + pos++] = (uint32_t)lp.idx[k]; }
       else if (lp.live[k]) { const double w = lp.f[k] / lp.p[k]; s1.add(w); s2.add(w * w); }
     }
     if (threadIdx.x == 0) bv.item_cnt[(size_t)d * (bv.cap / PTS_F64) + b] = all;
@@ -219,6 +221,7 @@ __global__ void __launch_bounds__(128) k_batch_compact(BatchView bv) {
       __syncthreads();
     }
     const unsigned o = s_base + sc[t] - c;
+    MQ_DASSERT(c <= (unsigned)PTS_F64 && (size_t)o + c <= (size_t)bv.cap);
     for (unsigned k = 0; k < c; k++) out[o + k] = raw[(size_t)b * PTS_F64 + k];
     __syncthreads();
     if (t == 127) s_base += sc[127];

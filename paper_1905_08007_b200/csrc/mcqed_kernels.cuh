@@ -17,6 +17,19 @@
 #include "pt2_arith.cuh"
 #include "device_layout.h"
 
+// Device-side bounds checks of the library's own (build with MCQED_DEFS=-DMQ_DEVICE_ASSERTS=1; compute-sanitizer is not
+// available on every pool). Every run-time index into shared memory, the per-thread arrays and the scratch lists is checked;
+// a violation prints its place and traps, which the host sees as a launch failure. Off (no code) in the normal build.
+#ifndef MQ_DEVICE_ASSERTS
+#define MQ_DEVICE_ASSERTS 0
+#endif
+#if MQ_DEVICE_ASSERTS
+#include <cstdio>
+#define MQ_DASSERT(c) do { if (!(c)) { printf("MQ_DASSERT %s:%d: %s (block %d thread %d)\n", __FILE__, __LINE__, #c, (int)blockIdx.x, (int)threadIdx.x); __trap(); } } while (0)
+#else
+#define MQ_DASSERT(c) ((void)0)
+#endif
+
 namespace mqk {
 
 // value types whose family code keeps the outer pairing levels (c >= 3) and the halves of a kd = 6 block in real loops:
@@ -174,6 +187,9 @@ template <int N> struct SAcc<ptn<N>> {
 // All methods are CTA-collective: every thread of the CTA calls them in the same order.
 struct StreamReader {
   const uint64_t *gsrc;   // first chunk in global memory
+#if MQ_DEVICE_ASSERTS
+  int dbg_scal_len;       // number of S indices of the point group (the bound of every index byte of the stream)
+#endif
   uint32_t s_buf;         // shared address of the two chunk buffers
   uint32_t s_bar;         // shared address of the two mbarriers
   int nchunks, chunk, pos;
@@ -508,10 +524,16 @@ __device__ __forceinline__ void run_loop(StreamReader &rd, int count, int sub, u
     const uint32_t idxw = (uint32_t)(hd >> 16 & 0xFFFF);
     if ((int)(hd & 7) == MQ_PAD_MARK) { pos += 1 + (int)idxw; continue; }
     const uint64_t hl = lds_u64(a0 + 8u * (uint32_t)sub);
+    MQ_DASSERT(pos >= 0 && pos + MQ_WL * (1 + (int)idxw) + (int)(hd >> 32 & 0xFFFF) <= MQ_CHUNK_WORDS);   // an entry never straddles a chunk
+    MQ_DASSERT((int)(hd & 7) == C && (int)(hd >> 3 & 7) == KD && (int)idxw * 8 >= NI + (int)(hl >> 10 & 15));
     const uint32_t sidx = a0 + 8u * MQ_WL + 8u * idxw * (uint32_t)sub;
     const uint64_t w0 = lds_u64(sidx), w1 = lds_u64(sidx + 8);
     const uint32_t scoef = a0 + 8u * MQ_WL * (1u + idxw) + (KD ? 16u : 8u) * (uint32_t)sub;
     const int keyk = (int)((hl & 7) | ((hl >> 6 & 15) << 3) | ((hl >> 14 & 1) << 7));
+    MQ_DASSERT((keyk & 7) < MQ_NGRADE && ((keyk >> 3) & 15) < MQ_MAXPAT && (keyk >> 7) < 2);
+#if MQ_DEVICE_ASSERTS
+    for (int j = 0; j < NI + (int)(hl >> 10 & 15); j++) MQ_DASSERT((int)lds_u8(sidx + j) < rd.dbg_scal_len);
+#endif
     if (keyk != key) {
       if (key >= 0) { N[key >> 7][(key >> 3) & 15][key & 7] = racc; Na[key >> 7][(key >> 3) & 15][key & 7] = racca; }
       key = keyk; racc = N[key >> 7][(key >> 3) & 15][key & 7]; racca = Na[key >> 7][(key >> 3) & 15][key & 7];
@@ -716,6 +738,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   rd.begin(v.blob + h.off_stream, (int)h.stream_chunks);
   for (int gi = 0; gi < h.ngeom; gi++) {
     const DevGeom &g = v.geom[gi];
+    MQ_DASSERT(g.scal_len <= h.max_scal_len && g.nslot <= MQ_MAXSLOT && g.nch <= MQ_MAXL && g.nS <= 4 && g.nchild <= MQ_MAXCHILD);
     T U = T(1.0), V = T(0.0), G = T(1.0); M Rp(1.0);
     if constexpr (LANES) __syncwarp();                 // every lane role has finished reading S of the previous piece
     if constexpr (SPREAD) __syncthreads();             // (entry-parallel) nobody still reads S of the previous piece
@@ -727,6 +750,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
     const int npat = 1 << g.nS;
     for (int ti = g.first_table; ti < g.first_table + g.ntable; ti++) {
       const DevTable &tb = v.tab[ti];
+      MQ_DASSERT(ti < h.ntable && tb.nout >= 1 && tb.nout <= 2 && npat <= MQ_MAXPAT && tb.geom == gi);
       T N[2][MQ_MAXPAT][MQ_NGRADE];
       M Na[TRACK ? 2 : 1][TRACK ? MQ_MAXPAT : 1][MQ_NGRADE];
       for (int o = 0; o < tb.nout; o++) for (int p = 0; p < npat; p++)
@@ -823,6 +847,8 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
       if (DIST || owner)
       for (int ni = tb.first_node; ni < tb.first_node + tb.nnode; ni++) {
         const DevNode &nd = v.node[ni];
+        MQ_DASSERT(ni < MQ_MAXNODE && ni < h.nnode && nd.ngr <= MQ_NGRADE && nd.nout <= tb.nout && nd.val_off >= 0 && nd.val_off + nd.nout * nd.ngr <= MQ_MAXNODEVAL);
+        for (int k = 0; k < nd.nchild; k++) MQ_DASSERT(nd.child[k] >= 0 && nd.child[k] < ni);      // children are assembled before their parent
         TT Up = Uq, Vs = Vq;
         for (int k = 0; k < nd.nchild; k++) { Up = Up * nodeU[nd.child[k]]; Vs = Vs + nodeV[nd.child[k]]; }
         nodeU[ni] = Up; nodeV[ni] = Vs;
@@ -855,6 +881,7 @@ __device__ __noinline__ void eval_integrand(const DiagView &v, StreamReader &rd_
   if (DIST || owner)
   for (int t = 0; t < h.nterm; t++) {
     const DevTerm tm = v.term[t];
+    MQ_DASSERT(tm.root >= 0 && tm.root < h.nnode && tm.root < MQ_MAXNODE);
     const DevNode &nd = v.node[tm.root];
     const TT U2 = nodeU[tm.root] * nodeU[tm.root], Vs = nodeV[tm.root];
     TT Vp = TT(1.0);
