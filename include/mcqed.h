@@ -65,7 +65,13 @@ typedef struct {
  * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
  *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.
  * flags bit 0: never run the double-double pass (only non-finite points are then flagged; they contribute 0).
- * flags bit 1: build no numerator tables (introspection of the combinatorics only; host handles). */
+ * flags bit 1: build no numerator tables (introspection of the combinatorics only; host handles).
+ * flags bit 2: the random stream is MRG32k3a (the generator of the paper's "Calc 1") instead of Philox4x32-10
+ *   (PAPER.md:94): the initial state is (1 + seed_lo mod (m-1), 1 + seed_hi mod (m-1), 12345) in both components, sample index i
+ *   of diagram id owns the 64 outputs from position (id * 2^38 + i) * 64 of the sequence, and uniform number r of the sample is
+ *   made from outputs 2r, 2r+1 with the 52-bit construction used for Philox (S1b). Calls with disjoint sample ranges stay
+ *   independent and additive. Fixed at prepare time (mc_diagram_set_flags cannot change it); sample indices must stay below 2^38
+ *   (MC_EINVAL beyond) and the diagram id below 2^20 (MC_ELIMIT). */
 typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; double deg_floor_ir; } mc_options;
 
 /* Host-side preparation of one diagram (not on the timed path): validates the graph, enumerates

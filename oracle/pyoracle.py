@@ -52,6 +52,13 @@ def lib():
         for f in ("oracle_det_log2", "oracle_det_exp2"):
             getattr(_lib, f).restype = C.c_double
             getattr(_lib, f).argtypes = [C.c_double]
+        _lib.oracle_sample_uniform_mrg.restype = C.c_double
+        _lib.oracle_sample_uniform_mrg.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_int]
+        _lib.oracle_mrg32k3a.restype = None
+        _lib.oracle_mrg32k3a.argtypes = [C.POINTER(C.c_uint64), C.c_uint64, C.c_int, C.POINTER(C.c_uint64)]
+        _lib.oracle_mrg_matpow.restype = None
+        _lib.oracle_mrg_matpow.argtypes = [C.c_int, C.c_int, C.c_uint64, C.POINTER(C.c_uint64)]
+        _lib.oracle_set_generator.argtypes = [C.c_void_p, C.c_int]
         _lib.oracle_prepare_diagram.argtypes = [C.POINTER(OracleGraph), C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         _lib.oracle_free_diagram.argtypes = [C.c_void_p]
     return _lib
@@ -115,6 +122,25 @@ def philox(ctr, key):
     return list(o)
 
 
+def mrg32k3a(state6, skip, nout):
+    """raw MRG32k3a outputs w_n (L'Ecuyer 1999) after skipping `skip` outputs from the six-word state"""
+    st = np.asarray(state6, dtype=np.uint64).copy()
+    out = np.zeros(nout, dtype=np.uint64)
+    lib().oracle_mrg32k3a(_p(st, C.c_uint64), C.c_uint64(skip), nout, _p(out, C.c_uint64))
+    return out
+
+
+def mrg_matpow(comp, e, mult=1):
+    """A_comp^(mult * 2^e) mod m_comp, 3x3"""
+    out = np.zeros(9, dtype=np.uint64)
+    lib().oracle_mrg_matpow(comp, e, C.c_uint64(mult), _p(out, C.c_uint64))
+    return out.reshape(3, 3)
+
+
+def sample_uniform_mrg(idx, diag, seed, r):
+    return lib().oracle_sample_uniform_mrg(C.c_uint64(idx), C.c_uint32(diag), C.c_uint64(seed), r)
+
+
 class Diagram:
     """One prepared diagram (combinatorics + sampler tables [+ integrand tables])."""
 
@@ -159,6 +185,10 @@ class Diagram:
         deg, Z, Cn = np.zeros(n), np.zeros(n), C.c_double()
         lib().oracle_get_sampler_tables(self.h, _p(deg, C.c_double), _p(Z, C.c_double), C.byref(Cn))
         return deg, Z, Cn.value
+
+    def set_generator(self, kind):
+        """0 = Philox4x32-10 (default), 1 = MRG32k3a (S1b)"""
+        assert lib().oracle_set_generator(self.h, kind) == 0
 
     def sample(self, first, n, seed):
         z, p, order = np.zeros((n, self.M)), np.zeros(n), np.zeros((n, self.M), np.int32)

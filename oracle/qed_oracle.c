@@ -280,6 +280,21 @@ int oracle_num_threads(void) {
 void oracle_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out) { philox4x32_10(ctr, key, out); }
 double oracle_u01(uint32_t x, uint32_t y) { return u01_from_words(x, y); }
 double oracle_sample_uniform(uint64_t idx, uint32_t diag, uint64_t seed, int r) { return sample_uniform(idx, diag, seed, r); }
+double oracle_sample_uniform_mrg(uint64_t idx, uint32_t diag, uint64_t seed, int r) { return sample_uniform_mrg(idx, diag, seed, r); }
+/* raw MRG32k3a: state6 = (x1_{n-3}, x1_{n-2}, x1_{n-1}, x2_{n-3}, x2_{n-2}, x2_{n-1}); skips `skip` outputs, then writes nout outputs w_n */
+void oracle_mrg32k3a(const uint64_t *state6, uint64_t skip, int nout, uint64_t *out) {
+  Mrg g; for (int i = 0; i < 3; i++) { g.s1[i] = state6[i]; g.s2[i] = state6[3 + i]; }
+  mrg_skip(&g, skip);
+  for (int i = 0; i < nout; i++) out[i] = mrg_next(&g);
+}
+/* A^(2^e * mult) mod m of component comp (0, 1), row-major into out9 */
+void oracle_mrg_matpow(int comp, int e, uint64_t mult, uint64_t *out9) {
+  uint64_t P[3][3], m = comp ? MRG_M2 : MRG_M1; mrg_matpow(comp, mult, P);
+  for (int i = 0; i < e; i++) mrg_matmul(P, P, m, P);
+  for (int i = 0; i < 9; i++) out9[i] = P[i / 3][i % 3];
+}
+/* generator of the sampler of an existing diagram: 0 = Philox4x32-10 (default), 1 = MRG32k3a */
+int oracle_set_generator(oracle_diagram *d, int kind) { if (kind < 0 || kind > 1) return -1; d->stab.rng = kind; return 0; }
 double oracle_det_pow(double u, double inv_deg) { return det_pow(u, inv_deg); }
 double oracle_det_log2(double u) { return det_log2(u); }
 double oracle_det_exp2(double y) { return det_exp2(y); }

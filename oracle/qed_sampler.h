@@ -5,7 +5,7 @@
  * on the sector z_{j_1} >= ... >= z_{j_M}; Deg(s) > 0 on proper non-empty subsets of lines
  * (PAPER.md:78). The paper does not print Deg ("quite complicated", two versions elsewhere);
  * DESIGN.md reading S5 is implemented here. Random stream: Philox4x32-10, the
- * public counter-based generator, written out by hand (S1).
+ * public counter-based generator, written out by hand (S1), or MRG32k3a (S1b).
  *
  * Bit-exactness contract (S2-S4): every floating-point operation below is a single
  * IEEE-754 binary64 add/mul/div in the order written; compile with -ffp-contract=off.
@@ -37,6 +37,72 @@ static double sample_uniform(uint64_t idx, uint32_t diag_id, uint64_t seed, int 
   uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, w[4];
   philox4x32_10(ctr, key, w);
   return (r & 1) ? u01_from_words(w[2], w[3]) : u01_from_words(w[0], w[1]);
+}
+
+/* ---------------- MRG32k3a ("Calc 1"; P. L'Ecuyer, Operations Research 47 (1999) 159, Table III) ----------------
+ * Two order-3 linear recurrences, m1 = 2^32 - 209, m2 = 2^32 - 22853:
+ *     x1_n = (1403580 x1_{n-2} -  810728 x1_{n-3}) mod m1,     x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod m2,
+ * output number n: w_n = (x1_n - x2_n) mod m1. The state holds (x_{n-3}, x_{n-2}, x_{n-1}) of both components.
+ * How the method uses it is a READING (S1b; the paper names the generator only): the initial state is
+ * (1 + seed_lo mod (m-1), 1 + seed_hi mod (m-1), 12345) in both components (seed_lo = seed_hi = 12344 gives L'Ecuyer's
+ * reference state, all 12345); sample idx (< 2^38) of diagram diag_id (< 2^20) owns the 64 outputs from position
+ * (diag_id * 2^38 + idx) * 64 on, and uniform number r of the sample is made from outputs 2r and 2r+1 of those, with the same
+ * 52-bit construction as for Philox. Positions are reached by plain skipping here: state_n = A^n state_0 with the 3x3 companion
+ * matrices, A^n by square-and-multiply at every call (slow, obviously right).
+ * Pins (tests/test_oracle_rng.py): the published jump matrices A^(2^76), A^(2^127) of both components (recurrences, moduli, matrix
+ * power), stepping = skipping. The output combination (x1 - x2) mod m1 and the seeding have no published number at hand: for
+ * them "parity unpinned" (restated with Python integers in the test only). */
+#define MRG_M1 4294967087ull
+#define MRG_M2 4294944443ull
+typedef struct { uint64_t s1[3], s2[3]; } Mrg;
+static uint64_t mrg_next(Mrg *g) {
+  uint64_t x1 = ((1403580ull * g->s1[1]) % MRG_M1 + ((MRG_M1 - 810728ull) * g->s1[0]) % MRG_M1) % MRG_M1;
+  uint64_t x2 = ((527612ull * g->s2[2]) % MRG_M2 + ((MRG_M2 - 1370589ull) * g->s2[0]) % MRG_M2) % MRG_M2;
+  g->s1[0] = g->s1[1]; g->s1[1] = g->s1[2]; g->s1[2] = x1;
+  g->s2[0] = g->s2[1]; g->s2[1] = g->s2[2]; g->s2[2] = x2;
+  return (x1 + MRG_M1 - x2) % MRG_M1;
+}
+static void mrg_matmul(const uint64_t A[3][3], const uint64_t B[3][3], uint64_t m, uint64_t out[3][3]) {
+  uint64_t T[3][3];
+  for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
+    uint64_t acc = 0;
+    for (int k = 0; k < 3; k++) acc = (acc + (A[i][k] * B[k][j]) % m) % m;     /* entries < 2^32: the products fit 64 bits */
+    T[i][j] = acc;
+  }
+  memcpy(out, T, sizeof T);
+}
+/* companion matrix of component comp (0, 1): (x_{n-3}, x_{n-2}, x_{n-1})^T -> (x_{n-2}, x_{n-1}, x_n)^T */
+static void mrg_companion(int comp, uint64_t A[3][3]) {
+  uint64_t A1[3][3] = {{0, 1, 0}, {0, 0, 1}, {MRG_M1 - 810728ull, 1403580ull, 0}};
+  uint64_t A2[3][3] = {{0, 1, 0}, {0, 0, 1}, {MRG_M2 - 1370589ull, 0, 527612ull}};
+  memcpy(A, comp ? A2 : A1, sizeof A1);
+}
+/* A^n mod m of component comp */
+static void mrg_matpow(int comp, uint64_t n, uint64_t out[3][3]) {
+  uint64_t m = comp ? MRG_M2 : MRG_M1, B[3][3], R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+  mrg_companion(comp, B);
+  for (; n; n >>= 1) { if (n & 1) mrg_matmul(B, R, m, R); mrg_matmul(B, B, m, B); }
+  memcpy(out, R, sizeof R);
+}
+static void mrg_skip(Mrg *g, uint64_t n) {
+  for (int comp = 0; comp < 2; comp++) {
+    uint64_t P[3][3], m = comp ? MRG_M2 : MRG_M1, *s = comp ? g->s2 : g->s1, t[3];
+    mrg_matpow(comp, n, P);
+    for (int i = 0; i < 3; i++) { t[i] = 0; for (int k = 0; k < 3; k++) t[i] = (t[i] + (P[i][k] * s[k]) % m) % m; }
+    for (int i = 0; i < 3; i++) s[i] = t[i];
+  }
+}
+static Mrg mrg_seed(uint64_t seed) {
+  uint64_t lo = (uint32_t)seed, hi = (uint32_t)(seed >> 32);
+  Mrg g = {{1 + lo % (MRG_M1 - 1), 1 + hi % (MRG_M1 - 1), 12345}, {1 + lo % (MRG_M2 - 1), 1 + hi % (MRG_M2 - 1), 12345}};
+  return g;
+}
+/* uniform number r of sample idx of diagram diag_id from the MRG32k3a stream */
+static double sample_uniform_mrg(uint64_t idx, uint32_t diag_id, uint64_t seed, int r) {
+  Mrg g = mrg_seed(seed);
+  mrg_skip(&g, (((uint64_t)diag_id << 38) + idx) * 64 + 2 * (uint64_t)r);
+  uint64_t a = mrg_next(&g), b = mrg_next(&g);
+  return u01_from_words((uint32_t)a, (uint32_t)b);
 }
 
 /* ---------------- deterministic pow: t = u^(1/Deg) = det_exp2(det_log2(u)*invDeg) ---------------- */
@@ -111,6 +177,7 @@ typedef struct {
   double *invdeg;  /* 1.0/deg */
   double *Z;       /* 2^M sector-sum table, Z[0]=1 */
   double C;        /* normalisation of Eq.(1) */
+  int rng;         /* 0 = Philox4x32-10, 1 = MRG32k3a (oracle_set_generator) */
 } SamplerTab;
 
 /* Deg(s) = clamp(|sbar| - |e(sbar)|/2 - 2 max_F sum_H loops_H(sbar∩H), floor, cap); sbar=full -> floor_ir: the sets whose I-closure
@@ -181,7 +248,7 @@ static double draw_point(const SamplerTab *tab, uint64_t idx, uint32_t diag_id, 
     int x = -1;
     if (l == M - 1) { x = __builtin_ctz(mask); }
     else {
-      double u = sample_uniform(idx, diag_id, seed, l);
+      double u = tab->rng ? sample_uniform_mrg(idx, diag_id, seed, l) : sample_uniform(idx, diag_id, seed, l);
       double total = 0.0;
       for (int y = 0; y < M; y++) if (mask >> y & 1) total = total + tab->Z[mask & ~(1u << y)];
       double target = u * total, cum = 0.0;
@@ -193,7 +260,7 @@ static double draw_point(const SamplerTab *tab, uint64_t idx, uint32_t diag_id, 
       if (x < 0) x = last;
     }
     if (l >= 1) {
-      double u = sample_uniform(idx, diag_id, seed, (M - 1) + (l - 1));
+      double u = tab->rng ? sample_uniform_mrg(idx, diag_id, seed, (M - 1) + (l - 1)) : sample_uniform(idx, diag_id, seed, (M - 1) + (l - 1));
       double t = det_pow(u, tab->invdeg[mask]);   /* mask = S_l before removing x */
       rl = rl * t; pu = pu * u;
     }

@@ -12,7 +12,7 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ELIMIT, MC_ETOOBIG = 0, -1, -2, -3, -4, -5
 STATIC_MAX_SAMPLES = 65536            # MC_STATIC_MAX_SAMPLES of include/mcqed.h
-FLAG_NO_DD, FLAG_NO_TABLES = 1, 2    # mc_options.flags
+FLAG_NO_DD, FLAG_NO_TABLES, FLAG_MRG32K3A = 1, 2, 4    # mc_options.flags
 FLAG_NO_QD = 2                        # mc_batch_integrate flags bit 1
 
 EXPORTS = [

@@ -83,6 +83,8 @@ struct DevHeader {
   double C, cond_max;
   int64_t off_Z, off_invdeg, off_geom, off_table, off_node, off_term, total_words;
   int64_t off_stream, stream_chunks;      // the family streams: stream_chunks chunks of MQ_CHUNK_WORDS words
+  int32_t rng, pad0;                      // 0 = Philox4x32-10, 1 = MRG32k3a (mc_options.flags bit 2)
+  int64_t off_mrg;                        // rng = 1: [2][64][9] uint32, the powers A^(2^k) mod m of the two companion matrices (row-major)
 };
 
 // Stream entry = MQ_WL families of the SAME shape (c, kd), evaluated side by side by the MQ_WL lanes that share a

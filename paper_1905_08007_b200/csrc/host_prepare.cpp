@@ -171,6 +171,31 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   H.off_table = off; off += words(sizeof(DevTable) * d->tables.size());
   H.off_node = off; off += words(sizeof(DevNode) * d->nodes.size());
   H.off_term = off; off += words(sizeof(DevTerm) * d->terms.size());
+  // MRG32k3a (mc_options.flags bit 2, S1b): the powers A^(2^k), k < 64, of the companion matrices of
+  // x1_n = (1403580 x1_{n-2} - 810728 x1_{n-3}) mod m1 and x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod m2, acting on
+  // (x_{n-3}, x_{n-2}, x_{n-1}); the kernels reach a sample's position in the sequence with one matrix-vector product per set bit
+  std::vector<uint32_t> mrg_pow;
+  if (d->opt.flags & 4u) {
+    if (d->id >= (1 << 20)) return MC_ELIMIT;
+    const uint64_t mod[2] = {4294967087ull, 4294944443ull};
+    mrg_pow.resize(2 * 64 * 9);
+    for (int comp = 0; comp < 2; comp++) {
+      const uint64_t m = mod[comp];
+      uint64_t A[3][3] = {{0, 1, 0}, {0, 0, 1}, {0, 0, 0}};
+      if (comp == 0) { A[2][0] = m - 810728ull; A[2][1] = 1403580ull; } else { A[2][0] = m - 1370589ull; A[2][2] = 527612ull; }
+      for (int k = 0; k < 64; k++) {
+        for (int i = 0; i < 9; i++) mrg_pow[(size_t)(comp * 64 + k) * 9 + i] = (uint32_t)A[i / 3][i % 3];
+        uint64_t Q[3][3];
+        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
+          uint64_t acc = 0;
+          for (int t = 0; t < 3; t++) acc = (acc + A[i][t] * A[t][j] % m) % m;
+          Q[i][j] = acc;
+        }
+        std::memcpy(A, Q, sizeof A);
+      }
+    }
+    H.rng = 1; H.off_mrg = off; off += words(sizeof(uint32_t) * mrg_pow.size());
+  }
   // streams: a sequence of entries of MQ_WL same-shape families (device_layout.h). The kernels stage the stream through
   // shared memory in chunks of MQ_CHUNK_WORDS (bulk async copies), so (i) the stream starts on a 16-byte boundary,
   // (ii) no entry straddles a chunk boundary (a PAD header, c = 7, fills the rest of a chunk), (iii) coefficients
@@ -280,6 +305,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   std::memcpy(d->blob.data() + H.off_table, d->tables.data(), sizeof(DevTable) * d->tables.size());
   std::memcpy(d->blob.data() + H.off_node, d->nodes.data(), sizeof(DevNode) * d->nodes.size());
   std::memcpy(d->blob.data() + H.off_term, d->terms.data(), sizeof(DevTerm) * d->terms.size());
+  if (!mrg_pow.empty()) std::memcpy(d->blob.data() + H.off_mrg, mrg_pow.data(), sizeof(uint32_t) * mrg_pow.size());
   if (!streams.empty()) std::memcpy(d->blob.data() + stream_base, streams.data(), sizeof(uint64_t) * streams.size());
   d->have_tables = !no_tables;
   *out = d.release();

@@ -116,9 +116,14 @@ int64_t mc_diagram_blob(const mc_diagram *d, uint64_t *out, int64_t cap) {
   return n;
 }
 
+// MRG32k3a stream (mc_options.flags bit 2): a sample owns 64 outputs of the sequence and a diagram 2^38 samples (S1b)
+static bool rng_range_ok(const mc_diagram *d, uint64_t first, uint64_t n) {
+  return !(d->opt.flags & 4u) || (first <= (1ull << 38) && n <= (1ull << 38) - first);
+}
+
 int mc_integrate(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
                  double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
-  if (!d || !d->on_device) return MC_EINVAL;
+  if (!d || !d->on_device || !rng_range_ok(d, first_sample, n_samples)) return MC_EINVAL;
   mq_stream st = (mq_stream)cuda_stream;
   const bool no_dd = d->opt.flags & 1u;
   for (uint64_t done = 0; done < n_samples; done += mqk::CHUNK) {
@@ -159,7 +164,7 @@ int mc_integrate_host(const mc_diagram *d, uint64_t first_sample, uint64_t n_sam
 
 int mc_integrate_static(const mc_diagram *d, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void *cuda_stream,
                         double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
-  if (!d || !d->on_device) return MC_EINVAL;
+  if (!d || !d->on_device || !rng_range_ok(d, first_sample, n_samples)) return MC_EINVAL;
   if (n_samples > (uint64_t)MC_STATIC_MAX_SAMPLES) return MC_ETOOBIG;       // the static flagged list has one slot per sample
   if (n_samples == 0) return MC_OK;
   if (mq_static_integrate_f64(d, first_sample, n_samples, seed, d->prec(true), out_sum, out_sumsq, out_n_flagged, out_n_dropped, (mq_stream)cuda_stream) != 0) return MC_ECUDA;
@@ -169,7 +174,7 @@ int mc_integrate_static(const mc_diagram *d, uint64_t first_sample, uint64_t n_s
 
 int mc_eval_points(const mc_diagram *d, uint64_t first_sample, uint64_t n, uint64_t seed, void *cuda_stream,
                    double *z_out, int32_t *order_out, double *p_out, double *f_out, double *f64_out, double *cond_out, uint8_t *flag_out) {
-  if (!d || !d->on_device) return MC_EINVAL;
+  if (!d || !d->on_device || !rng_range_ok(d, first_sample, n)) return MC_EINVAL;
   mq_stream st = (mq_stream)cuda_stream;
   const bool no_dd = d->opt.flags & 1u;
   const int M = d->g.M;
@@ -301,6 +306,7 @@ void batch_pass(mc_batch *b, const mqk::BatchView &v, uint64_t items, uint64_t f
 int mc_batch_integrate(mc_batch *b, uint64_t first_sample, uint64_t n_samples, uint64_t seed, uint32_t flags, void *cuda_stream,
                        double *out_sum, double *out_sumsq, unsigned long long *out_n_flagged, unsigned long long *out_n_dropped) {
   if (!b) return MC_EINVAL;
+  for (const mc_diagram *d : b->diags) if (!rng_range_ok(d, first_sample, n_samples)) return MC_EINVAL;
   mq_stream st = (mq_stream)cuda_stream;
   for (uint64_t done = 0; done < n_samples; done += b->cap) {
     const uint64_t n = std::min<uint64_t>(b->cap, n_samples - done);
@@ -318,7 +324,7 @@ int mc_batch_integrate_counts(mc_batch *b, const uint64_t *first_sample, const u
   cudaStream_t cst = (cudaStream_t)cuda_stream;
   const size_t nd = b->diags.size();
   uint64_t longest = 0;
-  for (size_t d = 0; d < nd; d++) longest = std::max(longest, n_samples[d]);
+  for (size_t d = 0; d < nd; d++) { longest = std::max(longest, n_samples[d]); if (!rng_range_ok(b->diags[d], first_sample[d], n_samples[d])) return MC_EINVAL; }
   std::vector<uint32_t> start(nd + 1), vn(nd);
   std::vector<uint64_t> vf(nd);
   for (uint64_t done = 0; done < longest; done += b->cap) {        // diagrams whose range is longer than the capacity take several passes

@@ -70,6 +70,55 @@ __device__ __forceinline__ double u01(uint32_t x, uint32_t y) {   // 52 random b
   return __dmul_rn(__dadd_rn(__dadd_rn(__dmul_rn((double)(x >> 6), 67108864.0), (double)(y >> 6)), 0.5), 1.0 / 4503599627370496.0);
 }
 
+// ------------------------------------------------------------------ a1': MRG32k3a ("Calc 1"; S1b)
+// x1_n = (1403580 x1_{n-2} - 810728 x1_{n-3}) mod m1, x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod m2, w_n = (x1_n - x2_n) mod m1,
+// m1 = 2^32 - 209, m2 = 2^32 - 22853. Used counter-style: sample idx of diagram id owns the 64 outputs from position
+// (id * 2^38 + idx) * 64 on; the position is reached with the stored powers A^(2^k) of the two companion matrices (pw: [2][64][9]
+// uint32 in the diagram blob, host_prepare.cpp), one 3x3 matrix-vector product mod m per set bit. Reduction mod 2^32 - c by folding
+// the high word twice (hi * c + lo), no division.
+#define MQ_MRG_M1 4294967087u
+#define MQ_MRG_M2 4294944443u
+template <uint32_t CC> __device__ __forceinline__ uint32_t mrg_red(uint64_t p) {      // p mod (2^32 - CC), any p < 2^64, CC < 2^15
+  p = (p >> 32) * CC + (p & 0xffffffffull);
+  p = (p >> 32) * CC + (p & 0xffffffffull);                                             // < 2^32 + 2^30
+  const uint64_t m = 4294967296ull - CC;
+  return (uint32_t)(p >= m ? p - m : p);
+}
+template <uint32_t CC> __device__ __forceinline__ uint32_t mrg_addmod(uint32_t a, uint32_t b) {
+  const uint64_t m = 4294967296ull - CC, t = (uint64_t)a + b;
+  return (uint32_t)(t >= m ? t - m : t);
+}
+template <uint32_t CC> __device__ __forceinline__ void mrg_matvec(const uint32_t *__restrict__ P, uint32_t s[3]) {
+  uint32_t t[3];
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+    uint32_t acc = mrg_red<CC>((uint64_t)__ldg(P + 3 * i) * s[0]);
+    acc = mrg_addmod<CC>(acc, mrg_red<CC>((uint64_t)__ldg(P + 3 * i + 1) * s[1]));
+    t[i] = mrg_addmod<CC>(acc, mrg_red<CC>((uint64_t)__ldg(P + 3 * i + 2) * s[2]));
+  }
+  s[0] = t[0]; s[1] = t[1]; s[2] = t[2];
+}
+// the first nu uniforms of the sample: uniform r from outputs 2r, 2r+1. Not inlined: it runs once per point, and its registers
+// stay out of the evaluator's allocation.
+static __device__ __noinline__ void mrg32k3a_uniforms(const uint32_t *__restrict__ pw, uint64_t seed, uint64_t skip, int nu, double *u) {
+  const uint32_t lo = (uint32_t)seed, hi = (uint32_t)(seed >> 32);
+  uint32_t s1[3] = {1u + lo % (MQ_MRG_M1 - 1u), 1u + hi % (MQ_MRG_M1 - 1u), 12345u};
+  uint32_t s2[3] = {1u + lo % (MQ_MRG_M2 - 1u), 1u + hi % (MQ_MRG_M2 - 1u), 12345u};
+  for (int k = 0; skip; k++, skip >>= 1)
+    if (skip & 1) { mrg_matvec<209u>(pw + 9 * k, s1); mrg_matvec<22853u>(pw + 9 * (64 + k), s2); }
+  uint32_t w[2];
+  for (int r = 0; r < nu; r++) {
+#pragma unroll
+    for (int j = 0; j < 2; j++) {
+      const uint32_t x1 = mrg_addmod<209u>(mrg_red<209u>(1403580ull * s1[1]), mrg_red<209u>((uint64_t)(MQ_MRG_M1 - 810728u) * s1[0]));
+      const uint32_t x2 = mrg_addmod<22853u>(mrg_red<22853u>(527612ull * s2[2]), mrg_red<22853u>((uint64_t)(MQ_MRG_M2 - 1370589u) * s2[0]));
+      s1[0] = s1[1]; s1[1] = s1[2]; s1[2] = x1; s2[0] = s2[1]; s2[1] = s2[2]; s2[2] = x2;
+      w[j] = x1 >= x2 ? x1 - x2 : x1 + (MQ_MRG_M1 - x2);       // (x1 - x2) mod m1 (x2 < m2 < m1)
+    }
+    u[r] = u01(w[0], w[1]);
+  }
+}
+
 // ------------------------------------------------------------------ a3: deterministic pow (S4)
 // explicit round-to-nearest mul/add only (never contracted) so that the bits equal the oracle's
 __device__ __forceinline__ double det_log2(double u) {
@@ -109,12 +158,15 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
   double r[MQ_MAXM]; int8_t ord[MQ_MAXM];
   double rl = 1.0, pu = 1.0;
   uint32_t ws[4], wr[4];
+  const bool mrg = v.h->rng != 0;                      // the same for every point of a launch: no divergence
+  double um[2 * MQ_MAXM];
+  if (mrg) mrg32k3a_uniforms(reinterpret_cast<const uint32_t *>(v.blob + v.h->off_mrg), seed, (((uint64_t)dg << 38) + idx) << 6, 2 * (M - 1), um);
   for (int l = 0; l < M; l++) {
     int x;
     if (l == M - 1) x = __ffs(mask) - 1;
     else {
-      if ((l & 1) == 0) philox4x32_10(i0, i1, (uint32_t)(l >> 1), dg, k0, k1, ws);
-      double u = (l & 1) ? u01(ws[2], ws[3]) : u01(ws[0], ws[1]);
+      if (!mrg && (l & 1) == 0) philox4x32_10(i0, i1, (uint32_t)(l >> 1), dg, k0, k1, ws);
+      double u = mrg ? um[l] : (l & 1) ? u01(ws[2], ws[3]) : u01(ws[0], ws[1]);
       double total = 0.0;
       for (uint32_t mm = mask; mm; mm &= mm - 1) { int y = __ffs(mm) - 1; total = __dadd_rn(total, __ldg(&v.Z[mask & ~(1u << y)])); }
       double target = __dmul_rn(u, total), cum = 0.0;
@@ -127,8 +179,8 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
     }
     if (l >= 1) {
       int ru = (M - 1) + (l - 1);
-      if ((ru & 1) == 0 || l == 1) philox4x32_10(i0, i1, (uint32_t)(ru >> 1), dg, k0, k1, wr);
-      double u = (ru & 1) ? u01(wr[2], wr[3]) : u01(wr[0], wr[1]);
+      if (!mrg && ((ru & 1) == 0 || l == 1)) philox4x32_10(i0, i1, (uint32_t)(ru >> 1), dg, k0, k1, wr);
+      double u = mrg ? um[ru] : (ru & 1) ? u01(wr[2], wr[3]) : u01(wr[0], wr[1]);
       double t = det_exp2(__dmul_rn(det_log2(u), __ldg(&v.invdeg[mask])));
       rl = __dmul_rn(rl, t); pu = __dmul_rn(pu, u);
     }

@@ -147,3 +147,23 @@ def test_oracle_wide_value_equals_exact_rational_value(po, mc, L, idx, npts):
     for k in range(npts):
         fe = float(b.integrand([Fr(float(v)) for v in z[k]]))
         assert abs(ref["fwide"][k] - fe) <= 2e-16 * abs(fe), (k, fe, ref["fwide"][k])
+
+
+def test_mrg32k3a_power_table_in_blob_equals_oracle(po, mc):
+    """mc_options.flags bit 2 (PAPER.md:93; DESIGN.md S1b): the blob carries A^(2^k) mod m, k < 64, of both companion matrices;
+    every entry against the oracle's own matrix power (pinned to the published A^(2^76) in test_oracle_rng.py). Without the flag
+    the blob has no such section."""
+    import blob_interp
+    d = mc.Diagram(2, 2, [(0, 4), (1, 3)], host_only=True, flags=mc.FLAG_MRG32K3A | mc.FLAG_NO_TABLES)
+    words = d.blob()
+    h = np.frombuffer(words.tobytes(), blob_interp.HDR, 1)[0]
+    assert h["rng"] == 1 and 0 < h["off_mrg"] and h["off_mrg"] + 576 <= h["off_stream"] and h["total_words"] == len(words)
+    tab = np.frombuffer(words.tobytes(), "<u4", 2 * 64 * 9, int(h["off_mrg"]) * 8).reshape(2, 64, 3, 3)
+    for comp in (0, 1):
+        for k in range(64):
+            assert np.array_equal(tab[comp, k].astype(np.uint64), po.mrg_matpow(comp, k)), (comp, k)
+    d.close()
+    d = mc.Diagram(2, 2, [(0, 4), (1, 3)], host_only=True, flags=mc.FLAG_NO_TABLES)
+    h = np.frombuffer(d.blob().tobytes(), blob_interp.HDR, 1)[0]
+    assert h["rng"] == 0 and h["off_mrg"] == 0
+    d.close()
