@@ -39,7 +39,7 @@ def parse():
     ap.add_argument("--ref-graphs", type=int, default=3, help="graphs of the workload the oracle is timed on, spread over the set")
     ap.add_argument("--no-second-policy", action="store_true", help="skip the timed step under the purely relative precision policy (w_abs_tol = 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of Eq.(1) (default: the library's, 0.75)")
+    ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of Eq.(1) (default: the library's, 1.0)")
     ap.add_argument("--deg-floor-ir", type=float, default=None, help="Deg on the soft-photon sets (default: the library's, 0.5)")
     return ap.parse_args()
 

@@ -60,7 +60,7 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {0.75, 1e30, 2.8e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
+/* NULL => defaults {1.0, 1e30, 2.8e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
  * value of Deg on the sets whose I-closure is the whole graph, the soft-photon sets (<= 0: same as deg_floor).
  * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
  *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.

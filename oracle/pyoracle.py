@@ -145,12 +145,12 @@ class Diagram:
     """One prepared diagram (combinatorics + sampler tables [+ integrand tables])."""
 
     def __init__(self, g, deg_floor=None, deg_cap=1e30, level=1, prune=1, deg_floor_ir=None):
-        """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (0.75, 0.5) (S5); a deg_floor given alone also is the value
+        """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (1.0, 0.5) (S5); a deg_floor given alone also is the value
         on the soft-photon sets (the one-floor reading of round 1)"""
         self.g = g
         self.h = C.c_void_p()
         if deg_floor is None:
-            deg_floor, deg_floor_ir = 0.75, (0.5 if deg_floor_ir is None else deg_floor_ir)
+            deg_floor, deg_floor_ir = 1.0, (0.5 if deg_floor_ir is None else deg_floor_ir)
         elif deg_floor_ir is None:
             deg_floor_ir = deg_floor
         rc = lib().oracle_prepare_diagram(C.byref(g), deg_floor, deg_cap, deg_floor_ir, level, prune, C.byref(self.h))

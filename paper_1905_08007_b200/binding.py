@@ -124,12 +124,12 @@ class Diagram:
     """RAII handle around mc_diagram*"""
 
     def __init__(self, loops, ext_pos, chords, deg_floor=None, deg_cap=1e30, cond_max=2.8e4, amin_min=1e-2, flags=0, host_only=False, forests=None, deg_floor_ir=None):
-        """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (0.75, 0.5) (mc_options); a deg_floor given alone also is the value on
+        """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (1.0, 0.5) (mc_options); a deg_floor given alone also is the value on
         the soft-photon sets"""
         self.loops, self.M = loops, 3 * loops
         g = make_graph(loops, ext_pos, chords)
         if deg_floor is None:
-            deg_floor, deg_floor_ir = 0.75, (0.5 if deg_floor_ir is None else deg_floor_ir)
+            deg_floor, deg_floor_ir = 1.0, (0.5 if deg_floor_ir is None else deg_floor_ir)
         elif deg_floor_ir is None:
             deg_floor_ir = deg_floor
         opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags, deg_floor_ir)

@@ -45,6 +45,7 @@ def main(argv=None):
     ap.add_argument("--mean-samples", type=int, default=16384, help="mean samples per graph in the main pass (budget = this x cost)")
     ap.add_argument("--chunk", type=int, default=384, help="graphs prepared and integrated together")
     ap.add_argument("--max-graphs", type=int, default=0, help="only the first N representatives (0 = all; for a quick look)")
+    ap.add_argument("--stride", type=int, default=1, help="every K-th representative only (a sample spread over the whole set)")
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of the UV-type sets (DESIGN.md S5; default: the library's)")
     ap.add_argument("--deg-floor-ir", type=float, default=None, help="Deg of the soft-photon sets (default: the library's)")
@@ -57,7 +58,7 @@ def main(argv=None):
     assert torch.cuda.is_available(), "campaign needs a CUDA device (no CPU fallback)"
     st = torch.cuda.current_stream().cuda_stream
     graphs = workloads.all_graphs(a.loops)
-    reps = representatives(graphs)
+    reps = representatives(graphs)[::max(1, a.stride)]
     if a.max_graphs:
         reps = reps[:a.max_graphs]
     G = len(reps)

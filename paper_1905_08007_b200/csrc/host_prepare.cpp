@@ -57,7 +57,7 @@ struct Builder {
 int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out) {
   if (!graph || !out) return MC_EINVAL;
   std::unique_ptr<mc_diagram> d(new mc_diagram);
-  d->opt = opts ? *opts : mc_options{0.75, 1e30, 2.8e4, 1e-2, 0u, 0.5};
+  d->opt = opts ? *opts : mc_options{1.0, 1e30, 2.8e4, 1e-2, 0u, 0.5};
   if (!(d->opt.deg_floor > 0) || !(d->opt.deg_cap >= d->opt.deg_floor) || !(d->opt.cond_max > 0)) return MC_EINVAL;
   if (!d->g.build(graph->loops, graph->ext_pos, graph->chord_a, graph->chord_b)) return MC_EINVAL;
   d->id = d->g.canonicalId();

@@ -36,7 +36,7 @@ def two_loop(n):
 def three_loop(n):
     _mc_all(3, n, 3, 0.75, os.path.join(HERE, "oracle_three_loop_mc.txt"),
             ["# Oracle Monte Carlo of all 50 3-loop graphs (BASELINE.json configs[2]), seed 3, first_sample 0, %d points per graph," % n,
-             "# default Deg (floor 0.75, no cap), oracle mode 0 (binary64 values: on graphs 0, 20, 45 the binary128 re-evaluation of mode 2",
+             "# Deg floor 0.75 on all clamped sets, no cap, oracle mode 0 (binary64 values: on graphs 0, 20, 45 the binary128 re-evaluation of mode 2",
              "# moves the mean by 1e-13, far below the statistical error, and costs 8x the time).  Written by make_oracle_golden.py (oracle only).",
              "# Soft pin: the literature value of the 3-loop contribution of graphs without lepton loops, 0.904979 (SURVEY.md P9; not in PAPER.md)."], mode=0)
 
@@ -44,7 +44,7 @@ def three_loop(n):
 def high_loop(L, indices, n, seed, first):
     """per-point oracle values at L=4,5 (the oracle's table build takes minutes per graph at L=5):
     sample index range, seed and, per point, the binary128 value rounded to binary64 (hex) and the binary64 value"""
-    lines = ["# Oracle per-point integrand values, loop order %d, points first_sample=%d..+%d of seed %d, default Deg (floor 0.75, 0.5 on the soft-photon sets: DESIGN.md S5)." % (L, first, n, seed),
+    lines = ["# Oracle per-point integrand values, loop order %d, points first_sample=%d..+%d of seed %d, default Deg (floor 1.0, 0.5 on the soft-photon sets: DESIGN.md S5)." % (L, first, n, seed),
              "# Written by make_oracle_golden.py (oracle only). Values of L>=4 graphs are 'parity unpinned' by the paper (DESIGN.md section 3).",
              "# graph_index point fwide(hex) f64(hex)"]
     for idx in indices:
