@@ -185,6 +185,9 @@ def test_five_loop_points_against_stored_oracle_values(po, mc):
     sys.path.insert(0, HERE)
     from blob_interp import Blob
     rows = read_golden("oracle_points_L5.txt")
+    import re
+    with open(os.path.join(HERE, "golden", "oracle_points_L5.txt")) as fh:      # the Deg floors the stored points were drawn with
+        dfl, dir_ = map(float, re.search(r"Deg \(floor ([0-9.]+), ([0-9.]+) on the soft-photon sets", fh.readline()).groups())
     gs = workloads.all_graphs(5)
     by_graph = {}
     for idx, k, fw, f64 in rows:
@@ -197,11 +200,11 @@ def test_five_loop_points_against_stored_oracle_values(po, mc):
     n_acc = n_acc_truth = 0
     for idx, pts in sorted(by_graph.items()):
         g = gs[idx]
-        d = mc.Diagram(g[0], g[1], g[2])
+        d = mc.Diagram(g[0], g[1], g[2], deg_floor=dfl, deg_floor_ir=dir_)
         assert d.id() == idx
         n = len(pts)
         r = _gpu_points(mc, d, 1000, n, 5)
-        o = po.Diagram(po.OracleGraph.make(*g), level=0)
+        o = po.Diagram(po.OracleGraph.make(*g), level=0, deg_floor=dfl, deg_floor_ir=dir_)
         zo, pz, oo = o.sample(1000, n, 5)
         assert np.array_equal(r["z"], zo) and np.array_equal(r["p"], pz) and np.array_equal(r["order"], oo), idx
         fw = np.array([p[1] for p in sorted(pts)])
