@@ -56,3 +56,24 @@ def test_batch_with_per_diagram_ranges_matches_per_diagram_calls():
     for j, d in enumerate(ds):
         r1, r2, _, _ = d.integrate_host(3, 500, 11, st)
         assert abs(h[0][j] - r1) <= 1e-12 * math.sqrt(500 * r2)
+
+
+def test_campaign_mirror_identification_matches_table_1(po):
+    """campaign.py runs ONE graph of every mirror pair and counts its estimate twice (PAPER.md:153 fn5): its host logic against the
+    paper's N_diag per class (tests/golden/paper_table1_ndiag.txt), the total 3213 and the
+    oracle's own mirror map; the multiplicities add up to all 6354 graphs. No GPU."""
+    from conftest import read_golden
+    from paper_1905_08007_b200 import campaign, workloads
+    graphs = workloads.all_graphs(5)
+    reps = campaign.representatives(graphs)
+    assert len(graphs) == 6354 and len(reps) == 3213 and sum(m for _, _, m in reps) == 6354
+    want = {(int(k), int(m), int(n)): int(c) for k, m, n, c in read_golden("paper_table1_ndiag.txt")}
+    got = {}
+    for _, g, _ in reps:
+        got[workloads.graph_class(g)] = got.get(workloads.graph_class(g), 0) + 1
+    assert got == want
+    og = po.all_graphs(5)
+    for i, g, m in reps[::97]:
+        mk = po.graph_mirror(og[i]).key()
+        assert campaign.mirror(g) == mk and (m == 1) == (mk == og[i].key())
+    assert len(campaign.representatives(graphs)[::8]) == 402          # the --stride 8 sample of DESIGN.md section 7
