@@ -45,6 +45,7 @@ def main(argv=None):
     ap.add_argument("--mean-samples", type=int, default=16384, help="mean samples per graph in the main pass (budget = this x cost)")
     ap.add_argument("--chunk", type=int, default=384, help="graphs prepared and integrated together")
     ap.add_argument("--max-graphs", type=int, default=0, help="only the first N representatives (0 = all; for a quick look)")
+    ap.add_argument("--cap", type=int, default=0, help="samples per graph and pass held by the batch scratch (0 = max(pilot, 4 x mean-samples); longer ranges take several passes)")
     ap.add_argument("--stride", type=int, default=1, help="every K-th representative only (a sample spread over the whole set)")
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of the UV-type sets (DESIGN.md S5; default: the library's)")
@@ -65,7 +66,7 @@ def main(argv=None):
     mean, err, n_used, cost, flagged = np.zeros(G), np.zeros(G), np.zeros(G), np.zeros(G), np.zeros(G)
     sig1 = np.zeros(G)
     t_prep = t_run = 0.0
-    cap = max(a.pilot, 4 * a.mean_samples)
+    cap = a.cap if a.cap > 0 else max(a.pilot, 4 * a.mean_samples)
     # per chunk: prepare once, pilot pass, allocation of the chunk's share of the budget (mean_samples x the chunk's cost: the
     # split between chunks stays equal-cost so that every chunk is prepared only once; inside a chunk of a few hundred graphs
     # the per-sample sigmas already span orders of magnitude), main pass on the sample indices after the pilot's
