@@ -12,8 +12,16 @@ namespace mqk {
 // condition number (or pivot / current loss) exceeds dd_cond_max (default 1e26: ~5 digits left) goes on to quad-double,
 // unless the absolute round-off bound on its weight is already below w_abs_tol (tier_decision, kern_common.cuh)
 
+// register budget of the double-double kernels: left to ptxas by default (it settles at 168 registers = 3 CTAs of 128 threads per SM);
+// MCQED_DEFS=-DMQ_MINB_DD=n forces n resident CTAs per SM (tuning builds)
+#ifdef MQ_MINB_DD
+#define MQ_DD_BOUNDS __launch_bounds__(TPB_DD, MQ_MINB_DD)
+#else
+#define MQ_DD_BOUNDS __launch_bounds__(TPB_DD)
+#endif
+
 // a8: double-double re-evaluation of the flagged points (dense lanes: one list entry per thread)
-__global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, MqPrec pr, double *partial,
+__global__ void MQ_DD_BOUNDS k_integrate_dd(const uint64_t *__restrict__ blob, uint64_t seed, MqPrec pr, double *partial,
                                                          const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
@@ -41,7 +49,7 @@ __global__ void __launch_bounds__(TPB_DD) k_integrate_dd(const uint64_t *__restr
 }
 
 // batched path, double-double tier: persistent CTAs; item = PTS_DD consecutive entries of one diagram's flagged list
-__global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
+__global__ void MQ_DD_BOUNDS k_batch_dd(BatchView bv, uint64_t first, uint64_t seed, int scal_len) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ unsigned s_item; __shared__ int s_d;
   const Roles<dd, W_DD, MQ_WL> ro(smem_raw, scal_len);
@@ -78,7 +86,7 @@ __global__ void __launch_bounds__(TPB_DD) k_batch_dd(BatchView bv, uint64_t firs
   }
 }
 
-__global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, MqPrec pr, double *f_out,
+__global__ void MQ_DD_BOUNDS k_eval_points_dd(const uint64_t *__restrict__ blob, uint64_t first, uint64_t seed, MqPrec pr, double *f_out,
                                                            const unsigned long long *flag_list, unsigned long long *lost_list, unsigned long long *counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
@@ -103,7 +111,7 @@ __global__ void __launch_bounds__(TPB_DD) k_eval_points_dd(const uint64_t *__res
   }
 }
 
-__global__ void __launch_bounds__(TPB_DD) k_eval_z_dd(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in, double *fdd_out) {
+__global__ void MQ_DD_BOUNDS k_eval_z_dd(const uint64_t *__restrict__ blob, uint64_t n, const double *__restrict__ z_in, double *fdd_out) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DiagView v = make_view(blob);
   const int M = v.h->M;
