@@ -60,7 +60,7 @@ typedef struct {
   int32_t n_forest; const uint32_t *forest_mask;
 } mc_forests;
 
-/* NULL => defaults {1.0, 1e30, 2.8e4, 1e-2, 0, 0.5}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
+/* NULL => defaults {1.0, 1e30, 2.8e4, 1e-2, 0, 0.5, 0, 0, 0}. deg_floor/deg_cap clamp Deg(s) of Eq.(1) (S5); deg_floor_ir is the
  * value of Deg on the sets whose I-closure is the whole graph, the soft-photon sets (<= 0: same as deg_floor).
  * cond_max, amin_min: thresholds of the relative acceptance test of the binary64 tier; the full precision policy
  *   (relative or absolute acceptance, three tiers) is stated at mc_diagram_set_precision.
@@ -72,7 +72,14 @@ typedef struct {
  *   made from outputs 2r, 2r+1 with the 52-bit construction used for Philox (S1b). Calls with disjoint sample ranges stay
  *   independent and additive. Fixed at prepare time (mc_diagram_set_flags cannot change it); sample indices must stay below 2^38
  *   (MC_EINVAL beyond) and the diagram id below 2^20 (MC_ELIMIT). */
-typedef struct { double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; double deg_floor_ir; } mc_options;
+typedef struct {
+  double deg_floor, deg_cap, cond_max, amin_min; uint32_t flags; double deg_floor_ir;
+  /* Defensive mixture (S5b; a READING: the paper has one density). mix_alpha in (0, 1): with
+   * probability mix_alpha (decided by uniform number 2(M-1) of the sample) the point is drawn from a SECOND Eq.(1) density built with
+   * the floors (deg_floor2, deg_floor_ir2; <= 0: same as deg_floor2) and the same cap, and the density every weight is divided by is
+   * (1 - mix_alpha) p_first(z) + mix_alpha p_second(z): a weight is bounded by the better of the two channels. 0 = off (default). */
+  double mix_alpha, deg_floor2, deg_floor_ir2;
+} mc_options;
 
 /* Host-side preparation of one diagram (not on the timed path): validates the graph, enumerates
  * subgraphs/forests/terms (forest-like formula, O1), builds Deg and the sector-sum table

@@ -59,6 +59,7 @@ def lib():
         _lib.oracle_mrg_matpow.restype = None
         _lib.oracle_mrg_matpow.argtypes = [C.c_int, C.c_int, C.c_uint64, C.POINTER(C.c_uint64)]
         _lib.oracle_set_generator.argtypes = [C.c_void_p, C.c_int]
+        _lib.oracle_set_mixture.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double]
         _lib.oracle_prepare_diagram.argtypes = [C.POINTER(OracleGraph), C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         _lib.oracle_free_diagram.argtypes = [C.c_void_p]
     return _lib
@@ -189,6 +190,10 @@ class Diagram:
     def set_generator(self, kind):
         """0 = Philox4x32-10 (default), 1 = MRG32k3a (S1b)"""
         assert lib().oracle_set_generator(self.h, kind) == 0
+
+    def set_mixture(self, alpha, deg_floor2, deg_floor_ir2=0.0, deg_cap2=1e30):
+        """defensive mixture (S5b): probability alpha of drawing from a second Eq.(1) density with these Deg floors"""
+        assert lib().oracle_set_mixture(self.h, alpha, deg_floor2, deg_cap2, deg_floor_ir2) == 0
 
     def sample(self, first, n, seed):
         z, p, order = np.zeros((n, self.M)), np.zeros(n), np.zeros((n, self.M), np.int32)

@@ -180,6 +180,7 @@ int oracle_prepare_diagram(const oracle_graph *og, double deg_floor, double deg_
 void oracle_free_diagram(oracle_diagram *d) {
   if (!d) return;
   for (int k = 0; k < d->ngeom; k++) for (int op = 0; op < 4; op++) if (d->geoms[k].tab[op]) { free(d->geoms[k].tab[op]->mono); free(d->geoms[k].tab[op]); }
+  if (d->stab.alt) { free_samplertab((SamplerTab *)d->stab.alt); free((void *)d->stab.alt); }
   free(d->geoms); free(d->nodes); free_samplertab(&d->stab); free(d);
 }
 /* info[0..7] = id, M, nsub, nforest, nterm, ngeom, nnode, n_monomials */
@@ -215,7 +216,7 @@ int oracle_sample_points(const oracle_diagram *d, uint64_t first, uint64_t n, ui
   return 0;
 }
 int oracle_density(const oracle_diagram *d, uint64_t n, const double *z, double *p) {
-  for (uint64_t i = 0; i < n; i++) p[i] = density_at(&d->stab, z + i * d->g.M);
+  for (uint64_t i = 0; i < n; i++) p[i] = density_mix_at(&d->stab, z + i * d->g.M);
   return 0;
 }
 /* integrand at given points. f64 / fwide (the wide value rounded to double) / abs64 (round-off scale) /
@@ -292,6 +293,19 @@ void oracle_mrg_matpow(int comp, int e, uint64_t mult, uint64_t *out9) {
   uint64_t P[3][3], m = comp ? MRG_M2 : MRG_M1; mrg_matpow(comp, mult, P);
   for (int i = 0; i < e; i++) mrg_matmul(P, P, m, P);
   for (int i = 0; i < 9; i++) out9[i] = P[i / 3][i % 3];
+}
+/* defensive mixture (S5b): with probability alpha a point is drawn from a second Eq.(1) density with the Deg floors
+ * (deg_floor2, deg_floor_ir2) and the same cap; alpha = 0 switches it off */
+int oracle_set_mixture(oracle_diagram *d, double alpha, double deg_floor2, double deg_cap2, double deg_floor_ir2) {
+  if (!(alpha >= 0.0 && alpha < 1.0)) return -1;
+  if (d->stab.alt) { free_samplertab((SamplerTab *)d->stab.alt); free((void *)d->stab.alt); d->stab.alt = NULL; }
+  d->stab.alpha = 0.0;
+  if (alpha == 0.0) return 0;
+  if (!(deg_floor2 > 0.0 && deg_cap2 >= deg_floor2)) return -1;
+  SamplerTab *t = (SamplerTab *)calloc(1, sizeof *t);
+  build_deg(&d->g, d->subs, d->nsub, d->forests, d->nforest, deg_floor2, deg_cap2, deg_floor_ir2 > 0 ? deg_floor_ir2 : deg_floor2, t);
+  d->stab.alt = t; d->stab.alpha = alpha;
+  return 0;
 }
 /* generator of the sampler of an existing diagram: 0 = Philox4x32-10 (default), 1 = MRG32k3a */
 int oracle_set_generator(oracle_diagram *d, int kind) { if (kind < 0 || kind > 1) return -1; d->stab.rng = kind; return 0; }

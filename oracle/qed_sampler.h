@@ -178,6 +178,10 @@ typedef struct {
   double *Z;       /* 2^M sector-sum table, Z[0]=1 */
   double C;        /* normalisation of Eq.(1) */
   int rng;         /* 0 = Philox4x32-10, 1 = MRG32k3a (oracle_set_generator) */
+  /* defensive mixture (S5b, a READING: the paper has one density): with probability alpha the
+   * point is drawn from the second Eq.(1) density `alt` (other Deg floors), and the density of the point is the mixture
+   * (1 - alpha) p_this + alpha p_alt, so that a weight f/p is bounded by the better of the two channels. NULL = off. */
+  const void *alt; double alpha;
 } SamplerTab;
 
 /* Deg(s) = clamp(|sbar| - |e(sbar)|/2 - 2 max_F sum_H loops_H(sbar∩H), floor, cap); sbar=full -> floor_ir: the sets whose I-closure
@@ -241,14 +245,20 @@ static void free_samplertab(SamplerTab *t) { free(t->deg); free(t->invdeg); free
 
 /* ---------------- one sample point (S3) ---------------- */
 /* out: z[M] (by line index), order[M] (j_1..j_M), returns p(z) */
-static double draw_point(const SamplerTab *tab, uint64_t idx, uint32_t diag_id, uint64_t seed, double *z, int *order) {
-  int M = tab->M; unsigned mask = (1u << M) - 1;
-  double r[MAXM], rl = 1.0, pu = 1.0;
+static double draw_point(const SamplerTab *tab0, uint64_t idx, uint32_t diag_id, uint64_t seed, double *z, int *order) {
+  int M = tab0->M; unsigned mask = (1u << M) - 1;
+  double r[MAXM], rl = 1.0, pu = 1.0, pq = 1.0;
+  /* mixture: uniform number 2(M-1) of the sample picks the channel; `tab` draws the point, `oth` only contributes its density */
+  const SamplerTab *tab = tab0, *oth = NULL;
+  if (tab0->alt) {
+    double uc = tab0->rng ? sample_uniform_mrg(idx, diag_id, seed, 2 * (M - 1)) : sample_uniform(idx, diag_id, seed, 2 * (M - 1));
+    if (uc < tab0->alpha) { tab = (const SamplerTab *)tab0->alt; oth = tab0; } else oth = (const SamplerTab *)tab0->alt;
+  }
   for (int l = 0; l < M; l++) {
     int x = -1;
     if (l == M - 1) { x = __builtin_ctz(mask); }
     else {
-      double u = tab->rng ? sample_uniform_mrg(idx, diag_id, seed, l) : sample_uniform(idx, diag_id, seed, l);
+      double u = tab0->rng ? sample_uniform_mrg(idx, diag_id, seed, l) : sample_uniform(idx, diag_id, seed, l);
       double total = 0.0;
       for (int y = 0; y < M; y++) if (mask >> y & 1) total = total + tab->Z[mask & ~(1u << y)];
       double target = u * total, cum = 0.0;
@@ -260,9 +270,11 @@ static double draw_point(const SamplerTab *tab, uint64_t idx, uint32_t diag_id, 
       if (x < 0) x = last;
     }
     if (l >= 1) {
-      double u = tab->rng ? sample_uniform_mrg(idx, diag_id, seed, (M - 1) + (l - 1)) : sample_uniform(idx, diag_id, seed, (M - 1) + (l - 1));
-      double t = det_pow(u, tab->invdeg[mask]);   /* mask = S_l before removing x */
+      double u = tab0->rng ? sample_uniform_mrg(idx, diag_id, seed, (M - 1) + (l - 1)) : sample_uniform(idx, diag_id, seed, (M - 1) + (l - 1));
+      double lg = det_log2(u) * tab->invdeg[mask];   /* mask = S_l before removing x; t = u^(1/Deg) = det_pow(u, invdeg) */
+      double t = det_exp2(lg);
       rl = rl * t; pu = pu * u;
+      if (oth) pq = pq * det_exp2(lg * oth->deg[mask]);   /* t^Deg_other: the other channel's factor of Eq.(1) at this point */
     }
     r[l] = rl; order[l] = x;
     mask &= ~(1u << x);
@@ -271,7 +283,11 @@ static double draw_point(const SamplerTab *tab, uint64_t idx, uint32_t diag_id, 
   for (int l = 0; l < M; l++) S = S + r[l];
   double pz = 1.0;
   for (int l = 0; l < M; l++) { double zz = r[l] / S; z[order[l]] = zz; pz = pz * zz; }
-  return (tab->C * pu) / pz;
+  double p_drawn = (tab->C * pu) / pz;
+  if (!oth) return p_drawn;
+  double p_other = (oth->C * pq) / pz;
+  double p_main = tab == tab0 ? p_drawn : p_other, p_alt = tab == tab0 ? p_other : p_drawn;
+  return (1.0 - tab0->alpha) * p_main + tab0->alpha * p_alt;
 }
 
 /* density of a given point (S6; tests only): sort descending, ties lower index first */
@@ -287,5 +303,10 @@ static double density_at(const SamplerTab *tab, const double *z) {
     mask &= ~(1u << ord[l]);
   }
   return exp(lp);
+}
+/* density the points are drawn with: Eq.(1), or the mixture of the two Eq.(1) densities */
+static double density_mix_at(const SamplerTab *tab, const double *z) {
+  if (!tab->alt) return density_at(tab, z);
+  return (1.0 - tab->alpha) * density_at(tab, z) + tab->alpha * density_at((const SamplerTab *)tab->alt, z);
 }
 #endif

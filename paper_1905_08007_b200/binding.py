@@ -34,7 +34,7 @@ class McForests(C.Structure):
 
 class McOptions(C.Structure):
     _fields_ = [("deg_floor", C.c_double), ("deg_cap", C.c_double), ("cond_max", C.c_double), ("amin_min", C.c_double), ("flags", C.c_uint32),
-                ("deg_floor_ir", C.c_double)]
+                ("deg_floor_ir", C.c_double), ("mix_alpha", C.c_double), ("deg_floor2", C.c_double), ("deg_floor_ir2", C.c_double)]
 
 
 class McError(RuntimeError):
@@ -123,16 +123,17 @@ def make_graph(loops, ext_pos, chords):
 class Diagram:
     """RAII handle around mc_diagram*"""
 
-    def __init__(self, loops, ext_pos, chords, deg_floor=None, deg_cap=1e30, cond_max=2.8e4, amin_min=1e-2, flags=0, host_only=False, forests=None, deg_floor_ir=None):
+    def __init__(self, loops, ext_pos, chords, deg_floor=None, deg_cap=1e30, cond_max=2.8e4, amin_min=1e-2, flags=0, host_only=False, forests=None, deg_floor_ir=None,
+                 mix_alpha=0.0, deg_floor2=0.0, deg_floor_ir2=0.0):
         """Deg of Eq.(1): defaults (deg_floor, deg_floor_ir) = (1.0, 0.5) (mc_options); a deg_floor given alone also is the value on
-        the soft-photon sets"""
+        the soft-photon sets. mix_alpha > 0: defensive mixture with a second Eq.(1) density of floors (deg_floor2, deg_floor_ir2)"""
         self.loops, self.M = loops, 3 * loops
         g = make_graph(loops, ext_pos, chords)
         if deg_floor is None:
             deg_floor, deg_floor_ir = 1.0, (0.5 if deg_floor_ir is None else deg_floor_ir)
         elif deg_floor_ir is None:
             deg_floor_ir = deg_floor
-        opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags, deg_floor_ir)
+        opt = McOptions(deg_floor, deg_cap, cond_max, amin_min, flags, deg_floor_ir, mix_alpha, deg_floor2, deg_floor_ir2)
         self.h = C.c_void_p()
         fo = None
         if forests is not None:

@@ -50,6 +50,7 @@ def main(argv=None):
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of the UV-type sets (DESIGN.md S5; default: the library's)")
     ap.add_argument("--deg-floor-ir", type=float, default=None, help="Deg of the soft-photon sets (default: the library's)")
+    ap.add_argument("--mix", type=float, nargs=3, default=None, metavar=("ALPHA", "FLOOR2", "FLOOR_IR2"), help="defensive mixture: probability and Deg floors of the second channel (DESIGN.md S5b)")
     ap.add_argument("--mrg32k3a", action="store_true", help="second random stream (mc_options.flags bit 2)")
     ap.add_argument("--out", default="")
     a = ap.parse_args(argv)
@@ -74,7 +75,8 @@ def main(argv=None):
     n_main = np.zeros(G, np.int64)
     for ids in chunks:
         t0 = time.perf_counter()
-        ds = [mc.Diagram(*reps[i][1], deg_floor=a.deg_floor, deg_floor_ir=a.deg_floor_ir, flags=mc.FLAG_MRG32K3A if a.mrg32k3a else 0) for i in ids]
+        ds = [mc.Diagram(*reps[i][1], deg_floor=a.deg_floor, deg_floor_ir=a.deg_floor_ir, flags=mc.FLAG_MRG32K3A if a.mrg32k3a else 0,
+                         **({} if a.mix is None else {"mix_alpha": a.mix[0], "deg_floor2": a.mix[1], "deg_floor_ir2": a.mix[2]})) for i in ids]
         t_prep += time.perf_counter() - t0
         for k, i in enumerate(ids):
             cost[i] = ds[k].info()["flop_per_sample"]
@@ -111,7 +113,7 @@ def main(argv=None):
     sig_ps = err * np.sqrt(n_used)
     n_eq = (a.pilot + a.mean_samples) * np.ones(G) * cost.mean() / cost          # equal COST per graph
     var_equal = float(((mult * sig_ps) ** 2 / np.maximum(n_eq, 1)).sum())
-    res = {"deg_floor": a.deg_floor, "deg_floor_ir": a.deg_floor_ir, "generator": "mrg32k3a" if a.mrg32k3a else "philox4x32_10", "loops": a.loops, "n_graphs_all": len(graphs), "n_mirror_identified": G, "pilot": a.pilot, "mean_samples": a.mean_samples, "seed": a.seed,
+    res = {"mix": a.mix, "deg_floor": a.deg_floor, "deg_floor_ir": a.deg_floor_ir, "generator": "mrg32k3a" if a.mrg32k3a else "philox4x32_10", "loops": a.loops, "n_graphs_all": len(graphs), "n_mirror_identified": G, "pilot": a.pilot, "mean_samples": a.mean_samples, "seed": a.seed,
            "samples_total": int(n_used.sum()), "prepare_s": t_prep, "run_s": t_run, "samples_per_s": float(n_used.sum()) / t_run,
            "total": total, "sigma": math.sqrt(tvar), "sigma2_time_s": tvar * t_run, "sigma_equal_cost_split_same_budget": math.sqrt(var_equal),
            "variance_gain_of_allocation": var_equal / tvar if tvar > 0 else None, "flagged_fraction": float(flagged.sum() / n_used.sum()),

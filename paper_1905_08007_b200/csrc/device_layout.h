@@ -85,6 +85,10 @@ struct DevHeader {
   int64_t off_stream, stream_chunks;      // the family streams: stream_chunks chunks of MQ_CHUNK_WORDS words
   int32_t rng, pad0;                      // 0 = Philox4x32-10, 1 = MRG32k3a (mc_options.flags bit 2)
   int64_t off_mrg;                        // rng = 1: [2][64][9] uint32, the powers A^(2^k) mod m of the two companion matrices (row-major)
+  // defensive mixture (mc_options.mix_alpha > 0; S5b): the second channel's Z, 1/Deg and normalisation, and Deg of BOTH
+  // channels (the density of the channel that did not draw the point needs t^Deg_other); all arrays 2^M doubles
+  double mix_alpha, C2;
+  int64_t off_Z2, off_invdeg2, off_deg1, off_deg2;
 };
 
 // Stream entry = MQ_WL families of the SAME shape (c, kd), evaluated side by side by the MQ_WL lanes that share a

@@ -47,7 +47,7 @@ struct McWorkspace {
 struct mc_diagram {
   mq::VertexGraph g;
   mq::ForestTerms ft;
-  mq::SamplerTables st;
+  mq::SamplerTables st, st2;               // st2: the second channel of the defensive mixture (empty when off)
   mc_options opt{};
   double dd_cond_max = 1e26, w_abs_tol = 1e-10;   // mc_diagram_set_precision
   mqk::MqPrec prec(bool no_dd) const {    // no_dd: nothing but non-finite points is handed on

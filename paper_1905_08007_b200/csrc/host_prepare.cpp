@@ -57,8 +57,10 @@ struct Builder {
 int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_options *opts, bool use_gpu, mc_diagram **out) {
   if (!graph || !out) return MC_EINVAL;
   std::unique_ptr<mc_diagram> d(new mc_diagram);
-  d->opt = opts ? *opts : mc_options{1.0, 1e30, 2.8e4, 1e-2, 0u, 0.5};
+  d->opt = opts ? *opts : mc_options{1.0, 1e30, 2.8e4, 1e-2, 0u, 0.5, 0.0, 0.0, 0.0};
   if (!(d->opt.deg_floor > 0) || !(d->opt.deg_cap >= d->opt.deg_floor) || !(d->opt.cond_max > 0)) return MC_EINVAL;
+  if (!(d->opt.mix_alpha >= 0.0 && d->opt.mix_alpha < 1.0)) return MC_EINVAL;
+  if (d->opt.mix_alpha > 0.0 && !(d->opt.deg_floor2 > 0 && d->opt.deg_cap >= d->opt.deg_floor2)) return MC_EINVAL;
   if (!d->g.build(graph->loops, graph->ext_pos, graph->chord_a, graph->chord_b)) return MC_EINVAL;
   d->id = d->g.canonicalId();
   if (d->id < 0) return MC_EINVAL;
@@ -69,6 +71,7 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
     for (int i = 0; i < uf->n_forest; i++) if (uf->forest_mask[i] != d->ft.forests[i]) return MC_EINVAL;
   }
   d->st.build(d->g, d->ft, d->opt.deg_floor, d->opt.deg_cap, d->opt.deg_floor_ir);
+  if (d->opt.mix_alpha > 0.0) d->st2.build(d->g, d->ft, d->opt.deg_floor2, d->opt.deg_cap, d->opt.deg_floor_ir2);
 
   // ---- term trees -> unique pieces (geoms) and nodes ----
   Builder B(*d);
@@ -171,6 +174,10 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   H.off_table = off; off += words(sizeof(DevTable) * d->tables.size());
   H.off_node = off; off += words(sizeof(DevNode) * d->nodes.size());
   H.off_term = off; off += words(sizeof(DevTerm) * d->terms.size());
+  if (d->opt.mix_alpha > 0.0) {
+    H.mix_alpha = d->opt.mix_alpha; H.C2 = d->st2.C;
+    H.off_Z2 = off; off += nZ; H.off_invdeg2 = off; off += nZ; H.off_deg1 = off; off += nZ; H.off_deg2 = off; off += nZ;
+  }
   // MRG32k3a (mc_options.flags bit 2, S1b): the powers A^(2^k), k < 64, of the companion matrices of
   // x1_n = (1403580 x1_{n-2} - 810728 x1_{n-3}) mod m1 and x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod m2, acting on
   // (x_{n-3}, x_{n-2}, x_{n-1}); the kernels reach a sample's position in the sequence with one matrix-vector product per set bit
@@ -306,6 +313,12 @@ int mq_prepare_host(const mc_graph *graph, const mc_forests *uf, const mc_option
   std::memcpy(d->blob.data() + H.off_node, d->nodes.data(), sizeof(DevNode) * d->nodes.size());
   std::memcpy(d->blob.data() + H.off_term, d->terms.data(), sizeof(DevTerm) * d->terms.size());
   if (!mrg_pow.empty()) std::memcpy(d->blob.data() + H.off_mrg, mrg_pow.data(), sizeof(uint32_t) * mrg_pow.size());
+  if (d->opt.mix_alpha > 0.0) {
+    std::memcpy(d->blob.data() + H.off_Z2, d->st2.Z.data(), sizeof(double) * nZ);
+    std::memcpy(d->blob.data() + H.off_invdeg2, d->st2.invdeg.data(), sizeof(double) * nZ);
+    std::memcpy(d->blob.data() + H.off_deg1, d->st.deg.data(), sizeof(double) * nZ);
+    std::memcpy(d->blob.data() + H.off_deg2, d->st2.deg.data(), sizeof(double) * nZ);
+  }
   if (!streams.empty()) std::memcpy(d->blob.data() + stream_base, streams.data(), sizeof(uint64_t) * streams.size());
   d->have_tables = !no_tables;
   *out = d.release();

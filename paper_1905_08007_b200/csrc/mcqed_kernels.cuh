@@ -160,7 +160,23 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
   uint32_t ws[4], wr[4];
   const bool mrg = v.h->rng != 0;                      // the same for every point of a launch: no divergence
   double um[2 * MQ_MAXM];
-  if (mrg) mrg32k3a_uniforms(reinterpret_cast<const uint32_t *>(v.blob + v.h->off_mrg), seed, (((uint64_t)dg << 38) + idx) << 6, 2 * (M - 1), um);
+  // defensive mixture (S5b): uniform number 2(M-1) picks the channel that draws the point; the other channel's density at
+  // the point is prod t_l^Deg_other, accumulated in pq. The same for every point of a launch when off (alpha = 0): no divergence.
+  const double alpha = v.h->mix_alpha;
+  const bool mix = alpha > 0.0;
+  if (mrg) mrg32k3a_uniforms(reinterpret_cast<const uint32_t *>(v.blob + v.h->off_mrg), seed, (((uint64_t)dg << 38) + idx) << 6, 2 * (M - 1) + (mix ? 1 : 0), um);
+  const double *Zt = v.Z, *idg = v.invdeg, *dgo = nullptr;
+  double Cd = v.h->C, Co = 0.0, pq = 1.0;
+  bool alt = false;
+  if (mix) {
+    double uc;
+    if (mrg) uc = um[2 * (M - 1)];
+    else { uint32_t wc[4]; philox4x32_10(i0, i1, (uint32_t)(M - 1), dg, k0, k1, wc); uc = u01(wc[0], wc[1]); }
+    alt = uc < alpha;
+    const double *b = reinterpret_cast<const double *>(v.blob);
+    if (alt) { Zt = b + v.h->off_Z2; idg = b + v.h->off_invdeg2; dgo = b + v.h->off_deg1; Cd = v.h->C2; Co = v.h->C; }
+    else { dgo = b + v.h->off_deg2; Co = v.h->C2; }
+  }
   for (int l = 0; l < M; l++) {
     int x;
     if (l == M - 1) x = __ffs(mask) - 1;
@@ -168,11 +184,11 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
       if (!mrg && (l & 1) == 0) philox4x32_10(i0, i1, (uint32_t)(l >> 1), dg, k0, k1, ws);
       double u = mrg ? um[l] : (l & 1) ? u01(ws[2], ws[3]) : u01(ws[0], ws[1]);
       double total = 0.0;
-      for (uint32_t mm = mask; mm; mm &= mm - 1) { int y = __ffs(mm) - 1; total = __dadd_rn(total, __ldg(&v.Z[mask & ~(1u << y)])); }
+      for (uint32_t mm = mask; mm; mm &= mm - 1) { int y = __ffs(mm) - 1; total = __dadd_rn(total, __ldg(&Zt[mask & ~(1u << y)])); }
       double target = __dmul_rn(u, total), cum = 0.0;
       x = -1; int last = -1;
       for (uint32_t mm = mask; mm; mm &= mm - 1) {
-        int y = __ffs(mm) - 1; cum = __dadd_rn(cum, __ldg(&v.Z[mask & ~(1u << y)])); last = y;
+        int y = __ffs(mm) - 1; cum = __dadd_rn(cum, __ldg(&Zt[mask & ~(1u << y)])); last = y;
         if (target < cum) { x = y; break; }
       }
       if (x < 0) x = last;
@@ -181,8 +197,10 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
       int ru = (M - 1) + (l - 1);
       if (!mrg && ((ru & 1) == 0 || l == 1)) philox4x32_10(i0, i1, (uint32_t)(ru >> 1), dg, k0, k1, wr);
       double u = mrg ? um[ru] : (ru & 1) ? u01(wr[2], wr[3]) : u01(wr[0], wr[1]);
-      double t = det_exp2(__dmul_rn(det_log2(u), __ldg(&v.invdeg[mask])));
+      const double lg = __dmul_rn(det_log2(u), __ldg(&idg[mask]));
+      double t = det_exp2(lg);
       rl = __dmul_rn(rl, t); pu = __dmul_rn(pu, u);
+      if (mix) pq = __dmul_rn(pq, det_exp2(__dmul_rn(lg, __ldg(&dgo[mask]))));
     }
     r[l] = rl; ord[l] = (int8_t)x;
     mask &= ~(1u << x);
@@ -191,7 +209,11 @@ __device__ __forceinline__ double draw_point(const DiagView &v, uint64_t idx, ui
   for (int l = 0; l < M; l++) S = __dadd_rn(S, r[l]);
   double pz = 1.0;
   for (int l = 0; l < M; l++) { double zz = __ddiv_rn(r[l], S); z[ord[l]] = zz; pz = __dmul_rn(pz, zz); if (WANT_ORDER) order_out[l] = ord[l]; }
-  return __ddiv_rn(__dmul_rn(v.h->C, pu), pz);
+  const double p_drawn = __ddiv_rn(__dmul_rn(Cd, pu), pz);
+  if (!mix) return p_drawn;
+  const double p_other = __ddiv_rn(__dmul_rn(Co, pq), pz);
+  const double p_main = alt ? p_other : p_drawn, p_alt = alt ? p_drawn : p_other;
+  return __dadd_rn(__dmul_rn(__dadd_rn(1.0, -alpha), p_main), __dmul_rn(alpha, p_alt));
 }
 
 // ------------------------------------------------------------------ shared-memory helpers (explicit LDS) and the stream reader

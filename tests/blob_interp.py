@@ -11,7 +11,8 @@ MAXL, MAXSLOT, MAXCHILD, NGRADE = 5, 14, 5, 6
 HDR = np.dtype([("L", "<i4"), ("M", "<i4"), ("diag_id", "<i4"), ("ngeom", "<i4"), ("ntable", "<i4"), ("nnode", "<i4"), ("nterm", "<i4"),
                 ("nodeval_len", "<i4"), ("max_scal_len", "<i4"), ("wl", "<i4"), ("C", "<f8"), ("cond_max", "<f8"),
                 ("off_Z", "<i8"), ("off_invdeg", "<i8"), ("off_geom", "<i8"), ("off_table", "<i8"), ("off_node", "<i8"), ("off_term", "<i8"), ("total_words", "<i8"),
-                ("off_stream", "<i8"), ("stream_chunks", "<i8"), ("rng", "<i4"), ("pad0", "<i4"), ("off_mrg", "<i8")])
+                ("off_stream", "<i8"), ("stream_chunks", "<i8"), ("rng", "<i4"), ("pad0", "<i4"), ("off_mrg", "<i8"),
+                ("mix_alpha", "<f8"), ("C2", "<f8"), ("off_Z2", "<i8"), ("off_invdeg2", "<i8"), ("off_deg1", "<i8"), ("off_deg2", "<i8")])
 SLOT = np.dtype([("kind", "i1"), ("zline", "i1"), ("sgn", "i1"), ("child", "i1"), ("eps", "<u4")])
 GEOM = np.dtype([("nch", "<i4"), ("nslot", "<i4"), ("nchild", "<i4"), ("nS", "<i4"), ("chord_zline", "<i4", (MAXL,)), ("slot", SLOT, (MAXSLOT,)),
                  ("child_type", "i1", (MAXCHILD,)), ("child_patbit", "i1", (MAXCHILD,)), ("pad", "<i2"), ("first_table", "<i4"), ("ntable", "<i4"),
@@ -20,7 +21,7 @@ TABLE = np.dtype([("geom", "<i4"), ("op", "<i4"), ("nout", "<i4"), ("nfam", "<i4
                   ("stream_off", "<i8"), ("stream_words", "<i8"), ("n_monomials", "<i8")])
 NODE = np.dtype([("table", "<i4"), ("geom", "<i4"), ("nchild", "<i4"), ("nout", "<i4"), ("child", "<i4", (MAXCHILD,)), ("val_off", "<i4"), ("ngr", "<i4")])
 TERM = np.dtype([("root", "<i4"), ("sign", "<i4")])
-assert GEOM.itemsize == 184 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 144
+assert GEOM.itemsize == 184 and TABLE.itemsize == 48 and NODE.itemsize == 44 and HDR.itemsize == 192
 
 
 def pairings(n2):

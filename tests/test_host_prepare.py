@@ -167,3 +167,32 @@ def test_mrg32k3a_power_table_in_blob_equals_oracle(po, mc):
     h = np.frombuffer(d.blob().tobytes(), blob_interp.HDR, 1)[0]
     assert h["rng"] == 0 and h["off_mrg"] == 0
     d.close()
+
+
+def test_mixture_tables_in_blob_equal_oracle(po, mc):
+    """mc_options.mix_alpha > 0 (S5b): the blob carries the second channel's Z, 1/Deg, C and Deg of both channels; against the
+    oracle's tables built with the same floors. Off by default: no such sections."""
+    import blob_interp
+    g = po.graph_get(3, 17)
+    d = mc.Diagram(3, g.ext_pos, g.chords(), host_only=True, flags=mc.FLAG_NO_TABLES, mix_alpha=0.25, deg_floor2=0.6, deg_floor_ir2=0.4)
+    w = d.blob()
+    h = np.frombuffer(w.tobytes(), blob_interp.HDR, 1)[0]
+    n = 1 << 9
+    o1, o2 = po.Diagram(g, level=0), po.Diagram(g, level=0, deg_floor=0.6, deg_floor_ir=0.4)
+    deg1, Z1, C1 = o1.sampler_tables()
+    deg2, Z2, C2 = o2.sampler_tables()
+    sec = lambda off: w[int(off):int(off) + n].view(np.float64)
+    assert h["mix_alpha"] == 0.25 and h["C2"] == C2 and h["C"] == C1
+    assert np.array_equal(sec(h["off_Z"]), Z1) and np.array_equal(sec(h["off_Z2"]), Z2)
+    assert np.array_equal(sec(h["off_deg1"]), deg1) and np.array_equal(sec(h["off_deg2"]), deg2)
+    inv2 = sec(h["off_invdeg2"])
+    assert np.array_equal(inv2[1:n - 1], 1.0 / deg2[1:n - 1])
+    d.close()
+    d = mc.Diagram(3, g.ext_pos, g.chords(), host_only=True, flags=mc.FLAG_NO_TABLES)
+    h = np.frombuffer(d.blob().tobytes(), blob_interp.HDR, 1)[0]
+    assert h["mix_alpha"] == 0.0 and h["off_Z2"] == 0 and h["off_deg1"] == 0
+    d.close()
+    with pytest.raises(mc.McError):
+        mc.Diagram(3, g.ext_pos, g.chords(), host_only=True, flags=mc.FLAG_NO_TABLES, mix_alpha=1.0, deg_floor2=0.6)
+    with pytest.raises(mc.McError):
+        mc.Diagram(3, g.ext_pos, g.chords(), host_only=True, flags=mc.FLAG_NO_TABLES, mix_alpha=0.2, deg_floor2=0.0)

@@ -116,3 +116,37 @@ def test_deg_values(po):
     d3 = _diag(po, 2, 1, [(0, 3), (2, 4)], deg_floor=0.5)
     deg3, _, _ = d3.sampler_tables()
     assert deg3[0b010011] == 0.5
+
+
+def test_defensive_mixture_of_two_eq1_densities(po):
+    """DESIGN.md S5b: with probability alpha a point comes from a second Eq.(1) density and every weight is
+    divided by the mixture. Pins: the density returned with the point equals (1 - alpha) p1(z) + alpha p2(z) recomputed from z alone
+    (two separate table sets, sort + tail sets); the share of points that differ from the single-channel draw is alpha; the
+    Dirichlet closed form still comes out (unbiased); alpha = 0 restores the single-channel stream bit for bit."""
+    g = po.OracleGraph.make(3, 1, [(0, 6), (2, 3), (4, 5)])
+    d = po.Diagram(g, level=0)
+    d1 = po.Diagram(g, level=0)
+    d2 = po.Diagram(g, level=0, deg_floor=0.5, deg_floor_ir=0.35)
+    z0, p0, o0 = d.sample(0, 20000, 11)
+    alpha = 0.3
+    d.set_mixture(alpha, 0.5, 0.35)
+    z, p, order = d.sample(0, 20000, 11)
+    want = (1 - alpha) * d1.density(z) + alpha * d2.density(z)
+    assert np.allclose(p, want, rtol=1e-9) and np.allclose(d.density(z), want, rtol=1e-12)
+    moved = ~np.all(z == z0, axis=1)
+    assert abs(moved.mean() - alpha) < 4 * math.sqrt(alpha * (1 - alpha) / len(z))
+    assert np.array_equal(p[~moved] > p0[~moved] * (1 - alpha) * 0.999999, np.ones((~moved).sum(), bool))   # p >= (1 - alpha) p1 on the unmoved points
+    zs = np.take_along_axis(z, order.astype(np.int64), axis=1)
+    assert np.all(np.diff(zs, axis=1) <= 0) and np.allclose(z.sum(1), 1.0, rtol=0, atol=1e-14)
+    zz, pp, _ = d.sample(0, 200000, 17)
+    a = np.array([1.0, 0.0, 2.0, 0.5, 0.0, 1.0, 0.0, 0.25, 1.0])
+    w = np.prod(zz ** a, axis=1) / pp
+    exact = math.exp(sum(math.lgamma(x + 1) for x in a) - math.lgamma(a.sum() + d.M))
+    assert abs(w.mean() - exact) < 5 * w.std() / math.sqrt(len(w))
+    d.set_generator(1)                                                       # the channel uniform on the MRG32k3a stream: outputs 4(M-1), 4(M-1)+1
+    zm, pm, _ = d.sample(0, 20000, 11)
+    assert np.allclose(pm, (1 - alpha) * d1.density(zm) + alpha * d2.density(zm), rtol=1e-9)
+    d.set_generator(0)
+    d.set_mixture(0.0, 1.0)
+    z1, p1, o1 = d.sample(0, 20000, 11)
+    assert np.array_equal(z1, z0) and np.array_equal(p1, p0) and np.array_equal(o1, o0)
