@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--no-second-policy", action="store_true", help="skip the timed step under the purely relative precision policy (w_abs_tol = 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--deg-floor", type=float, default=None, help="Deg floor of Eq.(1) (default: the library's, 1.0)")
+    ap.add_argument("--mix", type=float, nargs=3, default=None, metavar=("ALPHA", "FLOOR2", "FLOOR_IR2"), help="defensive mixture of two Eq.(1) densities (DESIGN.md S5b; default: off)")
     ap.add_argument("--deg-floor-ir", type=float, default=None, help="Deg on the soft-photon sets (default: the library's, 0.5)")
     return ap.parse_args()
 
@@ -147,7 +148,8 @@ def run_ours(args):
     G, B = len(graphs), args.batch
     # ---- prepare (not timed as throughput; reported) ----
     t0 = time.perf_counter()
-    diagrams = [mc.Diagram(g[0], g[1], g[2], deg_floor=args.deg_floor, deg_floor_ir=args.deg_floor_ir) for _, g in graphs]
+    mix = {} if args.mix is None else {"mix_alpha": args.mix[0], "deg_floor2": args.mix[1], "deg_floor_ir2": args.mix[2]}
+    diagrams = [mc.Diagram(g[0], g[1], g[2], deg_floor=args.deg_floor, deg_floor_ir=args.deg_floor_ir, **mix) for _, g in graphs]
     prepare_s = time.perf_counter() - t0
     infos = [d.info() for d in diagrams]
     flop = [i["flop_per_sample"] for i in infos]
