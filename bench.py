@@ -14,7 +14,6 @@ import math
 import os
 import subprocess
 import sys
-import threading
 import time
 
 import numpy as np
@@ -45,24 +44,41 @@ def parse():
     return ap.parse_args()
 
 
-class ClockSampler(threading.Thread):
-    """samples nvidia-smi clocks and throttle reasons during the timed region"""
+class ClockSampler:
+    """samples nvidia-smi clocks and throttle reasons during the timed region: ONE looping nvidia-smi process (-lms 200, the
+    profiling recipe's form), started and past its NVML set-up before the timed region begins and killed after it, so that
+    no process start and no driver attach falls into the timed steps"""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, index):
-        super().__init__(daemon=True)
-        self.index, self.rows, self.stop_flag = index, [], False
+        self.index, self.rows, self.proc, self.log = index, [], None, None
 
-    def run(self):
-        while not self.stop_flag:
+    def start(self):
+        import tempfile
+        try:
+            self.log = tempfile.NamedTemporaryFile(prefix="mcqed_clocks_", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=self.log, stderr=subprocess.DEVNULL)
+            t0 = time.perf_counter()
+            while os.path.getsize(self.log.name) == 0 and time.perf_counter() - t0 < 5.0 and self.proc.poll() is None:
+                time.sleep(0.05)                 # first row written = set-up done
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
             try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
-                                     capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([x.strip() for x in out.split(",")])
+                self.proc.wait(timeout=5)
             except Exception:
-                pass
-            time.sleep(0.2)
+                self.proc.kill()
+        if self.log is not None:
+            self.log.close()
+            with open(self.log.name) as fh:
+                self.rows = [[x.strip() for x in ln.split(",")] for ln in fh if ln.count(",") >= 5]
+            os.unlink(self.log.name)
+        if len(self.rows) > 2:
+            self.rows = self.rows[1:]            # the row written before the timed region began
 
     def summary(self):
         sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
@@ -192,8 +208,7 @@ def run_ours(args):
     l0 = mc.kernel_launch_count()
     ms = timed(args.steps)
     launches = mc.kernel_launch_count() - l0
-    clocks.stop_flag = True
-    clocks.join(timeout=2)
+    clocks.stop()
     n_tot = args.steps * B
     s = sums.cpu().numpy(); c = cnts.cpu().numpy()
     value = world * G * n_tot / (ms * 1e-3)
