@@ -34,7 +34,9 @@ def parse():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (4 = the metric's workload)")
     ap.add_argument("--graphs", type=int, default=0, help="use only the first G graphs of the config (0 = all; for debugging)")
     ap.add_argument("--batch", type=int, default=37888, help="sample points per diagram per step")
-    ap.add_argument("--ref-points", type=int, default=384, help="oracle sample points per graph and step (reference arm / cpu_baseline)")
+    ap.add_argument("--ref-points", type=int, default=384, help="oracle sample points per graph and step, at most (reference arm / cpu_baseline)")
+    ap.add_argument("--ref-seconds", type=float, default=150.0, help="reference arm: oracle work of the whole --steps/--warmup run, seconds (the points per step are cut to fit)")
+    ap.add_argument("--cpu-seconds", type=float, default=25.0, help="cpu_baseline leg of the default run: oracle work of its one timed step, seconds")
     ap.add_argument("--ref-graphs", type=int, default=3, help="graphs of the workload the oracle is timed on, spread over the set")
     ap.add_argument("--no-second-policy", action="store_true", help="skip the timed step under the purely relative precision policy (w_abs_tol = 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -91,40 +93,48 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2] if sm else 0, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_run(args, graphs, seed, steps, warmup):
+def oracle_run(args, graphs, seed, steps, warmup, budget_s):
     """times the CPU oracle as it stands on a bounded sample of the workload: --ref-graphs graphs spread evenly over the set
-    (the set is sorted by canonical index = by external-vertex position, so the sample spans the gauge classes), --ref-points
-    points per graph and step, after one untimed warm-up pass per graph"""
+    (the set is sorted by canonical index = by external-vertex position, so the sample spans the gauge classes), the same n
+    points per graph and step for every graph. n is --ref-points, cut down so that the timed steps and the warm-up steps
+    together take about budget_s seconds: the first warm-up pass of every graph (32 points) is timed for that estimate."""
     from oracle import pyoracle as po
     from paper_1905_08007_b200 import workloads
     G = len(graphs)
     pick = sorted(set(int(round(k * (G - 1) / max(1, args.ref_graphs - 1))) for k in range(args.ref_graphs))) if args.ref_graphs > 1 else [0]
-    n = args.ref_points
-    prep = dt = 0.0
-    var = 0.0
-    classes = []
+    n0 = min(32, args.ref_points)
+    prep = 0.0
+    ds, spp, classes = [], 0.0, []
     for gi in pick:
         idx, g = graphs[gi]
         t0 = time.perf_counter()
         d = po.Diagram(po.OracleGraph.make(g[0], g[1], g[2]))
         prep += time.perf_counter() - t0
-        for w in range(max(1, warmup)):
-            d.integrate(w * n, n, seed, 2)
+        t0 = time.perf_counter()
+        d.integrate(0, n0, seed, 2)                       # warm-up pass 1 = the pilot
+        spp += (time.perf_counter() - t0) / n0
+        ds.append(d)
+        classes.append("%d,%d,%d" % workloads.graph_class(g))
+    passes = steps + max(0, warmup - 1)
+    n = int(max(16, min(args.ref_points, budget_s / (passes * spp))))
+    dt = var = 0.0
+    for d in ds:
+        for w in range(max(0, warmup - 1)):
+            d.integrate(n0 + w * n, n, seed, 2)
         t0 = time.perf_counter()
         s1 = s2 = 0.0
         for k in range(steps):
-            a, b, _ = d.integrate((max(1, warmup) + k) * n, n, seed, 2)
+            a, b, _ = d.integrate(n0 + (max(0, warmup - 1) + k) * n, n, seed, 2)
             s1 += a
             s2 += b
         dt += time.perf_counter() - t0
         mean, err = po.estimate(s1, s2, n * steps)
         var += err * err
-        classes.append("%d,%d,%d" % workloads.graph_class(g))
-        del d
+    del ds
     tot = n * steps * len(pick)
     return {"value": tot / dt, "seconds": dt, "cores": po.num_threads(), "prepare_s": prep, "points": tot,
-            "sample": "graphs #%s of the workload (classes %s), %d points per graph and step, %d step(s) after a warm-up pass, binary64 + __float128 re-evaluation" % (
-                ",".join(str(x) for x in pick), " ".join(classes), n, steps),
+            "sample": "graphs #%s of the workload (classes %s), %d points per graph and step (sized for about %.0f s of oracle work), %d timed step(s) after %d warm-up pass(es), binary64 + __float128 re-evaluation" % (
+                ",".join(str(x) for x in pick), " ".join(classes), n, budget_s, steps, max(1, warmup)),
             "sigma2_time": var * dt}
 
 
@@ -135,7 +145,7 @@ def run_reference(args):
     from paper_1905_08007_b200 import workloads
     graphs = workloads.config_graphs(args.config)
     seed = workloads.CONFIG_SEED[args.config]
-    r = oracle_run(args, graphs, seed, max(1, args.steps), args.warmup)
+    r = oracle_run(args, graphs, seed, max(1, args.steps), args.warmup, args.ref_seconds)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * r["seconds"] / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": {"workload": "configs[%d] (bounded sample)" % args.config, "sample": r["sample"]},
@@ -352,7 +362,7 @@ def run_ours(args):
                        "algorithmic_flop_per_sample_mean": sum(flop) / G, "classes": classes},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = oracle_run(args, graphs, seed, 1, 1)
+        r = oracle_run(args, graphs, seed, 1, 1, args.cpu_seconds)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
                                 "prepare_s": r["prepare_s"], "sigma2_time_s": r["sigma2_time"]}
     if rank == 0:
