@@ -238,15 +238,17 @@ def run_ours(args):
         e["sigma"] = math.sqrt(e.pop("var"))
     # ---- per-kernel times: the same steps with the higher tiers switched off (flags bit 0: binary64 kernel alone;
     #      bit 1: no quad-double pass); the double-double and quad-double kernels are timed as the differences ----
-    state["flags"] = mc.FLAG_NO_DD
+    keep = (sums.clone(), cnts.clone())           # the sums of the timed region: the legs below add to them and are undone (with bit 0 set
+    state["flags"] = mc.FLAG_NO_DD                # the ill-conditioned points keep their binary64 values, which must not reach the tail diagnostic)
     step()
-    ms_f64 = timed(args.steps)
+    nk = min(args.steps, 5)                      # the per-kernel legs time at most 5 steps and are scaled to args.steps
+    sc = args.steps / nk
+    ms_f64 = timed(nk) * sc
     state["flags"] = mc.FLAG_NO_QD
-    keep = (sums.clone(), cnts.clone())
     step()
     cnts.zero_()
-    ms_noqd = timed(args.steps)
-    n_qd = float(cnts[1].sum().item())           # with the quad-double pass skipped its points are counted as dropped
+    ms_noqd = timed(nk) * sc
+    n_qd = float(cnts[1].sum().item()) * sc           # with the quad-double pass skipped its points are counted as dropped
     sums.copy_(keep[0]); cnts.copy_(keep[1])
     state["flags"] = 0
     ms_dd = max(ms_noqd - ms_f64, 0.0)
@@ -282,7 +284,7 @@ def run_ours(args):
     #      the timed region, with a snapshot after each (heavy-tailed weights show up as a growing sigma*sqrt(N)) ----
     keep2 = (sums.clone(), cnts.clone())
     trace = []
-    for k in range(max(2, args.steps)):
+    for k in range(min(4, max(2, args.steps))):
         step()
         torch.cuda.synchronize()
         nn = n_tot + (k + 1) * B
